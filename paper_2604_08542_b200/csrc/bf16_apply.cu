@@ -1,0 +1,253 @@
+// bf16_apply.cu — fused tensor-core apply kernel (steps 9-11 of the hot path):
+//   O = ( SiLU(Q W1) o (Q W3) ) W2        Eq. 4 with Eq. 12, updated weights.
+//
+// Formulation ("tokens on lanes"): a CTA owns one head and a strided set of 128-token tiles.
+//   Q tile  -> TMEM as the A operand (bf16, [128 tokens x hd]), written by the I/O warpgroup
+//   step n  (64 hidden units):  Aq = Q W1[:, n], Bq = Q W3[:, n]   MMA 128 x 64 x hd, B = weights (K-major)
+//            epilogue  Hq = SiLU(Aq) o Bq -> bf16 -> TMEM over its own fp32 source
+//            O += Hq W2[n, :]                                      MMA 128 x hd x 64, B = W2 slice (MN-major)
+//   O (fp32, TMEM) -> bf16 -> global by the I/O warpgroup.
+// The bf16 weights of the head (3 x H x hd) sit in shared memory for the CTA's lifetime (TMA, 128-B
+// swizzle). Forward accumulators, Q operands and O accumulators are double-buffered in TMEM, so the
+// MMA of step n+1 overlaps the SwiGLU epilogue of step n, and Q loads / O stores overlap both.
+//
+// Warp roles (512 threads): warp 0 = TMA (weights, once), warp 1 = MMA issuer, warps 4-7 / 8-11 =
+// two epilogue warpgroups alternating steps, warps 12-15 = I/O warpgroup (Q in, O out).
+#include "tc_common.cuh"
+#include "ttt_internal.h"
+
+namespace ttt {
+
+int make_token_map(ttt_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int64_t cols,
+                   int64_t ld, int box_rows);  // bf16_update.cu
+
+namespace app {
+constexpr int TM = 128;        // tokens per tile (MMA M)
+constexpr int NS = 64;         // hidden units per step
+constexpr int THREADS = 512;
+// TMEM column plan for hd = 64
+constexpr uint32_t C_Q = 0;      // 2 x 32 cols: Q operand (bf16)
+constexpr uint32_t C_O = 64;     // 2 x 64 cols: O accumulator (fp32)
+constexpr uint32_t C_F = 192;    // 2 x 128 cols: Aq (64) | Bq (64) forward accumulators (fp32)
+}  // namespace app
+
+__device__ __forceinline__ float fast_sigmoid_app(float a) {
+#if !defined(TTT_SIGMOID_TANH) || TTT_SIGMOID_TANH
+  float th;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(th) : "f"(0.5f * a));
+  return fmaf(0.5f, th, 0.5f);
+#else
+  float e, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(a * -1.4426950408889634f));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
+  return r;
+#endif
+}
+
+__global__ void __launch_bounds__(app::THREADS, 1)
+bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __nv_bfloat16* __restrict__ Q,
+                  __nv_bfloat16* __restrict__ O, int M, long ld, int nh, int H, int tiles_total) {
+  using namespace app;
+  constexpr int HD = 64;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) &
+                                             ~static_cast<uintptr_t>(1023));
+  __shared__ uint64_t w_full, fwd_full[2], epi_done[2], q_full[2], q_empty[2], o_full[2], o_empty[2];
+  __shared__ uint32_t tmem_base_s;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int h = blockIdx.y;
+  const int nsl = H / NS;                                    // steps per tile
+  // tiles of this CTA: blockIdx.x, blockIdx.x + gridDim.x, ...
+  const int my_tiles = (tiles_total - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  const int total_steps = my_tiles * nsl;
+  const uint32_t w_bytes = 3u * H * 128u;                    // bf16 weights of the head
+
+  if (tid == 0) {
+    mbar_init(&w_full, 1);
+    for (int b = 0; b < 2; ++b) {
+      mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 128);
+      mbar_init(&q_full[b], 128); mbar_init(&q_empty[b], 1);
+      mbar_init(&o_full[b], 1);   mbar_init(&o_empty[b], 128);
+    }
+    fence_mbar_init();
+  }
+  if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tb = tmem_base_s;
+
+  if (warp == 0) {
+    // ===================== TMA: the head's weights, once =====================
+    if (elect_one() && my_tiles > 0) {
+      tma_prefetch_desc(&mapW);
+      mbar_arrive_expect_tx(&w_full, w_bytes);
+      // smem: [mat][H rows][128 B]; boxes of 64 rows (8 KB)
+      for (int mat = 0; mat < 3; ++mat)
+        for (int r = 0; r < H; r += 64)
+          tma_load_2d_hint(smem + ((size_t)mat * H + r) * 128, &mapW, &w_full, 0,
+                           (mat * nh + h) * H + r, kEvictLast);
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (elect_one() && my_tiles > 0) {
+      constexpr uint32_t idesc_f = umma_idesc_bf16(TM, NS, 0, 0);   // B = W1^T / W3^T rows, K-major
+      constexpr uint32_t idesc_d = umma_idesc_bf16(TM, HD, 0, 1);   // B = W2 rows, MN-major
+      const uint32_t w1s = smem_u32(smem), w2s = w1s + H * 128, w3s = w2s + H * 128;
+      mbar_wait(&w_full, 0);
+      tc_fence_after();
+      auto fwd = [&](int st) {
+        const int tl = st / nsl, n = st - tl * nsl, fb = st & 1, qb = tl & 1;
+        if (n == 0) { mbar_wait(&q_full[qb], (tl >> 1) & 1); tc_fence_after(); }
+        const uint32_t acc = tb + C_F + fb * 128, qop = tb + C_Q + qb * 32;
+        const uint32_t b1 = w1s + n * (NS * 128), b3 = w3s + n * (NS * 128);
+#pragma unroll
+        for (int k = 0; k < HD / 16; ++k)
+          umma_ts(acc, qop + 8 * k, umma_smem_desc_sw128(b1 + 32 * k, 16, 1024), idesc_f, k > 0);
+#pragma unroll
+        for (int k = 0; k < HD / 16; ++k)
+          umma_ts(acc + 64, qop + 8 * k, umma_smem_desc_sw128(b3 + 32 * k, 16, 1024), idesc_f, k > 0);
+        tc_commit(&fwd_full[fb]);
+        if (n == nsl - 1) tc_commit(&q_empty[qb]);
+      };
+      auto down = [&](int st) {
+        const int tl = st / nsl, n = st - tl * nsl, fb = st & 1, ob = tl & 1;
+        mbar_wait(&epi_done[fb], (st >> 1) & 1);
+        if (n == 0) mbar_wait(&o_empty[ob], ((tl >> 1) & 1) ^ 1);
+        tc_fence_after();
+        const uint32_t hq = tb + C_F + fb * 128, oacc = tb + C_O + ob * 64;
+        const uint32_t b2 = w2s + n * (NS * 128);
+#pragma unroll
+        for (int k = 0; k < NS / 16; ++k)
+          umma_ts(oacc, hq + 8 * k, umma_smem_desc_sw128(b2 + 2048 * k, 8192, 1024), idesc_d,
+                  (n > 0 || k > 0));
+        if (n == nsl - 1) tc_commit(&o_full[ob]);
+      };
+      fwd(0);
+      for (int st = 0; st < total_steps; ++st) {
+        if (st + 1 < total_steps) fwd(st + 1);
+        down(st);
+      }
+    }
+  } else if (warp >= 4 && warp < 12) {
+    // ===================== SwiGLU epilogue warpgroups =====================
+    const int wg = (warp - 4) >> 2, q = warp & 3;
+    const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
+    for (int st = wg; st < total_steps; st += 2) {
+      const int fb = st & 1;
+      const uint32_t buf = tb + lane_base + C_F + fb * 128;
+      mbar_wait(&fwd_full[fb], (st >> 1) & 1);
+      tc_fence_after();
+#pragma unroll
+      for (int part = 0; part < 4; ++part) {     // 16 hidden columns at a time
+        uint32_t ra[16], rb[16];
+        tmem_ld_x16(buf + 16 * part, ra);
+        tmem_ld_x16(buf + 64 + 16 * part, rb);
+        tc_wait_ld();
+        uint32_t ph[8];
+#pragma unroll
+        for (int c = 0; c < 16; c += 2) {
+          const float a0 = __uint_as_float(ra[c]), a1 = __uint_as_float(ra[c + 1]);
+          const float h0 = a0 * fast_sigmoid_app(a0) * __uint_as_float(rb[c]);
+          const float h1 = a1 * fast_sigmoid_app(a1) * __uint_as_float(rb[c + 1]);
+          ph[c >> 1] = pack_bf16x2(h0, h1);
+        }
+        tmem_st_x8(buf + 8 * part, ph);          // Hq (bf16) over the first 32 columns of Aq
+      }
+      tc_wait_st();
+      tc_fence_before();
+      mbar_arrive(&epi_done[fb]);
+    }
+  } else if (warp >= 12) {
+    // ===================== I/O warpgroup: Q rows in, O rows out =====================
+    const int q = warp & 3;
+    const int r = q * 32 + lane;                               // token row within the tile
+    const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
+    auto load_q = [&](int tl) {
+      const int qb = tl & 1;
+      const long t = (long)(blockIdx.x + (long)tl * gridDim.x) * TM + r;
+      uint32_t w[32];
+      if (t < M) {
+        const uint4* src = reinterpret_cast<const uint4*>(Q + t * ld + (size_t)h * HD);
+#pragma unroll
+        for (int v = 0; v < 8; ++v) {
+          const uint4 x = __ldg(src + v);
+          w[4 * v] = x.x; w[4 * v + 1] = x.y; w[4 * v + 2] = x.z; w[4 * v + 3] = x.w;
+        }
+      } else {
+#pragma unroll
+        for (int v = 0; v < 32; ++v) w[v] = 0u;
+      }
+      mbar_wait(&q_empty[qb], ((tl >> 1) & 1) ^ 1);
+      tc_fence_after();
+      tmem_st_x32(tb + lane_base + C_Q + qb * 32, w);
+      tc_wait_st();
+      tc_fence_before();
+      mbar_arrive(&q_full[qb]);
+    };
+    auto store_o = [&](int tl) {
+      const int ob = tl & 1;
+      const long t = (long)(blockIdx.x + (long)tl * gridDim.x) * TM + r;
+      mbar_wait(&o_full[ob], (tl >> 1) & 1);
+      tc_fence_after();
+      uint4* dst = reinterpret_cast<uint4*>(O + t * ld + (size_t)h * HD);
+#pragma unroll
+      for (int half = 0; half < 2; ++half) {
+        uint32_t ro[32];
+        tmem_ld_x32(tb + lane_base + C_O + ob * 64 + 32 * half, ro);
+        tc_wait_ld();
+        if (t < M) {
+#pragma unroll
+          for (int v = 0; v < 4; ++v) {
+            uint4 x;
+            x.x = pack_bf16x2(__uint_as_float(ro[8 * v]), __uint_as_float(ro[8 * v + 1]));
+            x.y = pack_bf16x2(__uint_as_float(ro[8 * v + 2]), __uint_as_float(ro[8 * v + 3]));
+            x.z = pack_bf16x2(__uint_as_float(ro[8 * v + 4]), __uint_as_float(ro[8 * v + 5]));
+            x.w = pack_bf16x2(__uint_as_float(ro[8 * v + 6]), __uint_as_float(ro[8 * v + 7]));
+            dst[4 * half + v] = x;
+          }
+        }
+      }
+      tc_fence_before();
+      mbar_arrive(&o_empty[ob]);
+    };
+    if (my_tiles > 0) load_q(0);
+    if (my_tiles > 1) load_q(1);
+    for (int tl = 0; tl < my_tiles; ++tl) {
+      store_o(tl);
+      if (tl + 2 < my_tiles) load_q(tl + 2);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tb, 512);
+}
+
+// ------------------------------------------------------------------------------------------------
+int bf16_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
+               cudaStream_t s) {
+  const ttt_config& c = ctx->cfg;
+  const int tiles = (int)((M + app::TM - 1) / app::TM);
+  int per_head = ctx->sm_count / c.nh;
+  if (per_head < 1) per_head = 1;
+  if (per_head > tiles) per_head = tiles;
+  CUtensorMap mapW;
+  int rc = make_token_map(ctx, &mapW, ctx->Wb, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, 64);
+  if (rc != TTT_OK) return rc;
+  const size_t smem = (size_t)3 * c.hidden * 128 + 1024;
+  static size_t attr_smem = 0;
+  if (smem > attr_smem) {
+    TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_apply_kernel,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
+                 "bf16_apply_kernel smem attr");
+    attr_smem = smem;
+  }
+  dim3 grid(per_head, c.nh);
+  bf16_apply_kernel<<<grid, app::THREADS, smem, s>>>(mapW, Q, O, (int)M, (long)ld, c.nh, c.hidden,
+                                                     tiles);
+  TTT_LAUNCH_CHECK(ctx, "bf16_apply_kernel");
+  return TTT_OK;
+}
+
+}  // namespace ttt

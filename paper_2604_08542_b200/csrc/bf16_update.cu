@@ -1,0 +1,361 @@
+// bf16_update.cu — fused tensor-core gradient kernel of the TTT update (steps 1-5 of the hot path,
+// DESIGN.md "Kernels"; Eq. 8 with Eq. 9 and Eq. 12).
+//
+// Formulation ("hidden on lanes"): one CTA owns 128 hidden units of one head and a range of tokens.
+// Everything is computed TRANSPOSED so that each MMA has M = 128 hidden units on the TMEM lanes:
+//   forward   A^T  = W1^T K^T,  B^T = W3^T K^T,  g^T = W2 V^T      [128 x T]  (contract over hd)
+//   epilogue  s = sigmoid(A); S = A s; Hd = S B; dHd = -eta g
+//             dA = dHd B (s + S (1 - s)); dB = dHd S; Hd' = -eta Hd            (fp32 -> bf16)
+//   gradient  G1^T += dA^T K,  G3^T += dB^T K,  G2 += Hd'^T V      [128 x hd] (contract over tokens)
+// The A operand of every MMA lives in TMEM (weights: loaded once; dA/dB/Hd': written by the
+// epilogue over their own fp32 sources), the B operand is the K or V token tile that TMA put in
+// shared memory with the 128-byte swizzle; the SAME tile serves the forward MMA as a K-major
+// operand and the gradient MMA as an MN-major operand. Gradient accumulators stay in TMEM for the
+// CTA's whole token range; one fp32 partial per CTA goes to HBM/L2 and is summed in a fixed order
+// by the commit kernel (deterministic, no float atomics).
+//
+// Warp roles (384 threads): warp 0 = TMA producer, warp 1 = MMA issuer, warps 4-7 / 8-11 = two
+// epilogue warpgroups that alternate token tiles (TMEM accumulators are double-buffered).
+#include <stdio.h>
+
+#include "tc_common.cuh"
+#include "ttt_internal.h"
+
+namespace ttt {
+
+namespace upd {
+constexpr int HS = 128;        // hidden units per CTA (MMA M)
+constexpr int T = 32;          // tokens per tile (forward MMA N, gradient MMA K)
+constexpr int STAGES = 6;      // K/V shared-memory ring
+constexpr int THREADS = 384;
+constexpr int TILE_BYTES = T * 128;  // one [T x 64] bf16 tile
+
+// TMEM column plan for hd = 64 (512 columns x 128 lanes x 32 bit)
+constexpr uint32_t C_W1 = 0, C_W3 = 32, C_W2 = 64;        // bf16 weights as A operands, 32 cols each
+constexpr uint32_t C_G1 = 96, C_G3 = 160, C_G2 = 224;     // fp32 gradient accumulators, 64 cols each
+constexpr uint32_t C_BUF = 288, BUF_STRIDE = 96;          // two forward buffers: A | B | g, 32 cols each
+}  // namespace upd
+
+#ifndef TTT_SIGMOID_TANH
+#define TTT_SIGMOID_TANH 1
+#endif
+
+// sigmoid on the MUFU: one tanh (default) or ex2 + rcp
+__device__ __forceinline__ float fast_sigmoid(float a) {
+#if TTT_SIGMOID_TANH
+  float th;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(th) : "f"(0.5f * a));
+  return fmaf(0.5f, th, 0.5f);
+#else
+  float e, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(a * -1.4426950408889634f));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
+  return r;
+#endif
+}
+
+__global__ void __launch_bounds__(upd::THREADS, 1)
+bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
+                   const __nv_bfloat16* __restrict__ Wb, const float* __restrict__ lr,
+                   float* __restrict__ P, float* __restrict__ loss_part, int M, int nh, int H,
+                   int tiles_total, int tiles_per_split, int want_loss) {
+  using namespace upd;
+  constexpr int HD = 64;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) &
+                                             ~static_cast<uintptr_t>(1023));
+  __shared__ uint64_t full[STAGES], empty[STAGES], fwd_full[2], epi_done[2], w_ready, grad_done;
+  __shared__ uint32_t tmem_base_s;
+  __shared__ float loss_red[8];
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int split = blockIdx.x, slice = blockIdx.y, h = blockIdx.z;
+  const int nslices = gridDim.y;
+  const int tile_lo = split * tiles_per_split;
+  const int ntiles = min(tiles_per_split, tiles_total - tile_lo);
+
+  if (tid == 0) {
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 128); }
+    mbar_init(&w_ready, 128);
+    mbar_init(&grad_done, 1);
+    fence_mbar_init();
+  }
+  if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tb = tmem_base_s;
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (elect_one()) {
+      tma_prefetch_desc(&mapK);
+      tma_prefetch_desc(&mapV);
+      for (int i = 0; i < ntiles; ++i) {
+        const int s = i % STAGES, it = i / STAGES;
+        mbar_wait(&empty[s], (it & 1) ^ 1);
+        mbar_arrive_expect_tx(&full[s], 2 * TILE_BYTES);
+        uint8_t* dst = smem + s * 2 * TILE_BYTES;
+        tma_load_2d(dst, &mapK, &full[s], h * HD, (tile_lo + i) * T);
+        tma_load_2d(dst + TILE_BYTES, &mapV, &full[s], h * HD, (tile_lo + i) * T);
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (elect_one()) {
+      constexpr uint32_t idesc_f = umma_idesc_bf16(HS, T, 0, 0);    // B = token tile, K-major
+      constexpr uint32_t idesc_g = umma_idesc_bf16(HS, HD, 0, 1);   // B = token tile, MN-major
+      const uint32_t smem_base = smem_u32(smem);
+      mbar_wait(&w_ready, 0);
+      tc_fence_after();
+      auto fwd = [&](int i) {
+        const int s = i % STAGES, it = i / STAGES, b = i & 1;
+        mbar_wait(&full[s], it & 1);
+        tc_fence_after();
+        const uint32_t ks = smem_base + s * 2 * TILE_BYTES, vs = ks + TILE_BYTES;
+        const uint32_t acc = tb + C_BUF + b * BUF_STRIDE;
+#pragma unroll
+        for (int k = 0; k < HD / 16; ++k)
+          umma_ts(acc, tb + C_W1 + 8 * k, umma_smem_desc_sw128(ks + 32 * k, 16, 1024), idesc_f, k > 0);
+#pragma unroll
+        for (int k = 0; k < HD / 16; ++k)
+          umma_ts(acc + 32, tb + C_W3 + 8 * k, umma_smem_desc_sw128(ks + 32 * k, 16, 1024), idesc_f, k > 0);
+#pragma unroll
+        for (int k = 0; k < HD / 16; ++k)
+          umma_ts(acc + 64, tb + C_W2 + 8 * k, umma_smem_desc_sw128(vs + 32 * k, 16, 1024), idesc_f, k > 0);
+        tc_commit(&fwd_full[b]);
+      };
+      auto grad = [&](int i) {
+        const int s = i % STAGES, b = i & 1, n = i >> 1;
+        mbar_wait(&epi_done[b], n & 1);
+        tc_fence_after();
+        const uint32_t ks = smem_base + s * 2 * TILE_BYTES, vs = ks + TILE_BYTES;
+        const uint32_t opnd = tb + C_BUF + b * BUF_STRIDE;   // dA | dB | Hd' alias A | B | g
+#pragma unroll
+        for (int k = 0; k < T / 16; ++k)
+          umma_ts(tb + C_G1, opnd + 8 * k, umma_smem_desc_sw128(ks + 2048 * k, TILE_BYTES, 1024),
+                  idesc_g, (i > 0 || k > 0));
+#pragma unroll
+        for (int k = 0; k < T / 16; ++k)
+          umma_ts(tb + C_G3, opnd + 32 + 8 * k, umma_smem_desc_sw128(ks + 2048 * k, TILE_BYTES, 1024),
+                  idesc_g, (i > 0 || k > 0));
+#pragma unroll
+        for (int k = 0; k < T / 16; ++k)
+          umma_ts(tb + C_G2, opnd + 64 + 8 * k, umma_smem_desc_sw128(vs + 2048 * k, TILE_BYTES, 1024),
+                  idesc_g, (i > 0 || k > 0));
+        tc_commit(&empty[s]);
+      };
+      if (ntiles > 0) fwd(0);
+      for (int i = 0; i < ntiles; ++i) {
+        if (i + 1 < ntiles) fwd(i + 1);
+        grad(i);
+      }
+      tc_commit(&grad_done);
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue warpgroups =====================
+    const int wg = (warp - 4) >> 2, q = warp & 3;
+    const int j = q * 32 + lane;                       // hidden unit within the slice = TMEM lane
+    const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
+    const size_t me = (size_t)nh * H * HD;
+    const size_t row = ((size_t)h * H + (size_t)slice * HS + j) * HD;
+    if (wg == 0) {
+      // weights -> TMEM as A operands: row j of W1^T, W3^T, W2 (64 bf16 = 32 words each)
+      const uint32_t cols[3] = {C_W1, C_W2, C_W3};
+#pragma unroll
+      for (int mat = 0; mat < 3; ++mat) {
+        const uint4* src = reinterpret_cast<const uint4*>(Wb + mat * me + row);
+        uint32_t r[32];
+#pragma unroll
+        for (int v = 0; v < 8; ++v) {
+          const uint4 x = __ldg(src + v);
+          r[4 * v] = x.x; r[4 * v + 1] = x.y; r[4 * v + 2] = x.z; r[4 * v + 3] = x.w;
+        }
+        tmem_st_x32(tb + lane_base + cols[mat], r);
+      }
+      tc_wait_st();
+      tc_fence_before();
+      mbar_arrive(&w_ready);
+    }
+    float loss = 0.f;
+    const float* lrh = lr + (size_t)h * M;
+    for (int i = wg; i < ntiles; i += 2) {
+      const int b = i & 1, n = i >> 1;
+      const int t0 = (tile_lo + i) * T;
+      const uint32_t buf = tb + lane_base + C_BUF + b * BUF_STRIDE;
+      mbar_wait(&fwd_full[b], n & 1);
+      tc_fence_after();
+#pragma unroll
+      for (int half = 0; half < 2; ++half) {
+        uint32_t ra[16], rb[16], rg[16];
+        tmem_ld_x16(buf + 16 * half, ra);
+        tmem_ld_x16(buf + 32 + 16 * half, rb);
+        tmem_ld_x16(buf + 64 + 16 * half, rg);
+        float ne[16];
+#pragma unroll
+        for (int c = 0; c < 16; ++c) {
+          const int t = t0 + 16 * half + c;
+          ne[c] = (t < M) ? -__ldg(lrh + t) : 0.f;
+        }
+        tc_wait_ld();
+        uint32_t pa[8], pb[8], ph[8];
+#pragma unroll
+        for (int c = 0; c < 16; c += 2) {
+          float oa[2], ob[2], oh[2];
+#pragma unroll
+          for (int u = 0; u < 2; ++u) {
+            const float a = __uint_as_float(ra[c + u]);
+            const float bb = __uint_as_float(rb[c + u]);
+            const float g = __uint_as_float(rg[c + u]);
+            const float s = fast_sigmoid(a);
+            const float S = a * s;                       // SiLU(a)
+            const float hdv = S * bb;                    // hidden activation Hd
+            const float dhd = ne[c + u] * g;             // dHd = (-eta v) W2^T
+            const float t2 = fmaf(-S, s, S) + s;         // SiLU'(a) = s + S (1 - s)
+            oa[u] = (dhd * bb) * t2;                     // dA
+            ob[u] = dhd * S;                             // dB
+            oh[u] = ne[c + u] * hdv;                     // Hd' = -eta Hd
+            loss = fmaf(hdv, dhd, loss);
+          }
+          pa[c >> 1] = pack_bf16x2(oa[0], oa[1]);
+          pb[c >> 1] = pack_bf16x2(ob[0], ob[1]);
+          ph[c >> 1] = pack_bf16x2(oh[0], oh[1]);
+        }
+        // bf16 operands overwrite the first 16 columns of their own fp32 sources
+        tmem_st_x8(buf + 8 * half, pa);
+        tmem_st_x8(buf + 32 + 8 * half, pb);
+        tmem_st_x8(buf + 64 + 8 * half, ph);
+      }
+      tc_wait_st();
+      tc_fence_before();
+      mbar_arrive(&epi_done[b]);
+    }
+    // ---- flush the gradient accumulators: one fp32 partial slice per CTA ----
+    mbar_wait(&grad_done, 0);
+    tc_fence_after();
+    float* Pset = P + (size_t)split * 3 * me;
+    auto flush = [&](uint32_t col, int mat, int c0, int ncols) {
+      float4* dst = reinterpret_cast<float4*>(Pset + mat * me + row + c0);
+      for (int c = 0; c < ncols; c += 16) {
+        uint32_t r[16];
+        if (ntiles > 0) {
+          tmem_ld_x16(tb + lane_base + col + c0 + c, r);
+          tc_wait_ld();
+        } else {
+#pragma unroll
+          for (int u = 0; u < 16; ++u) r[u] = 0u;
+        }
+#pragma unroll
+        for (int v = 0; v < 4; ++v)
+          dst[(c >> 2) + v] = make_float4(__uint_as_float(r[4 * v]), __uint_as_float(r[4 * v + 1]),
+                                          __uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3]));
+      }
+    };
+    if (wg == 0) { flush(C_G1, 0, 0, 64); flush(C_G2, 1, 0, 32); }
+    else         { flush(C_G3, 2, 0, 64); flush(C_G2, 1, 32, 32); }
+    if (want_loss) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) loss += __shfl_xor_sync(0xffffffffu, loss, o);
+      if (lane == 0) loss_red[warp - 4] = loss;
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      if (warp == 4 && lane == 0) {
+        float t = 0.f;
+        for (int w = 0; w < 8; ++w) t += loss_red[w];
+        loss_part[((size_t)split * nslices + slice) * nh + h] = t;
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tb, 512);
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                    const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                    const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// 2-D bf16 tensor [rows][cols] (row stride ld elements), box = [box_rows][64 cols], 128-B swizzle.
+// Out-of-bounds rows are zero-filled, which makes the ragged last token tile contribute nothing.
+int make_token_map(ttt_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int64_t cols,
+                   int64_t ld, int box_rows) {
+  cuuint64_t gdim[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t gstr[1] = {(cuuint64_t)ld * 2};
+  cuuint32_t box[2] = {64, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = reinterpret_cast<encode_tiled_fn>(ctx->encode_tiled)(
+      map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstr, box, estr,
+      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    snprintf(ctx->err, sizeof(ctx->err), "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+    return TTT_ERR_CUDA;
+  }
+  return TTT_OK;
+}
+
+static void update_split(const ttt_ctx* ctx, int64_t M, int* tiles_total, int* tiles_per_split,
+                         int* splits) {
+  const int tiles = (int)((M + upd::T - 1) / upd::T);
+  const int pairs = ctx->cfg.nh * (ctx->cfg.hidden / upd::HS);
+  int want = ctx->sm_count / pairs;           // one wave of CTAs, one CTA per SM
+  if (want < 1) want = 1;
+  if (want > tiles) want = tiles;
+  const int tps = (tiles + want - 1) / want;
+  *tiles_total = tiles;
+  *tiles_per_split = tps;
+  *splits = (tiles + tps - 1) / tps;
+}
+
+int bf16_partials_needed(const ttt_ctx* ctx, int64_t M) {
+  int a, b, s;
+  update_split(ctx, M, &a, &b, &s);
+  return s;
+}
+
+int bf16_supported(const ttt_config* cfg, char* why, size_t why_len) {
+  if (cfg->hd != 64) { snprintf(why, why_len, "bf16 path: hd must be 64 (got %d)", cfg->hd); return 0; }
+  if (cfg->hidden % 128 != 0 || cfg->hidden < 128 || cfg->hidden > 512) {
+    snprintf(why, why_len, "bf16 path: hidden must be a multiple of 128 in [128, 512] (got %d)", cfg->hidden);
+    return 0;
+  }
+  if (cfg->linear_fast_weight) { snprintf(why, why_len, "bf16 path: linear test mode is f32-only"); return 0; }
+  return 1;
+}
+
+int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V, const float* lr,
+                    int64_t M, int64_t ld, bool want_loss, int* used, int* loss_rows,
+                    cudaStream_t s) {
+  const ttt_config& c = ctx->cfg;
+  int tiles, tps, splits;
+  update_split(ctx, M, &tiles, &tps, &splits);
+  CUtensorMap mapK, mapV;
+  int rc = make_token_map(ctx, &mapK, K, M, (int64_t)c.nh * c.hd, ld, upd::T);
+  if (rc != TTT_OK) return rc;
+  rc = make_token_map(ctx, &mapV, V, M, (int64_t)c.nh * c.hd, ld, upd::T);
+  if (rc != TTT_OK) return rc;
+  const size_t smem = (size_t)upd::STAGES * 2 * upd::TILE_BYTES + 1024;
+  static bool attr_set = false;
+  if (!attr_set) {
+    TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_update_kernel,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
+                 "bf16_update_kernel smem attr");
+    attr_set = true;
+  }
+  const int nslices = c.hidden / upd::HS;
+  float* P = ctx->partials + (size_t)ctx->n_partials * 3 * ctx->mat_elems;
+  dim3 grid(splits, nslices, c.nh);
+  bf16_update_kernel<<<grid, upd::THREADS, smem, s>>>(mapK, mapV, ctx->Wb, lr, P, ctx->loss_part,
+                                                      (int)M, c.nh, c.hidden, tiles, tps,
+                                                      want_loss ? 1 : 0);
+  TTT_LAUNCH_CHECK(ctx, "bf16_update_kernel");
+  *used = splits;
+  *loss_rows = splits * nslices;
+  return TTT_OK;
+}
+
+}  // namespace ttt

@@ -1,0 +1,273 @@
+// ttt_api.cu — the C ABI of include/ttt.h: argument validation, context life cycle and the launch
+// chains. No arithmetic here; every step of the path runs in the kernels of the other files.
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "ttt_internal.h"
+
+using namespace ttt;
+
+namespace {
+
+int fail(ttt_ctx* ctx, int status, const char* fmt, long long a = 0, long long b = 0) {
+  if (ctx) snprintf(ctx->err, sizeof(ctx->err), fmt, a, b);
+  return status;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+size_t elt_size(const ttt_ctx* ctx) { return ctx->cfg.act_dtype == TTT_BF16 ? 2 : 4; }
+
+int check_tokens(ttt_ctx* ctx, int64_t M, int64_t ld) {
+  if (M < 0) return fail(ctx, TTT_ERR_ARG, "M = %lld is negative", M);
+  if (M > ctx->cfg.max_tokens)
+    return fail(ctx, TTT_ERR_SHAPE, "M = %lld exceeds max_tokens = %lld", M, ctx->cfg.max_tokens);
+  if (ld < (int64_t)ctx->cfg.nh * ctx->cfg.hd)
+    return fail(ctx, TTT_ERR_SHAPE, "ld = %lld is smaller than nh*hd = %lld", ld,
+                (long long)ctx->cfg.nh * ctx->cfg.hd);
+  if ((ld * (int64_t)elt_size(ctx)) % 16 != 0)
+    return fail(ctx, TTT_ERR_ALIGN, "ld*sizeof(elt) = %lld is not a multiple of 16",
+                ld * (long long)elt_size(ctx));
+  return TTT_OK;
+}
+
+int do_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, int64_t M,
+                  int64_t ld, float* loss, cudaStream_t s) {
+  const bool bf16 = ctx->cfg.act_dtype == TTT_BF16;
+  const int need = bf16 ? bf16_partials_needed(ctx, M) : f32_partials_needed(ctx, M);
+  if (need > ctx->cap_partials)
+    return fail(ctx, TTT_ERR_SHAPE, "internal: %lld partial sets needed, capacity %lld", need,
+                ctx->cap_partials);
+  if (ctx->n_partials + need > ctx->cap_partials) {  // fold the pending sets into G first
+    int rc = launch_reduce_pending(ctx, s);
+    if (rc != TTT_OK) return rc;
+  }
+  int used = 0, loss_rows = 0, rc;
+  if (bf16)
+    rc = bf16_accumulate(ctx, static_cast<const __nv_bfloat16*>(K),
+                         static_cast<const __nv_bfloat16*>(V), lr, M, ld, loss != nullptr, &used,
+                         &loss_rows, s);
+  else
+    rc = f32_accumulate(ctx, static_cast<const float*>(K), static_cast<const float*>(V), lr, M, ld,
+                        loss != nullptr, &used, &loss_rows, s);
+  if (rc != TTT_OK) return rc;
+  ctx->n_partials += used;
+  if (loss != nullptr) return launch_loss_reduce(ctx, loss_rows, loss, s);
+  return TTT_OK;
+}
+
+int do_apply(ttt_ctx* ctx, const void* Q, void* O, int64_t M, int64_t ld, cudaStream_t s) {
+  if (ctx->cfg.act_dtype == TTT_BF16)
+    return bf16_apply(ctx, static_cast<const __nv_bfloat16*>(Q), static_cast<__nv_bfloat16*>(O), M,
+                      ld, s);
+  return f32_apply(ctx, static_cast<const float*>(Q), static_cast<float*>(O), M, ld, s);
+}
+
+int check_update_args(ttt_ctx* ctx, const void* K, const void* V, const float* lr, int64_t M,
+                      int64_t ld) {
+  if (!ctx->initialised) return fail(ctx, TTT_ERR_STATE, "ttt_init has not been called");
+  int rc = check_tokens(ctx, M, ld);
+  if (rc != TTT_OK) return rc;
+  if (M == 0) return TTT_OK;
+  if (!K || !V || !lr) return fail(ctx, TTT_ERR_ARG, "K, V and lr must not be NULL");
+  if (!aligned16(K) || !aligned16(V))
+    return fail(ctx, TTT_ERR_ALIGN, "K and V must be 16-byte aligned");
+  return TTT_OK;
+}
+
+int check_apply_args(ttt_ctx* ctx, const void* Q, const void* O, int64_t M, int64_t ld) {
+  if (!ctx->initialised) return fail(ctx, TTT_ERR_STATE, "ttt_init has not been called");
+  int rc = check_tokens(ctx, M, ld);
+  if (rc != TTT_OK) return rc;
+  if (M == 0) return TTT_OK;
+  if (!Q || !O) return fail(ctx, TTT_ERR_ARG, "Q and O must not be NULL");
+  if (Q == O) return fail(ctx, TTT_ERR_ARG, "O must not alias Q");
+  if (!aligned16(Q) || !aligned16(O))
+    return fail(ctx, TTT_ERR_ALIGN, "Q and O must be 16-byte aligned");
+  return TTT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
+  if (!out || !cfg) return TTT_ERR_ARG;
+  if (cfg->nh < 1 || cfg->hd < 1 || cfg->hidden < 1 || cfg->max_tokens < 1 || cfg->ns_iters < 0 ||
+      (cfg->renorm != 0 && cfg->renorm != 1) ||
+      (cfg->linear_fast_weight != 0 && cfg->linear_fast_weight != 1) ||
+      (cfg->act_dtype != TTT_F32 && cfg->act_dtype != TTT_BF16))
+    return TTT_ERR_ARG;
+  if (cfg->hd % 4 != 0 || cfg->hidden % 4 != 0 || cfg->hd > 128) return TTT_ERR_SHAPE;
+  if (cfg->linear_fast_weight && cfg->hidden != cfg->hd) return TTT_ERR_SHAPE;
+  if (cfg->ns_iters > 0 && cfg->hidden < cfg->hd) return TTT_ERR_UNSUPPORTED;
+  if (cfg->act_dtype == TTT_BF16) {
+    char why[256];
+    if (!bf16_supported(cfg, why, sizeof(why))) return TTT_ERR_UNSUPPORTED;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev)
+    return TTT_ERR_CUDA;
+  if (cudaSetDevice(cfg->device) != cudaSuccess) return TTT_ERR_CUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) return TTT_ERR_CUDA;
+  if (prop.major != 10) return TTT_ERR_UNSUPPORTED;  // sm_100a only; no fallback
+
+  ttt_ctx* ctx = new (std::nothrow) ttt_ctx();
+  if (!ctx) return TTT_ERR_NOMEM;
+  memset(ctx, 0, sizeof(*ctx));
+  ctx->cfg = *cfg;
+  ctx->sm_count = prop.multiProcessorCount;
+  ctx->mat_elems = (size_t)cfg->nh * cfg->hidden * cfg->hd;
+  const size_t set = 3 * ctx->mat_elems;
+  const bool bf16 = cfg->act_dtype == TTT_BF16;
+  ctx->cap_partials = 2 * (bf16 ? bf16_partials_needed(ctx, cfg->max_tokens)
+                                : f32_partials_needed(ctx, cfg->max_tokens));
+  if (ctx->cap_partials < 4) ctx->cap_partials = 4;
+  ctx->cap_loss_rows = ctx->cap_partials * ((cfg->hidden + 127) / 128);
+  const int nblk = (cfg->hidden + 15) / 16;
+
+  bool ok = true;
+  auto alloc = [&](void** p, size_t bytes) {
+    if (ok && cudaMalloc(p, bytes) != cudaSuccess) ok = false;
+  };
+  alloc((void**)&ctx->Wm, set * sizeof(float));
+  alloc((void**)&ctx->Wb, set * sizeof(__nv_bfloat16));
+  alloc((void**)&ctx->n0, ((size_t)2 * cfg->nh * cfg->hidden + (size_t)cfg->nh * cfg->hd) * sizeof(float));
+  alloc((void**)&ctx->colsq, (size_t)cfg->nh * nblk * cfg->hd * sizeof(float));
+  alloc((void**)&ctx->G, set * sizeof(float));
+  alloc((void**)&ctx->partials, (size_t)ctx->cap_partials * set * sizeof(float));
+  alloc((void**)&ctx->loss_part, (size_t)ctx->cap_loss_rows * cfg->nh * sizeof(float));
+  if (!bf16) {
+    const size_t act = (size_t)cfg->nh * cfg->max_tokens * cfg->hidden * sizeof(float);
+    for (int i = 0; i < 3; ++i) alloc((void**)&ctx->act[i], act);
+    alloc((void**)&ctx->loss_blk, (size_t)cfg->nh * ((cfg->max_tokens + 63) / 64) *
+                                      ((cfg->hidden + 63) / 64) * sizeof(float));
+  } else {
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ctx->encode_tiled, cudaEnableDefault,
+                                &qres) != cudaSuccess ||
+        ctx->encode_tiled == nullptr)
+      ok = false;
+  }
+  if (!ok) {
+    cudaGetLastError();
+    ttt_destroy(ctx);
+    return TTT_ERR_NOMEM;
+  }
+  *out = ctx;
+  return TTT_OK;
+}
+
+void ttt_destroy(ttt_ctx* ctx) {
+  if (!ctx) return;
+  cudaSetDevice(ctx->cfg.device);
+  cudaDeviceSynchronize();
+  cudaFree(ctx->Wm); cudaFree(ctx->Wb); cudaFree(ctx->n0); cudaFree(ctx->colsq);
+  cudaFree(ctx->G); cudaFree(ctx->partials); cudaFree(ctx->loss_part); cudaFree(ctx->loss_blk);
+  for (int i = 0; i < 3; ++i) cudaFree(ctx->act[i]);
+  delete ctx;
+}
+
+int ttt_init(ttt_ctx* ctx, const float* W1, const float* W2, const float* W3, void* stream) {
+  if (!ctx) return TTT_ERR_ARG;
+  if (!W1 || !W2 || !W3) return fail(ctx, TTT_ERR_ARG, "W1, W2 and W3 must not be NULL");
+  int rc = launch_init(ctx, W1, W2, W3, static_cast<cudaStream_t>(stream));
+  if (rc != TTT_OK) return rc;
+  ctx->initialised = true;
+  ctx->n_partials = 0;
+  ctx->G_valid = false;
+  return TTT_OK;
+}
+
+int ttt_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, int64_t M,
+                   int64_t ld, float* loss, void* stream) {
+  if (!ctx) return TTT_ERR_ARG;
+  int rc = check_update_args(ctx, K, V, lr, M, ld);
+  if (rc != TTT_OK || M == 0) return rc;
+  return do_accumulate(ctx, K, V, lr, M, ld, loss, static_cast<cudaStream_t>(stream));
+}
+
+int ttt_commit(ttt_ctx* ctx, void* stream) {
+  if (!ctx) return TTT_ERR_ARG;
+  if (!ctx->initialised) return fail(ctx, TTT_ERR_STATE, "ttt_init has not been called");
+  if (ctx->n_partials == 0 && !ctx->G_valid) return TTT_OK;  // nothing pending
+  return launch_commit(ctx, static_cast<cudaStream_t>(stream));
+}
+
+int ttt_pending_gradient(ttt_ctx* ctx, float** G, int64_t* n_elements, void* stream) {
+  if (!ctx || !G || !n_elements) return TTT_ERR_ARG;
+  if (!ctx->initialised) return fail(ctx, TTT_ERR_STATE, "ttt_init has not been called");
+  if (ctx->n_partials == 0 && !ctx->G_valid)
+    return fail(ctx, TTT_ERR_STATE, "no pending gradient (call ttt_accumulate first)");
+  int rc = launch_reduce_pending(ctx, static_cast<cudaStream_t>(stream));
+  if (rc != TTT_OK) return rc;
+  *G = ctx->G;
+  *n_elements = (int64_t)(3 * ctx->mat_elems);
+  return TTT_OK;
+}
+
+int ttt_update(ttt_ctx* ctx, const void* K, const void* V, const float* lr, int64_t M, int64_t ld,
+               float* loss, void* stream) {
+  if (!ctx) return TTT_ERR_ARG;
+  int rc = check_update_args(ctx, K, V, lr, M, ld);
+  if (rc != TTT_OK || M == 0) return rc;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  rc = do_accumulate(ctx, K, V, lr, M, ld, loss, s);
+  if (rc != TTT_OK) return rc;
+  return launch_commit(ctx, s);
+}
+
+int ttt_apply(ttt_ctx* ctx, const void* Q, void* O, int64_t M, int64_t ld, void* stream) {
+  if (!ctx) return TTT_ERR_ARG;
+  int rc = check_apply_args(ctx, Q, O, M, ld);
+  if (rc != TTT_OK || M == 0) return rc;
+  return do_apply(ctx, Q, O, M, ld, static_cast<cudaStream_t>(stream));
+}
+
+int ttt_chunk_step(ttt_ctx* ctx, const void* Q, const void* K, const void* V, const float* lr,
+                   void* O, int64_t M, int64_t ld, float* loss, void* stream) {
+  if (!ctx) return TTT_ERR_ARG;
+  int rc = check_update_args(ctx, K, V, lr, M, ld);
+  if (rc != TTT_OK) return rc;
+  rc = check_apply_args(ctx, Q, O, M, ld);
+  if (rc != TTT_OK || M == 0) return rc;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  rc = do_accumulate(ctx, K, V, lr, M, ld, loss, s);
+  if (rc != TTT_OK) return rc;
+  rc = launch_commit(ctx, s);
+  if (rc != TTT_OK) return rc;
+  return do_apply(ctx, Q, O, M, ld, s);
+}
+
+int ttt_get_weights(ttt_ctx* ctx, float* W1, float* W2, float* W3, void* stream) {
+  if (!ctx) return TTT_ERR_ARG;
+  if (!ctx->initialised) return fail(ctx, TTT_ERR_STATE, "ttt_init has not been called");
+  if (!W1 || !W2 || !W3) return fail(ctx, TTT_ERR_ARG, "W1, W2 and W3 must not be NULL");
+  return launch_get_weights(ctx, W1, W2, W3, static_cast<cudaStream_t>(stream));
+}
+
+int64_t ttt_launch_count(const ttt_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+const char* ttt_strerror(int status) {
+  switch (status) {
+    case TTT_OK: return "ok";
+    case TTT_ERR_ARG: return "invalid argument";
+    case TTT_ERR_SHAPE: return "shape out of range";
+    case TTT_ERR_ALIGN: return "misaligned pointer or stride";
+    case TTT_ERR_STATE: return "context not in the required state";
+    case TTT_ERR_UNSUPPORTED: return "configuration not supported by the sm_100a kernels";
+    case TTT_ERR_NOMEM: return "out of device memory";
+    case TTT_ERR_CUDA: return "CUDA error";
+    default: return "unknown status";
+  }
+}
+
+const char* ttt_last_error(const ttt_ctx* ctx) { return ctx ? ctx->err : ""; }
+
+const char* ttt_version(void) { return "ttt-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,91 @@
+// ttt_internal.h — context layout and launcher prototypes shared by the translation units of
+// libttt_b200.so. Not part of the public ABI (that is include/ttt.h).
+#pragma once
+
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/ttt.h"
+
+// Internal weight layout ("hidden-major"): three matrices per head, each [H][hd], hd contiguous:
+//   mat 0 = W1^T   (row j = fan-in vector of hidden unit j of the gate branch, Eq. 12)
+//   mat 1 = W2     (row j = fan-out vector of hidden unit j;  column o = fan-in of output o)
+//   mat 2 = W3^T   (row j = fan-in vector of hidden unit j of the up branch)
+// Element (mat, h, j, i) lives at ((mat*nh + h)*H + j)*hd + i, in the fp32 master `Wm`, the bf16
+// operand copy `Wb`, the dense gradient `G` and every partial-gradient set.
+struct ttt_ctx {
+  ttt_config cfg;
+  int sm_count;
+  bool initialised;
+  int64_t launches;
+  char err[512];
+
+  size_t mat_elems;      // nh*H*hd
+  float* Wm;             // [3][nh][H][hd] fp32 master weights
+  __nv_bfloat16* Wb;     // [3][nh][H][hd] bf16 operand copy (refreshed by init/commit)
+  float* n0;             // initial fan-in norms: [nh][H] (mat 0), [nh][hd] (mat 1), [nh][H] (mat 2)
+  float* colsq;          // [nh][rowblocks][hd] partial column sums of squares of W2 (renorm)
+
+  // pending gradient = (G_valid ? G : 0) + sum_{s < n_partials} partials[s], summed in this order
+  float* G;              // [3][nh][H][hd]
+  bool G_valid;
+  float* partials;       // [cap_partials][3][nh][H][hd]
+  int cap_partials;
+  int n_partials;
+  float* loss_part;      // [cap_loss_rows][nh] per-CTA-group loss partials of the last accumulate
+  int cap_loss_rows;
+  float* loss_blk;       // f32 path: per-block loss partials [nh][ceil(max_tokens/64)][ceil(H/64)]
+
+  // f32 path workspaces: three [nh][max_tokens][H] fp32 activation buffers
+  float* act[3];
+
+  // bf16 path: driver entry point for cuTensorMapEncodeTiled
+  void* encode_tiled;
+};
+
+namespace ttt {
+
+int set_error(ttt_ctx* ctx, int status, const char* what, cudaError_t e);
+
+// --- state kernels (state_kernels.cu) -----------------------------------------------------------
+int launch_init(ttt_ctx* ctx, const float* W1, const float* W2, const float* W3, cudaStream_t s);
+int launch_get_weights(ttt_ctx* ctx, float* W1, float* W2, float* W3, cudaStream_t s);
+// G = (G_valid ? G : 0) + sum partials; marks G_valid, clears n_partials
+int launch_reduce_pending(ttt_ctx* ctx, cudaStream_t s);
+// [NS] -> W -= pending -> [renorm] -> bf16 copy; clears the pending set
+int launch_commit(ttt_ctx* ctx, cudaStream_t s);
+// loss[h] = sum_{r in [0, n)} loss_part[r][h]  (fixed order)
+int launch_loss_reduce(ttt_ctx* ctx, int n, float* loss, cudaStream_t s);
+
+// --- f32 path (f32_path.cu) ---------------------------------------------------------------------
+// appends partial-gradient sets [n_partials, n_partials + used); writes loss_part rows [0, loss_rows)
+int f32_accumulate(ttt_ctx* ctx, const float* K, const float* V, const float* lr, int64_t M,
+                   int64_t ld, bool want_loss, int* used, int* loss_rows, cudaStream_t s);
+int f32_apply(ttt_ctx* ctx, const float* Q, float* O, int64_t M, int64_t ld, cudaStream_t s);
+int f32_partials_needed(const ttt_ctx* ctx, int64_t M);
+
+// --- bf16 tensor-core path (bf16_update.cu / bf16_apply.cu) -------------------------------------
+int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V, const float* lr,
+                    int64_t M, int64_t ld, bool want_loss, int* used, int* loss_rows,
+                    cudaStream_t s);
+int bf16_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
+               cudaStream_t s);
+int bf16_partials_needed(const ttt_ctx* ctx, int64_t M);
+int bf16_supported(const ttt_config* cfg, char* why, size_t why_len);
+
+}  // namespace ttt
+
+#define TTT_CUDA_TRY(ctx, call, what)                                   \
+  do {                                                                  \
+    cudaError_t e__ = (call);                                           \
+    if (e__ != cudaSuccess) return ttt::set_error((ctx), TTT_ERR_CUDA, (what), e__); \
+  } while (0)
+
+#define TTT_LAUNCH_CHECK(ctx, what)                                     \
+  do {                                                                  \
+    cudaError_t e__ = cudaGetLastError();                               \
+    if (e__ != cudaSuccess) return ttt::set_error((ctx), TTT_ERR_CUDA, (what), e__); \
+    (ctx)->launches += 1;                                               \
+  } while (0)

@@ -1,0 +1,248 @@
+"""Parity of the CUDA path (through the C ABI) against the float64 oracle, same seeded inputs.
+
+Tolerances (BASELINE.json:north_star): err(X) = max|X_gpu - X_ora| /
+max|X_ora| per tensor (reading P17). fp32 path: <= 1e-4 on every chunk's O and on the final
+fast weights. bf16 path: <= 2e-2 on outputs and updated fast weights after the final chunk.
+"""
+import numpy as np
+import pytest
+import torch
+
+import ttt_inputs as ti
+from oracle.ttt_oracle import OracleTTT, rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL_F32 = 1e-4
+TOL_BF16 = 2e-2
+# The optional loss output is ONE scalar per head, a sum of M*H terms of both signs: cancellation
+# makes its relative error several times that of the tensors; it is not
+# part of north_star's bar (outputs and updated fast weights).
+TOL_LOSS_F32 = 2e-3
+TOL_LOSS_BF16 = 5e-2
+
+
+def _mk(w: ti.TTTWorkload, max_tokens=None):
+    from paper_2604_08542_b200 import TTT, TTT_BF16, TTT_F32
+    return TTT(w.nh, w.hd, w.hidden, TTT_BF16 if w.act_dtype == "bf16" else TTT_F32,
+               ns_iters=w.ns_iters, renorm=w.renorm, max_tokens=max_tokens or w.chunk_tokens)
+
+
+def _run_stream(w: ti.TTTWorkload, check_loss=True):
+    """Run the whole chunk stream on both sides; returns per-chunk O errors and final W errors."""
+    dev = torch.device("cuda", 0)
+    W1, W2, W3 = ti.fast_weights(w)
+    ora = OracleTTT(W1, W2, W3, ns_iters=w.ns_iters, renorm=w.renorm)
+    gpu = _mk(w)
+    gpu.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    errs_o, errs_l = [], []
+    for (Q, K, V, lr) in ti.TokenStream(w):
+        loss = torch.zeros(w.nh, dtype=torch.float32, device=dev)
+        O = gpu.ttt_chunk_step(Q.to(dev), K.to(dev), V.to(dev), lr.to(dev), loss=loss)
+        O_ref, loss_ref = ora.chunk_step(Q, K, V, lr)
+        errs_o.append(rel_err(O.float().cpu(), O_ref))
+        errs_l.append(rel_err(loss.cpu(), loss_ref))
+    g1, g2, g3 = (x.cpu() for x in gpu.ttt_get_weights())
+    errs_w = [rel_err(g1, ora.W1), rel_err(g2, ora.W2), rel_err(g3, ora.W3)]
+    gpu.close()
+    return errs_o, errs_w, errs_l
+
+
+# ------------------------------------------------------------------------------------------------
+# fp32 path
+# ------------------------------------------------------------------------------------------------
+def test_cfg1_fp32_full_config():
+    """BASELINE.json:configs[0] exactly: 1 head, d=64, H=128, 4 chunks x 256 tokens, lr 0.01."""
+    errs_o, errs_w, errs_l = _run_stream(ti.CONFIGS["cfg1"])
+    assert max(errs_o) <= TOL_F32, errs_o
+    assert max(errs_w) <= TOL_F32, errs_w
+    assert max(errs_l) <= TOL_LOSS_F32, errs_l
+
+
+@pytest.mark.parametrize("nh,hd,H,tpf,ns,renorm", [
+    (3, 32, 96, 77, 0, 0),      # ragged everything
+    (2, 64, 128, 200, 5, 0),    # Newton-Schulz
+    (2, 64, 256, 130, 0, 1),    # re-normalisation
+    (2, 128, 256, 90, 5, 1),    # hd = 128, both
+])
+def test_fp32_variants(nh, hd, H, tpf, ns, renorm):
+    w = ti.scaled(ti.CONFIGS["cfg1"], nh=nh, hd=hd, hidden=H, tokens_per_frame=tpf, n_frames=3,
+                  ns_iters=ns, renorm=renorm, lr=0.002)
+    errs_o, errs_w, errs_l = _run_stream(w)
+    assert max(errs_o) <= TOL_F32, errs_o
+    assert max(errs_w) <= TOL_F32, errs_w
+    assert max(errs_l) <= TOL_LOSS_F32, errs_l
+
+
+def test_fp32_linear_closed_form_on_gpu():
+    """north_star closed form through the CUDA path: W1 += K^T diag(lr) V, O = Q W1."""
+    from paper_2604_08542_b200 import TTT, TTT_F32
+    dev = torch.device("cuda", 0)
+    g = torch.Generator().manual_seed(3)
+    nh, hd, M = 2, 64, 300
+    W1 = torch.randn(nh, hd, hd, generator=g) / 8
+    W2 = torch.randn(nh, hd, hd, generator=g) / 8
+    W3 = torch.randn(nh, hd, hd, generator=g) / 8
+    Q, K, V = (torch.randn(M, nh * hd, generator=g) for _ in range(3))
+    lr = torch.rand(nh, M, generator=g) * 0.02
+    t = TTT(nh, hd, hd, TTT_F32, linear_fast_weight=1, max_tokens=M)
+    t.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    for a, b in ((0, 100), (100, 300)):
+        t.ttt_update(K[a:b].to(dev), V[a:b].to(dev), lr[:, a:b].contiguous().to(dev))
+    O = t.ttt_apply(Q.to(dev)).cpu()
+    w1 = t.ttt_get_weights()[0].cpu()
+    for h in range(nh):
+        s = slice(h * hd, (h + 1) * hd)
+        expect = W1[h].double() + K[:, s].double().T @ (lr[h].double()[:, None] * V[:, s].double())
+        assert rel_err(w1[h], expect) <= 1e-5
+        assert rel_err(O[:, s], Q[:, s].double() @ expect) <= 1e-5
+    t.close()
+
+
+def test_fp32_lr_zero_and_update_then_apply_equals_chunk_step():
+    from paper_2604_08542_b200 import TTT, TTT_F32
+    dev = torch.device("cuda", 0)
+    w = ti.scaled(ti.CONFIGS["cfg1"], nh=2, tokens_per_frame=150, n_frames=1)
+    W1, W2, W3 = (x.to(dev) for x in ti.fast_weights(w))
+    Q, K, V, lr = (x.to(dev) for x in ti.TokenStream(w).next_chunk())
+    a = _mk(w); a.ttt_init(W1, W2, W3)
+    O0 = a.ttt_apply(Q)
+    O1 = a.ttt_chunk_step(Q, K, V, torch.zeros_like(lr))
+    assert torch.equal(O0, O1)                                   # lr = 0: output = f_{W0}(Q)
+    for x, y in zip(a.ttt_get_weights(), (W1, W2, W3)):
+        assert torch.equal(x, y)                                 # ... and W bit-identical
+    Oa = a.ttt_chunk_step(Q, K, V, lr)
+    b = _mk(w); b.ttt_init(W1, W2, W3)
+    b.ttt_update(K, V, lr); Ob = b.ttt_apply(Q)
+    assert torch.equal(Oa, Ob)
+    a.close(); b.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# bf16 tensor-core path
+# ------------------------------------------------------------------------------------------------
+def _bf16_workload(base, **kw):
+    return ti.scaled(ti.CONFIGS[base], **kw)
+
+
+@pytest.mark.parametrize("base,kw", [
+    # several 32-token update tiles and 128-token apply tiles plus ragged tails, one chunk
+    ("cfg2", dict(nh=2, tokens_per_frame=333, frames_per_chunk=3, n_frames=3)),
+    # hidden 256 (two hidden slices), Newton-Schulz, 3 chunks, AR(1) tokens
+    ("cfg3", dict(nh=2, tokens_per_frame=257, frames_per_chunk=2, n_frames=6)),
+    # re-normalised plain update, L2-normalised K, 4 chunks with a short last chunk
+    ("cfg4", dict(nh=3, tokens_per_frame=190, frames_per_chunk=2, n_frames=7)),
+])
+def test_bf16_stream_parity(base, kw):
+    w = _bf16_workload(base, **kw)
+    errs_o, errs_w, errs_l = _run_stream(w)
+    assert errs_o[-1] <= TOL_BF16 and max(errs_o) <= TOL_BF16, errs_o
+    assert max(errs_w) <= TOL_BF16, errs_w
+    assert max(errs_l) <= TOL_LOSS_BF16, errs_l
+
+
+def test_bf16_gradient_against_oracle():
+    """The raw gradient (before the commit) is the most sensitive quantity: compare G1, G2, G3."""
+    dev = torch.device("cuda", 0)
+    w = _bf16_workload("cfg2", nh=2, tokens_per_frame=500, frames_per_chunk=2, n_frames=2)
+    W1, W2, W3 = ti.fast_weights(w)
+    Q, K, V, lr = ti.TokenStream(w).next_chunk()
+    gpu = _mk(w)
+    gpu.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    gpu.ttt_accumulate(K.to(dev), V.to(dev), lr.to(dev))
+    G = gpu.ttt_pending_gradient().cpu()                        # [3, nh, H, hd] hidden-major
+    # the oracle consumes the SAME bf16-rounded weights? No: it keeps the fp32 masters; the
+    # rounding of the MMA weight operand is part of the error budget being measured.
+    G1, G2, G3, _ = OracleTTT(W1, W2, W3).grad(K, V, lr)
+    assert rel_err(G[0].transpose(1, 2), G1) <= 1e-2
+    assert rel_err(G[1], G2) <= 1e-2
+    assert rel_err(G[2].transpose(1, 2), G3) <= 1e-2
+    gpu.close()
+
+
+def test_bf16_apply_only_and_head_independence():
+    dev = torch.device("cuda", 0)
+    w = _bf16_workload("cfg2", nh=4, tokens_per_frame=129, frames_per_chunk=3, n_frames=3)
+    W1, W2, W3 = ti.fast_weights(w)
+    Q, K, V, lr = ti.TokenStream(w).next_chunk()
+    gpu = _mk(w)
+    gpu.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    O = gpu.ttt_apply(Q.to(dev)).float().cpu()
+    assert rel_err(O, OracleTTT(W1, W2, W3).apply(Q)) <= 1e-2
+    # head 1 of a 4-head call == a 1-head call on the strided slice
+    O4 = gpu.ttt_chunk_step(Q.to(dev), K.to(dev), V.to(dev), lr.to(dev))
+    one = ti.scaled(w, nh=1)
+    g1 = _mk(one, max_tokens=w.chunk_tokens)
+    g1.ttt_init(W1[1:2].contiguous().to(dev), W2[1:2].contiguous().to(dev), W3[1:2].contiguous().to(dev))
+    s = slice(w.hd, 2 * w.hd)
+    O1 = g1.ttt_chunk_step(Q.to(dev)[:, s], K.to(dev)[:, s], V.to(dev)[:, s], lr[1:2].contiguous().to(dev))
+    assert rel_err(O4[:, s].float().cpu(), O1.float().cpu()) <= 1e-2   # split counts differ -> summation order
+    gpu.close(); g1.close()
+
+
+def test_bf16_bitwise_determinism_and_chunk_step_composition():
+    dev = torch.device("cuda", 0)
+    w = _bf16_workload("cfg3", nh=2, tokens_per_frame=300, frames_per_chunk=2, n_frames=4)
+    W1, W2, W3 = (x.to(dev) for x in ti.fast_weights(w))
+    chunks = [tuple(x.to(dev) for x in c) for c in ti.TokenStream(w)]
+    outs = []
+    for rep in range(3):
+        g = _mk(w); g.ttt_init(W1, W2, W3)
+        res = []
+        for (Q, K, V, lr) in chunks:
+            if rep < 2:
+                res.append(g.ttt_chunk_step(Q, K, V, lr))
+            else:                                   # update ; apply as two calls
+                g.ttt_update(K, V, lr); res.append(g.ttt_apply(Q))
+        outs.append(res + list(g.ttt_get_weights()))
+        g.close()
+    for x, y, z in zip(*outs):
+        assert torch.equal(x, y) and torch.equal(x, z)
+
+
+def test_accumulate_commit_equals_update_on_concatenation():
+    """Eq. 10: accumulate over two chunks at the same W, one commit == update on the concatenation
+    (up to the fp32 summation order of the partials)."""
+    dev = torch.device("cuda", 0)
+    w = _bf16_workload("cfg2", nh=2, tokens_per_frame=256, frames_per_chunk=2, n_frames=4)
+    W1, W2, W3 = (x.to(dev) for x in ti.fast_weights(w))
+    (Q0, K0, V0, l0), (Q1, K1, V1, l1) = [tuple(x.to(dev) for x in c) for c in ti.TokenStream(w)]
+    a = _mk(w, max_tokens=2 * w.chunk_tokens); a.ttt_init(W1, W2, W3)
+    a.ttt_accumulate(K0, V0, l0); a.ttt_accumulate(K1, V1, l1); a.ttt_commit()
+    b = _mk(w, max_tokens=2 * w.chunk_tokens); b.ttt_init(W1, W2, W3)
+    b.ttt_update(torch.cat([K0, K1]), torch.cat([V0, V1]), torch.cat([l0, l1], dim=1).contiguous())
+    for x, y in zip(a.ttt_get_weights(), b.ttt_get_weights()):
+        assert rel_err(x.cpu(), y.cpu()) <= 1e-5
+    a.close(); b.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# boundary behaviour
+# ------------------------------------------------------------------------------------------------
+def test_error_codes_and_empty_chunk():
+    from paper_2604_08542_b200 import TTT, TTT_BF16, TTT_F32, TTTError
+    dev = torch.device("cuda", 0)
+    with pytest.raises(TTTError) as e:
+        TTT(2, 48, 128, TTT_BF16)                       # hd not supported on the tensor path
+    assert e.value.status == -5
+    t = TTT(2, 64, 128, TTT_BF16, max_tokens=256)
+    Q = torch.zeros(64, 128, dtype=torch.bfloat16, device=dev)
+    lr = torch.zeros(2, 64, device=dev)
+    with pytest.raises(TTTError) as e:
+        t.ttt_apply(Q)                                  # before ttt_init
+    assert e.value.status == -4
+    W1, W2, W3 = (torch.zeros(2, 64, 128, device=dev), torch.zeros(2, 128, 64, device=dev),
+                  torch.zeros(2, 64, 128, device=dev))
+    t.ttt_init(W1, W2, W3)
+    big = torch.zeros(512, 128, dtype=torch.bfloat16, device=dev)
+    with pytest.raises(TTTError) as e:
+        t.ttt_apply(big)                                # M > max_tokens
+    assert e.value.status == -2
+    with pytest.raises(TTTError) as e:
+        t.ttt_apply(Q, O=Q)                             # O aliases Q
+    assert e.value.status == -1
+    # empty chunk: no-op, no launch
+    n0 = t.launch_count()
+    t.ttt_chunk_step(Q[:0], Q[:0], Q[:0], lr[:, :0].contiguous())
+    assert t.launch_count() == n0
+    t.close()
