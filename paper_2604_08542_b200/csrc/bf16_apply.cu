@@ -2,17 +2,20 @@
 //   O = ( SiLU(Q W1) o (Q W3) ) W2        Eq. 4 with Eq. 12, updated weights.
 //
 // Formulation ("tokens on lanes"): a CTA owns one head and a strided set of 128-token tiles.
-//   Q tile  -> TMEM as the A operand (bf16, [128 tokens x hd]), written by the I/O warpgroup
+//   Q tile  -> shared memory by TMA (4-stage ring) -> TMEM as the A operand (bf16 [128 x hd])
 //   step n  (64 hidden units):  Aq = Q W1[:, n], Bq = Q W3[:, n]   MMA 128 x 64 x hd, B = weights (K-major)
 //            epilogue  Hq = SiLU(Aq) o Bq -> bf16 -> TMEM over its own fp32 source
 //            O += Hq W2[n, :]                                      MMA 128 x hd x 64, B = W2 slice (MN-major)
-//   O (fp32, TMEM) -> bf16 -> global by the I/O warpgroup.
+//   O (fp32, TMEM) -> bf16 -> swizzled shared memory -> TMA store (rows beyond M are clipped).
 // The bf16 weights of the head (3 x H x hd) sit in shared memory for the CTA's lifetime (TMA, 128-B
 // swizzle). Forward accumulators, Q operands and O accumulators are double-buffered in TMEM, so the
 // MMA of step n+1 overlaps the SwiGLU epilogue of step n, and Q loads / O stores overlap both.
 //
-// Warp roles (512 threads): warp 0 = TMA (weights, once), warp 1 = MMA issuer, warps 4-7 / 8-11 =
-// two epilogue warpgroups alternating steps, warps 12-15 = I/O warpgroup (Q in, O out).
+// Warp roles (512 threads): warp 0 = TMA producer (weights once, then Q tiles), warp 1 = MMA issuer,
+// warps 4-7 / 8-11 = two epilogue warpgroups alternating steps, warps 12-15 = I/O warpgroup
+// (Q: shared -> TMEM; O: TMEM -> shared -> TMA store).
+#include <stdio.h>
+
 #include "tc_common.cuh"
 #include "ttt_internal.h"
 
@@ -25,34 +28,24 @@ namespace app {
 constexpr int TM = 128;        // tokens per tile (MMA M)
 constexpr int NS = 64;         // hidden units per step
 constexpr int THREADS = 512;
+constexpr int QST = 4;         // Q tile ring stages
+constexpr int TILE_BYTES = TM * 128;   // one [128 x 64] bf16 tile
 // TMEM column plan for hd = 64
 constexpr uint32_t C_Q = 0;      // 2 x 32 cols: Q operand (bf16)
 constexpr uint32_t C_O = 64;     // 2 x 64 cols: O accumulator (fp32)
 constexpr uint32_t C_F = 192;    // 2 x 128 cols: Aq (64) | Bq (64) forward accumulators (fp32)
 }  // namespace app
 
-__device__ __forceinline__ float fast_sigmoid_app(float a) {
-#if !defined(TTT_SIGMOID_TANH) || TTT_SIGMOID_TANH
-  float th;
-  asm("tanh.approx.f32 %0, %1;" : "=f"(th) : "f"(0.5f * a));
-  return fmaf(0.5f, th, 0.5f);
-#else
-  float e, r;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(a * -1.4426950408889634f));
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
-  return r;
-#endif
-}
-
 __global__ void __launch_bounds__(app::THREADS, 1)
-bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __nv_bfloat16* __restrict__ Q,
-                  __nv_bfloat16* __restrict__ O, int M, long ld, int nh, int H, int tiles_total) {
+bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ CUtensorMap mapQ,
+                  const __grid_constant__ CUtensorMap mapO, int nh, int H, int tiles_total) {
   using namespace app;
   constexpr int HD = 64;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) &
                                              ~static_cast<uintptr_t>(1023));
   __shared__ uint64_t w_full, fwd_full[2], epi_done[2], q_full[2], q_empty[2], o_full[2], o_empty[2];
+  __shared__ uint64_t qr_full[QST], qr_empty[QST];
   __shared__ uint32_t tmem_base_s;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -62,6 +55,8 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __nv_bfloat16*
   const int my_tiles = (tiles_total - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
   const int total_steps = my_tiles * nsl;
   const uint32_t w_bytes = 3u * H * 128u;                    // bf16 weights of the head
+  uint8_t* q_ring = smem + w_bytes;                          // QST x 16 KB
+  uint8_t* o_stage = q_ring + QST * TILE_BYTES;              // 2 x 16 KB
 
   if (tid == 0) {
     mbar_init(&w_full, 1);
@@ -70,6 +65,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __nv_bfloat16*
       mbar_init(&q_full[b], 128); mbar_init(&q_empty[b], 1);
       mbar_init(&o_full[b], 1);   mbar_init(&o_empty[b], 128);
     }
+    for (int s = 0; s < QST; ++s) { mbar_init(&qr_full[s], 1); mbar_init(&qr_empty[s], 128); }
     fence_mbar_init();
   }
   if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
@@ -79,15 +75,23 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __nv_bfloat16*
   const uint32_t tb = tmem_base_s;
 
   if (warp == 0) {
-    // ===================== TMA: the head's weights, once =====================
+    // ===================== TMA producer: weights once, then the Q tiles =====================
     if (elect_one() && my_tiles > 0) {
       tma_prefetch_desc(&mapW);
+      tma_prefetch_desc(&mapQ);
       mbar_arrive_expect_tx(&w_full, w_bytes);
       // smem: [mat][H rows][128 B]; boxes of 64 rows (8 KB)
       for (int mat = 0; mat < 3; ++mat)
         for (int r = 0; r < H; r += 64)
           tma_load_2d_hint(smem + ((size_t)mat * H + r) * 128, &mapW, &w_full, 0,
                            (mat * nh + h) * H + r, kEvictLast);
+      for (int tl = 0; tl < my_tiles; ++tl) {
+        const int rs = tl % QST, it = tl / QST;
+        mbar_wait(&qr_empty[rs], (it & 1) ^ 1);
+        mbar_arrive_expect_tx(&qr_full[rs], TILE_BYTES);
+        tma_load_2d_hint(q_ring + rs * TILE_BYTES, &mapQ, &qr_full[rs], h * HD,
+                         ((int)blockIdx.x + tl * (int)gridDim.x) * TM, kEvictFirst);
+      }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
@@ -134,51 +138,52 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __nv_bfloat16*
     // ===================== SwiGLU epilogue warpgroups =====================
     const int wg = (warp - 4) >> 2, q = warp & 3;
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
+    const uint64_t HALF2 = pack2(0.5f, 0.5f);
     for (int st = wg; st < total_steps; st += 2) {
       const int fb = st & 1;
       const uint32_t buf = tb + lane_base + C_F + fb * 128;
       mbar_wait(&fwd_full[fb], (st >> 1) & 1);
       tc_fence_after();
 #pragma unroll
-      for (int part = 0; part < 4; ++part) {     // 16 hidden columns at a time
-        uint32_t ra[16], rb[16];
-        tmem_ld_x16(buf + 16 * part, ra);
-        tmem_ld_x16(buf + 64 + 16 * part, rb);
+      for (int part = 0; part < 2; ++part) {     // 32 hidden columns at a time
+        uint32_t ra[32], rb[32];
+        tmem_ld_x32(buf + 32 * part, ra);
+        tmem_ld_x32(buf + 64 + 32 * part, rb);
         tc_wait_ld();
-        uint32_t ph[8];
+        uint32_t ph[16];
 #pragma unroll
-        for (int c = 0; c < 16; c += 2) {
-          const float a0 = __uint_as_float(ra[c]), a1 = __uint_as_float(ra[c + 1]);
-          const float h0 = a0 * fast_sigmoid_app(a0) * __uint_as_float(rb[c]);
-          const float h1 = a1 * fast_sigmoid_app(a1) * __uint_as_float(rb[c + 1]);
-          ph[c >> 1] = pack_bf16x2(h0, h1);
+        for (int c = 0; c < 32; c += 2) {
+          const uint64_t a = pack2u(ra[c], ra[c + 1]);
+          const uint64_t bb = pack2u(rb[c], rb[c + 1]);
+          float x0, x1;
+          unpack2(fmul2(a, HALF2), x0, x1);
+          const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
+          const uint64_t sg = ffma2(th, HALF2, HALF2);             // sigmoid(a)
+          ph[c >> 1] = pack_bf16x2_from2(fmul2(fmul2(a, sg), bb));  // Hq = SiLU(a) b
         }
-        tmem_st_x8(buf + 8 * part, ph);          // Hq (bf16) over the first 32 columns of Aq
+        tmem_st_x16(buf + 16 * part, ph);        // Hq (bf16) over the first 32 columns of Aq
       }
       tc_wait_st();
       tc_fence_before();
       mbar_arrive(&epi_done[fb]);
     }
   } else if (warp >= 12) {
-    // ===================== I/O warpgroup: Q rows in, O rows out =====================
+    // ===================== I/O warpgroup =====================
     const int q = warp & 3;
     const int r = q * 32 + lane;                               // token row within the tile
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
+    const uint32_t swz = static_cast<uint32_t>(r & 7);         // 128-B swizzle: chunk ^= row & 7
     auto load_q = [&](int tl) {
-      const int qb = tl & 1;
-      const long t = (long)(blockIdx.x + (long)tl * gridDim.x) * TM + r;
+      const int qb = tl & 1, rs = tl % QST;
+      mbar_wait(&qr_full[rs], (tl / QST) & 1);
+      const uint8_t* rowp = q_ring + rs * TILE_BYTES + r * 128;
       uint32_t w[32];
-      if (t < M) {
-        const uint4* src = reinterpret_cast<const uint4*>(Q + t * ld + (size_t)h * HD);
 #pragma unroll
-        for (int v = 0; v < 8; ++v) {
-          const uint4 x = __ldg(src + v);
-          w[4 * v] = x.x; w[4 * v + 1] = x.y; w[4 * v + 2] = x.z; w[4 * v + 3] = x.w;
-        }
-      } else {
-#pragma unroll
-        for (int v = 0; v < 32; ++v) w[v] = 0u;
+      for (int c = 0; c < 8; ++c) {
+        const uint4 x = *reinterpret_cast<const uint4*>(rowp + ((c ^ swz) << 4));
+        w[4 * c] = x.x; w[4 * c + 1] = x.y; w[4 * c + 2] = x.z; w[4 * c + 3] = x.w;
       }
+      mbar_arrive(&qr_empty[rs]);
       mbar_wait(&q_empty[qb], ((tl >> 1) & 1) ^ 1);
       tc_fence_after();
       tmem_st_x32(tb + lane_base + C_Q + qb * 32, w);
@@ -188,29 +193,34 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __nv_bfloat16*
     };
     auto store_o = [&](int tl) {
       const int ob = tl & 1;
-      const long t = (long)(blockIdx.x + (long)tl * gridDim.x) * TM + r;
       mbar_wait(&o_full[ob], (tl >> 1) & 1);
       tc_fence_after();
-      uint4* dst = reinterpret_cast<uint4*>(O + t * ld + (size_t)h * HD);
-#pragma unroll
-      for (int half = 0; half < 2; ++half) {
-        uint32_t ro[32];
-        tmem_ld_x32(tb + lane_base + C_O + ob * 64 + 32 * half, ro);
-        tc_wait_ld();
-        if (t < M) {
-#pragma unroll
-          for (int v = 0; v < 4; ++v) {
-            uint4 x;
-            x.x = pack_bf16x2(__uint_as_float(ro[8 * v]), __uint_as_float(ro[8 * v + 1]));
-            x.y = pack_bf16x2(__uint_as_float(ro[8 * v + 2]), __uint_as_float(ro[8 * v + 3]));
-            x.z = pack_bf16x2(__uint_as_float(ro[8 * v + 4]), __uint_as_float(ro[8 * v + 5]));
-            x.w = pack_bf16x2(__uint_as_float(ro[8 * v + 6]), __uint_as_float(ro[8 * v + 7]));
-            dst[4 * half + v] = x;
-          }
-        }
-      }
+      uint32_t ro[64];
+      tmem_ld_x32(tb + lane_base + C_O + ob * 64, *reinterpret_cast<uint32_t(*)[32]>(&ro[0]));
+      tmem_ld_x32(tb + lane_base + C_O + ob * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&ro[32]));
+      tc_wait_ld();
       tc_fence_before();
-      mbar_arrive(&o_empty[ob]);
+      mbar_arrive(&o_empty[ob]);                               // TMEM buffer is free again
+      // staging buffer `ob` was last used by tile tl-2: its TMA store must have read it
+      if (tid == 12 * 32) tma_store_wait_read<1>();
+      asm volatile("bar.sync 2, 128;" ::: "memory");
+      uint8_t* rowp = o_stage + ob * TILE_BYTES + r * 128;
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        uint4 x;
+        x.x = pack_bf16x2(__uint_as_float(ro[8 * c]), __uint_as_float(ro[8 * c + 1]));
+        x.y = pack_bf16x2(__uint_as_float(ro[8 * c + 2]), __uint_as_float(ro[8 * c + 3]));
+        x.z = pack_bf16x2(__uint_as_float(ro[8 * c + 4]), __uint_as_float(ro[8 * c + 5]));
+        x.w = pack_bf16x2(__uint_as_float(ro[8 * c + 6]), __uint_as_float(ro[8 * c + 7]));
+        *reinterpret_cast<uint4*>(rowp + ((c ^ swz) << 4)) = x;
+      }
+      fence_proxy_async_smem();
+      asm volatile("bar.sync 2, 128;" ::: "memory");
+      if (tid == 12 * 32) {
+        tma_store_2d(&mapO, o_stage + ob * TILE_BYTES, h * HD,
+                     ((int)blockIdx.x + tl * (int)gridDim.x) * TM);
+        tma_store_commit();
+      }
     };
     if (my_tiles > 0) load_q(0);
     if (my_tiles > 1) load_q(1);
@@ -218,6 +228,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __nv_bfloat16*
       store_o(tl);
       if (tl + 2 < my_tiles) load_q(tl + 2);
     }
+    if (tid == 12 * 32) tma_store_wait<0>();
   }
   tc_fence_before();
   __syncthreads();
@@ -232,10 +243,14 @@ int bf16_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M
   int per_head = ctx->sm_count / c.nh;
   if (per_head < 1) per_head = 1;
   if (per_head > tiles) per_head = tiles;
-  CUtensorMap mapW;
+  CUtensorMap mapW, mapQ, mapO;
   int rc = make_token_map(ctx, &mapW, ctx->Wb, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, 64);
   if (rc != TTT_OK) return rc;
-  const size_t smem = (size_t)3 * c.hidden * 128 + 1024;
+  rc = make_token_map(ctx, &mapQ, Q, M, (int64_t)c.nh * c.hd, ld, app::TM);
+  if (rc != TTT_OK) return rc;
+  rc = make_token_map(ctx, &mapO, O, M, (int64_t)c.nh * c.hd, ld, app::TM);
+  if (rc != TTT_OK) return rc;
+  const size_t smem = (size_t)3 * c.hidden * 128 + (app::QST + 2) * app::TILE_BYTES + 1024;
   static size_t attr_smem = 0;
   if (smem > attr_smem) {
     TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_apply_kernel,
@@ -244,8 +259,7 @@ int bf16_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M
     attr_smem = smem;
   }
   dim3 grid(per_head, c.nh);
-  bf16_apply_kernel<<<grid, app::THREADS, smem, s>>>(mapW, Q, O, (int)M, (long)ld, c.nh, c.hidden,
-                                                     tiles);
+  bf16_apply_kernel<<<grid, app::THREADS, smem, s>>>(mapW, mapQ, mapO, c.nh, c.hidden, tiles);
   TTT_LAUNCH_CHECK(ctx, "bf16_apply_kernel");
   return TTT_OK;
 }

@@ -14,8 +14,10 @@
 // CTA's whole token range; one fp32 partial per CTA goes to HBM/L2 and is summed in a fixed order
 // by the commit kernel (deterministic, no float atomics).
 //
-// Warp roles (384 threads): warp 0 = TMA producer, warp 1 = MMA issuer, warps 4-7 / 8-11 = two
-// epilogue warpgroups that alternate token tiles (TMEM accumulators are double-buffered).
+// Warp roles (384 threads): warp 0 = TMA producer, warp 1 = MMA issuer, warp 2 = learning-rate
+// loader (-eta of each tile into the stage's shared-memory slot), warps 4-7 / 8-11 = two epilogue
+// warpgroups that alternate token tiles (TMEM accumulators are double-buffered). The epilogue math
+// is packed fp32x2 (FFMA2/FMUL2): two tokens of one hidden unit per instruction.
 #include <stdio.h>
 
 #include "tc_common.cuh"
@@ -36,29 +38,12 @@ constexpr uint32_t C_G1 = 96, C_G3 = 160, C_G2 = 224;     // fp32 gradient accum
 constexpr uint32_t C_BUF = 288, BUF_STRIDE = 96;          // two forward buffers: A | B | g, 32 cols each
 }  // namespace upd
 
-#ifndef TTT_SIGMOID_TANH
-#define TTT_SIGMOID_TANH 1
-#endif
-
-// sigmoid on the MUFU: one tanh (default) or ex2 + rcp
-__device__ __forceinline__ float fast_sigmoid(float a) {
-#if TTT_SIGMOID_TANH
-  float th;
-  asm("tanh.approx.f32 %0, %1;" : "=f"(th) : "f"(0.5f * a));
-  return fmaf(0.5f, th, 0.5f);
-#else
-  float e, r;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(a * -1.4426950408889634f));
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
-  return r;
-#endif
-}
-
+template <bool LOSS>
 __global__ void __launch_bounds__(upd::THREADS, 1)
 bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
                    const __nv_bfloat16* __restrict__ Wb, const float* __restrict__ lr,
                    float* __restrict__ P, float* __restrict__ loss_part, int M, int nh, int H,
-                   int tiles_total, int tiles_per_split, int want_loss) {
+                   int tiles_total, int tiles_per_split) {
   using namespace upd;
   constexpr int HD = 64;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -67,6 +52,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   __shared__ uint64_t full[STAGES], empty[STAGES], fwd_full[2], epi_done[2], w_ready, grad_done;
   __shared__ uint32_t tmem_base_s;
   __shared__ float loss_red[8];
+  __shared__ __align__(16) float ne_s[STAGES][T];   // -eta of the stage's tokens (0 beyond M)
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int split = blockIdx.x, slice = blockIdx.y, h = blockIdx.z;
@@ -75,7 +61,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   const int ntiles = min(tiles_per_split, tiles_total - tile_lo);
 
   if (tid == 0) {
-    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 2); mbar_init(&empty[s], 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 128); }
     mbar_init(&w_ready, 128);
     mbar_init(&grad_done, 1);
@@ -153,6 +139,18 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       }
       tc_commit(&grad_done);
     }
+  } else if (warp == 2) {
+    // ===================== learning-rate loader =====================
+    const float* lrh = lr + (size_t)h * M;
+    for (int i = 0; i < ntiles; ++i) {
+      const int s = i % STAGES, it = i / STAGES;
+      const int t = (tile_lo + i) * T + lane;
+      const float v = (t < M) ? -__ldg(lrh + t) : 0.f;
+      mbar_wait(&empty[s], (it & 1) ^ 1);
+      ne_s[s][lane] = v;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&full[s]);
+    }
   } else if (warp >= 4) {
     // ===================== epilogue warpgroups =====================
     const int wg = (warp - 4) >> 2, q = warp & 3;
@@ -178,49 +176,44 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       tc_fence_before();
       mbar_arrive(&w_ready);
     }
-    float loss = 0.f;
-    const float* lrh = lr + (size_t)h * M;
+    uint64_t loss2 = 0ull;
+    const uint64_t HALF2 = pack2(0.5f, 0.5f), NHALF2 = pack2(-0.5f, -0.5f);
     for (int i = wg; i < ntiles; i += 2) {
-      const int b = i & 1, n = i >> 1;
-      const int t0 = (tile_lo + i) * T;
+      const int b = i & 1, n = i >> 1, s = i % STAGES;
       const uint32_t buf = tb + lane_base + C_BUF + b * BUF_STRIDE;
       mbar_wait(&fwd_full[b], n & 1);
+      mbar_wait(&full[s], (i / STAGES) & 1);     // direct acquire of the loader's -eta slot
       tc_fence_after();
+      const uint2* nes = reinterpret_cast<const uint2*>(&ne_s[s][0]);
 #pragma unroll
       for (int half = 0; half < 2; ++half) {
         uint32_t ra[16], rb[16], rg[16];
         tmem_ld_x16(buf + 16 * half, ra);
         tmem_ld_x16(buf + 32 + 16 * half, rb);
         tmem_ld_x16(buf + 64 + 16 * half, rg);
-        float ne[16];
-#pragma unroll
-        for (int c = 0; c < 16; ++c) {
-          const int t = t0 + 16 * half + c;
-          ne[c] = (t < M) ? -__ldg(lrh + t) : 0.f;
-        }
         tc_wait_ld();
         uint32_t pa[8], pb[8], ph[8];
 #pragma unroll
         for (int c = 0; c < 16; c += 2) {
-          float oa[2], ob[2], oh[2];
-#pragma unroll
-          for (int u = 0; u < 2; ++u) {
-            const float a = __uint_as_float(ra[c + u]);
-            const float bb = __uint_as_float(rb[c + u]);
-            const float g = __uint_as_float(rg[c + u]);
-            const float s = fast_sigmoid(a);
-            const float S = a * s;                       // SiLU(a)
-            const float hdv = S * bb;                    // hidden activation Hd
-            const float dhd = ne[c + u] * g;             // dHd = (-eta v) W2^T
-            const float t2 = fmaf(-S, s, S) + s;         // SiLU'(a) = s + S (1 - s)
-            oa[u] = (dhd * bb) * t2;                     // dA
-            ob[u] = dhd * S;                             // dB
-            oh[u] = ne[c + u] * hdv;                     // Hd' = -eta Hd
-            loss = fmaf(hdv, dhd, loss);
-          }
-          pa[c >> 1] = pack_bf16x2(oa[0], oa[1]);
-          pb[c >> 1] = pack_bf16x2(ob[0], ob[1]);
-          ph[c >> 1] = pack_bf16x2(oh[0], oh[1]);
+          const uint64_t a = pack2u(ra[c], ra[c + 1]);
+          const uint64_t bb = pack2u(rb[c], rb[c + 1]);
+          const uint64_t g = pack2u(rg[c], rg[c + 1]);
+          const uint2 nev = nes[8 * half + (c >> 1)];
+          const uint64_t ne = pack2u(nev.x, nev.y);
+          // sigmoid(a) = 0.5 tanh(a/2) + 0.5 on the MUFU; 1 - sigmoid = 0.5 - 0.5 tanh(a/2)
+          float x0, x1;
+          unpack2(fmul2(a, HALF2), x0, x1);
+          const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
+          const uint64_t sg = ffma2(th, HALF2, HALF2);
+          const uint64_t om = ffma2(th, NHALF2, HALF2);
+          const uint64_t S = fmul2(a, sg);                 // SiLU(a)
+          const uint64_t t2 = ffma2(S, om, sg);            // SiLU'(a) = s + S (1 - s)
+          const uint64_t hdv = fmul2(S, bb);               // hidden activation Hd
+          const uint64_t dhd = fmul2(ne, g);               // dHd = (-eta v) W2^T
+          pa[c >> 1] = pack_bf16x2_from2(fmul2(fmul2(dhd, bb), t2));   // dA
+          pb[c >> 1] = pack_bf16x2_from2(fmul2(dhd, S));               // dB
+          ph[c >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));              // Hd' = -eta Hd
+          if (LOSS) loss2 = ffma2(hdv, dhd, loss2);
         }
         // bf16 operands overwrite the first 16 columns of their own fp32 sources
         tmem_st_x8(buf + 8 * half, pa);
@@ -254,7 +247,10 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     };
     if (wg == 0) { flush(C_G1, 0, 0, 64); flush(C_G2, 1, 0, 32); }
     else         { flush(C_G3, 2, 0, 64); flush(C_G2, 1, 32, 32); }
-    if (want_loss) {
+    if (LOSS) {
+      float l0, l1;
+      unpack2(loss2, l0, l1);
+      float loss = l0 + l1;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) loss += __shfl_xor_sync(0xffffffffu, loss, o);
       if (lane == 0) loss_red[warp - 4] = loss;
@@ -319,8 +315,8 @@ int bf16_partials_needed(const ttt_ctx* ctx, int64_t M) {
 
 int bf16_supported(const ttt_config* cfg, char* why, size_t why_len) {
   if (cfg->hd != 64) { snprintf(why, why_len, "bf16 path: hd must be 64 (got %d)", cfg->hd); return 0; }
-  if (cfg->hidden % 128 != 0 || cfg->hidden < 128 || cfg->hidden > 512) {
-    snprintf(why, why_len, "bf16 path: hidden must be a multiple of 128 in [128, 512] (got %d)", cfg->hidden);
+  if (cfg->hidden % 128 != 0 || cfg->hidden < 128 || cfg->hidden > 256) {
+    snprintf(why, why_len, "bf16 path: hidden must be 128 or 256 (got %d)", cfg->hidden);
     return 0;
   }
   if (cfg->linear_fast_weight) { snprintf(why, why_len, "bf16 path: linear test mode is f32-only"); return 0; }
@@ -341,7 +337,10 @@ int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V
   const size_t smem = (size_t)upd::STAGES * 2 * upd::TILE_BYTES + 1024;
   static bool attr_set = false;
   if (!attr_set) {
-    TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_update_kernel,
+    TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_update_kernel<false>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
+                 "bf16_update_kernel smem attr");
+    TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_update_kernel<true>,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
                  "bf16_update_kernel smem attr");
     attr_set = true;
@@ -349,9 +348,14 @@ int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V
   const int nslices = c.hidden / upd::HS;
   float* P = ctx->partials + (size_t)ctx->n_partials * 3 * ctx->mat_elems;
   dim3 grid(splits, nslices, c.nh);
-  bf16_update_kernel<<<grid, upd::THREADS, smem, s>>>(mapK, mapV, ctx->Wb, lr, P, ctx->loss_part,
-                                                      (int)M, c.nh, c.hidden, tiles, tps,
-                                                      want_loss ? 1 : 0);
+  if (want_loss)
+    bf16_update_kernel<true><<<grid, upd::THREADS, smem, s>>>(mapK, mapV, ctx->Wb, lr, P,
+                                                             ctx->loss_part, (int)M, c.nh,
+                                                             c.hidden, tiles, tps);
+  else
+    bf16_update_kernel<false><<<grid, upd::THREADS, smem, s>>>(mapK, mapV, ctx->Wb, lr, P,
+                                                              ctx->loss_part, (int)M, c.nh,
+                                                              c.hidden, tiles, tps);
   TTT_LAUNCH_CHECK(ctx, "bf16_update_kernel");
   *used = splits;
   *loss_rows = splits * nslices;

@@ -27,74 +27,88 @@ __device__ __forceinline__ float warp_sum(float v) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// ttt_init: user layout -> hidden-major masters + bf16 copies + initial fan-in norms.
-// grid (ceil(H/32), nh, 3), block (32, 8). A 32x32 smem tile transposes W1/W3 ([hd][H] -> [H][hd]).
+// ttt_init: user layout -> hidden-major masters + bf16 copies + initial fan-in norms, fused.
+// grid (ceil(H/32), nh, 3), block (32, 8): a CTA owns 32 hidden rows of one matrix. A 32x32 smem
+// tile transposes W1/W3 ([hd][H] -> [H][hd]). Fan-in norms (DESIGN.md R-RENORM):
+//   mat 0/2: n0[h][j] = ||row j||  (length hd)   -> finished here (a warp owns whole rows)
+//   mat 1  : n0[h][o] = ||column o|| (length H)  -> per-CTA partial sums of squares to colsq,
+//            finished by init_colnorm_kernel in a fixed order.
 // ------------------------------------------------------------------------------------------------
 __global__ void init_load_kernel(const float* __restrict__ W1, const float* __restrict__ W2,
                                  const float* __restrict__ W3, float* __restrict__ Wm,
-                                 __nv_bfloat16* __restrict__ Wb, int nh, int hd, int H) {
+                                 __nv_bfloat16* __restrict__ Wb, float* __restrict__ n0,
+                                 float* __restrict__ colsq, int nh, int hd, int H) {
   __shared__ float tile[32][33];
+  __shared__ float cs[8][128];
   const int mat = blockIdx.z, h = blockIdx.y, j0 = blockIdx.x * 32;
+  const int tx = threadIdx.x, ty = threadIdx.y;
   const size_t me = (size_t)nh * H * hd;
   float* dst = Wm + mat * me + (size_t)h * H * hd;
   __nv_bfloat16* dstb = Wb + mat * me + (size_t)h * H * hd;
-  if (mat == 1) {  // W2 [H][hd]: straight copy
+  if (mat == 1) {  // W2 [H][hd]: straight copy + column sums of squares over this CTA's rows
     const float* src = W2 + (size_t)h * H * hd;
-    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-      int j = j0 + r;
+    float colacc[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int r = ty; r < 32; r += 8) {
+      const int j = j0 + r;
       if (j >= H) break;
-      for (int i = threadIdx.x; i < hd; i += 32) {
-        float v = src[(size_t)j * hd + i];
-        dst[(size_t)j * hd + i] = v;
-        dstb[(size_t)j * hd + i] = __float2bfloat16_rn(v);
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const int i = tx + 32 * c;
+        if (i < hd) {
+          const float v = src[(size_t)j * hd + i];
+          dst[(size_t)j * hd + i] = v;
+          dstb[(size_t)j * hd + i] = __float2bfloat16_rn(v);
+          colacc[c] = fmaf(v, v, colacc[c]);
+        }
       }
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c) cs[ty][tx + 32 * c] = colacc[c];
+    __syncthreads();
+    for (int i = ty * 32 + tx; i < hd; i += 256) {
+      float t = 0.f;
+      for (int w = 0; w < 8; ++w) t += cs[w][i];
+      colsq[((size_t)h * gridDim.x + blockIdx.x) * hd + i] = t;
     }
     return;
   }
   const float* src = (mat == 0 ? W1 : W3) + (size_t)h * hd * H;  // [hd][H]
+  float rowacc[4] = {0.f, 0.f, 0.f, 0.f};                        // rows j0 + ty + 8k
   for (int i0 = 0; i0 < hd; i0 += 32) {
-    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-      int i = i0 + r, j = j0 + threadIdx.x;
-      tile[r][threadIdx.x] = (i < hd && j < H) ? src[(size_t)i * H + j] : 0.f;
+    for (int r = ty; r < 32; r += 8) {
+      const int i = i0 + r, j = j0 + tx;
+      tile[r][tx] = (i < hd && j < H) ? src[(size_t)i * H + j] : 0.f;
     }
     __syncthreads();
-    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-      int j = j0 + r, i = i0 + threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int r = ty + 8 * k, j = j0 + r, i = i0 + tx;
       if (j < H && i < hd) {
-        float v = tile[threadIdx.x][r];
+        const float v = tile[tx][r];
         dst[(size_t)j * hd + i] = v;
         dstb[(size_t)j * hd + i] = __float2bfloat16_rn(v);
+        rowacc[k] = fmaf(v, v, rowacc[k]);
       }
     }
     __syncthreads();
   }
+  float* out = n0 + (mat == 0 ? (size_t)h * H : (size_t)nh * H + (size_t)nh * hd + (size_t)h * H);
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const float t = warp_sum(rowacc[k]);
+    const int j = j0 + ty + 8 * k;
+    if (tx == 0 && j < H) out[j] = sqrtf(t);
+  }
 }
 
-// initial fan-in norms. grid (nh, 3), block 256.
-//   mat 0/2: n0[h][j] = || Wm[mat][h][j][:] ||   (row norm, length hd)
-//   mat 1  : n0[h][o] = || Wm[1][h][:][o]   ||   (column norm, length H)
-__global__ void init_norms_kernel(const float* __restrict__ Wm, float* __restrict__ n0, int nh,
-                                  int hd, int H) {
-  const int h = blockIdx.x, mat = blockIdx.y;
-  const size_t me = (size_t)nh * H * hd;
-  const float* W = Wm + mat * me + (size_t)h * H * hd;
-  float* out = n0 + (mat == 0 ? (size_t)h * H
-                              : mat == 1 ? (size_t)nh * H + (size_t)h * hd
-                                         : (size_t)nh * H + (size_t)nh * hd + (size_t)h * H);
-  if (mat == 1) {
-    for (int o = threadIdx.x; o < hd; o += blockDim.x) {
-      float acc = 0.f;
-      for (int j = 0; j < H; ++j) { float v = W[(size_t)j * hd + o]; acc = fmaf(v, v, acc); }
-      out[o] = sqrtf(acc);
-    }
-  } else {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
-    for (int j = warp; j < H; j += nw) {
-      float acc = 0.f;
-      for (int i = lane; i < hd; i += 32) { float v = W[(size_t)j * hd + i]; acc = fmaf(v, v, acc); }
-      acc = warp_sum(acc);
-      if (lane == 0) out[j] = sqrtf(acc);
-    }
+// n0[h][o] of W2 from the per-CTA partial column sums of squares. grid (nh), block 128.
+__global__ void init_colnorm_kernel(const float* __restrict__ colsq, float* __restrict__ n0,
+                                    int nblk, int nh, int hd, int H) {
+  const int h = blockIdx.x;
+  for (int i = threadIdx.x; i < hd; i += blockDim.x) {
+    float t = 0.f;
+    for (int b = 0; b < nblk; ++b) t += colsq[((size_t)h * nblk + b) * hd + i];
+    n0[(size_t)nh * H + (size_t)h * hd + i] = sqrtf(t);
   }
 }
 
@@ -249,59 +263,74 @@ newton_schulz_kernel(float* __restrict__ G, int H, int hd, int iters) {
 // ------------------------------------------------------------------------------------------------
 constexpr int CM_ROWS = 16;
 
+// float4 per thread, `tpr` (power of two >= hd/4, <= 32) threads per row, 256/tpr rows per pass.
 __global__ void __launch_bounds__(256)
 commit_kernel(float* __restrict__ Wm, __nv_bfloat16* __restrict__ Wb, const float* __restrict__ G,
               const float* __restrict__ P, int n_sets, int use_G, const float* __restrict__ n0,
-              float* __restrict__ colsq, int renorm, int nh, int hd, int H) {
-  __shared__ float cs[8][128];
+              float* __restrict__ colsq, int renorm, int nh, int hd, int H, int tpr) {
+  __shared__ float4 cs[256];
   const int mat = blockIdx.z, h = blockIdx.y, j0 = blockIdx.x * CM_ROWS;
   const size_t me = (size_t)nh * H * hd, set = 3 * me;
   const size_t base = mat * me + (size_t)h * H * hd;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int rows_per_pass = 256 / tpr;
+  const int rr = threadIdx.x / tpr, c4 = (threadIdx.x % tpr) * 4;
+  const bool col_ok = c4 < hd;
   const float* n0m = n0 + (mat == 0 ? (size_t)h * H
                                     : (size_t)nh * H + (size_t)nh * hd + (size_t)h * H);
-  float colacc[4] = {0.f, 0.f, 0.f, 0.f};  // hd <= 128: lane owns columns lane + 32*c
-  for (int r = warp; r < CM_ROWS; r += 8) {
+  float4 colacc = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int r = rr; r < CM_ROWS; r += rows_per_pass) {
     const int j = j0 + r;
-    if (j >= H) break;
-    const size_t row = base + (size_t)j * hd;
-    float w[4];
-    float sq = 0.f;
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      const int i = lane + 32 * c;
-      w[c] = 0.f;
-      if (i < hd) {
-        float g = use_G ? G[row + i] : 0.f;
-        for (int s = 0; s < n_sets; ++s) g += P[(size_t)s * set + row + i];
-        w[c] = Wm[row + i] - g;
-        sq = fmaf(w[c], w[c], sq);
+    const bool ok = col_ok && j < H;
+    const size_t e = base + (size_t)j * hd + c4;
+    float4 w = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (ok) {
+      float4 g = use_G ? *reinterpret_cast<const float4*>(G + e) : make_float4(0.f, 0.f, 0.f, 0.f);
+      const float* p = P + e;
+      int s = 0;
+      for (; s + 4 <= n_sets; s += 4) {     // four loads in flight, summed in set order
+        const float4 p0 = *reinterpret_cast<const float4*>(p + (size_t)s * set);
+        const float4 p1 = *reinterpret_cast<const float4*>(p + (size_t)(s + 1) * set);
+        const float4 p2 = *reinterpret_cast<const float4*>(p + (size_t)(s + 2) * set);
+        const float4 p3 = *reinterpret_cast<const float4*>(p + (size_t)(s + 3) * set);
+        g.x += p0.x; g.y += p0.y; g.z += p0.z; g.w += p0.w;
+        g.x += p1.x; g.y += p1.y; g.z += p1.z; g.w += p1.w;
+        g.x += p2.x; g.y += p2.y; g.z += p2.z; g.w += p2.w;
+        g.x += p3.x; g.y += p3.y; g.z += p3.z; g.w += p3.w;
       }
-    }
-    if (renorm && mat != 1) {
-      sq = warp_sum(sq);
-      const float f = n0m[j] / (sqrtf(sq) + 1e-5f);
-#pragma unroll
-      for (int c = 0; c < 4; ++c) w[c] *= f;
-    }
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      const int i = lane + 32 * c;
-      if (i < hd) {
-        Wm[row + i] = w[c];
-        Wb[row + i] = __float2bfloat16_rn(w[c]);
-        colacc[c] = fmaf(w[c], w[c], colacc[c]);
+      for (; s < n_sets; ++s) {
+        const float4 p0 = *reinterpret_cast<const float4*>(p + (size_t)s * set);
+        g.x += p0.x; g.y += p0.y; g.z += p0.z; g.w += p0.w;
       }
+      const float4 w0 = *reinterpret_cast<const float4*>(Wm + e);
+      w = make_float4(w0.x - g.x, w0.y - g.y, w0.z - g.z, w0.w - g.w);
+    }
+    if (renorm && mat != 1) {               // row fan-in: scale the row back to its initial norm
+      float sq = w.x * w.x + w.y * w.y + w.z * w.z + w.w * w.w;
+      for (int o = tpr >> 1; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+      const float f = (j < H) ? n0m[j] / (sqrtf(sq) + 1e-5f) : 0.f;
+      w.x *= f; w.y *= f; w.z *= f; w.w *= f;
+    }
+    if (ok) {
+      *reinterpret_cast<float4*>(Wm + e) = w;
+      __nv_bfloat162 lo = __floats2bfloat162_rn(w.x, w.y), hi = __floats2bfloat162_rn(w.z, w.w);
+      uint2 packed;
+      packed.x = *reinterpret_cast<uint32_t*>(&lo);
+      packed.y = *reinterpret_cast<uint32_t*>(&hi);
+      *reinterpret_cast<uint2*>(Wb + e) = packed;
+      colacc.x = fmaf(w.x, w.x, colacc.x); colacc.y = fmaf(w.y, w.y, colacc.y);
+      colacc.z = fmaf(w.z, w.z, colacc.z); colacc.w = fmaf(w.w, w.w, colacc.w);
     }
   }
-  if (renorm && mat == 1) {
-#pragma unroll
-    for (int c = 0; c < 4; ++c) cs[warp][lane + 32 * c] = colacc[c];
+  if (renorm && mat == 1) {                 // column fan-in: per-CTA partial sums of squares
+    cs[threadIdx.x] = colacc;
     __syncthreads();
-    for (int i = threadIdx.x; i < hd; i += blockDim.x) {
-      float t = 0.f;
-      for (int w8 = 0; w8 < 8; ++w8) t += cs[w8][i];
-      colsq[((size_t)h * gridDim.x + blockIdx.x) * hd + i] = t;
+    if (threadIdx.x < tpr && col_ok) {
+      float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
+      for (int r = 0; r < rows_per_pass; ++r) {
+        const float4 v = cs[r * tpr + threadIdx.x];
+        t.x += v.x; t.y += v.y; t.z += v.z; t.w += v.w;
+      }
+      *reinterpret_cast<float4*>(colsq + ((size_t)h * gridDim.x + blockIdx.x) * hd + c4) = t;
     }
   }
 }
@@ -338,10 +367,11 @@ renorm_w2_kernel(float* __restrict__ Wm, __nv_bfloat16* __restrict__ Wb,
 int launch_init(ttt_ctx* ctx, const float* W1, const float* W2, const float* W3, cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
   dim3 grid((c.hidden + 31) / 32, c.nh, 3), block(32, 8);
-  init_load_kernel<<<grid, block, 0, s>>>(W1, W2, W3, ctx->Wm, ctx->Wb, c.nh, c.hd, c.hidden);
+  init_load_kernel<<<grid, block, 0, s>>>(W1, W2, W3, ctx->Wm, ctx->Wb, ctx->n0, ctx->colsq, c.nh,
+                                          c.hd, c.hidden);
   TTT_LAUNCH_CHECK(ctx, "init_load_kernel");
-  init_norms_kernel<<<dim3(c.nh, 3), 256, 0, s>>>(ctx->Wm, ctx->n0, c.nh, c.hd, c.hidden);
-  TTT_LAUNCH_CHECK(ctx, "init_norms_kernel");
+  init_colnorm_kernel<<<c.nh, 128, 0, s>>>(ctx->colsq, ctx->n0, (int)grid.x, c.nh, c.hd, c.hidden);
+  TTT_LAUNCH_CHECK(ctx, "init_colnorm_kernel");
   return TTT_OK;
 }
 
@@ -393,9 +423,12 @@ int launch_commit(ttt_ctx* ctx, cudaStream_t s) {
     TTT_LAUNCH_CHECK(ctx, "newton_schulz_kernel");
   }
   const int nblk = (c.hidden + CM_ROWS - 1) / CM_ROWS;
+  int tpr = 1;
+  while (tpr * 4 < c.hd) tpr <<= 1;
   commit_kernel<<<dim3(nblk, c.nh, 3), 256, 0, s>>>(ctx->Wm, ctx->Wb, ctx->G, ctx->partials,
                                                     ctx->n_partials, ctx->G_valid ? 1 : 0, ctx->n0,
-                                                    ctx->colsq, c.renorm, c.nh, c.hd, c.hidden);
+                                                    ctx->colsq, c.renorm, c.nh, c.hd, c.hidden,
+                                                    tpr);
   TTT_LAUNCH_CHECK(ctx, "commit_kernel");
   if (c.renorm) {
     renorm_w2_kernel<<<dim3(nblk, c.nh), 256, 0, s>>>(ctx->Wm, ctx->Wb, ctx->colsq, ctx->n0, nblk,
