@@ -16,7 +16,7 @@ import torch
 
 TTT_F32, TTT_BF16 = 0, 1
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libttt_b200.so")
+_LIB_PATH = os.environ.get("TTT_B200_LIB") or os.path.join(_HERE, "libttt_b200.so")  # debug-build override
 _lib = None
 
 EXPORTS = ("ttt_create", "ttt_destroy", "ttt_init", "ttt_update", "ttt_apply", "ttt_chunk_step",

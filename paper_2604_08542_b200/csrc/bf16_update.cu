@@ -23,6 +23,20 @@
 #include "tc_common.cuh"
 #include "ttt_internal.h"
 
+#ifdef TTT_TRACE   // debug builds only: per-tile clock timeline of CTA (0,0,0), staged in smem
+__device__ long long g_ttt_trace[64 * 16];
+#define TTT_TR(i, k)                                                                  \
+  do {                                                                                \
+    if ((i) < 64 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0)            \
+      tr_s[(i) * 16 + (k)] = (unsigned)clock();                                       \
+  } while (0)
+extern "C" int ttt_debug_trace(long long* host) {
+  return (int)cudaMemcpyFromSymbol(host, g_ttt_trace, sizeof(g_ttt_trace));
+}
+#else
+#define TTT_TR(i, k) do { } while (0)
+#endif
+
 namespace ttt {
 
 namespace upd {
@@ -53,6 +67,12 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   __shared__ uint32_t tmem_base_s;
   __shared__ float loss_red[8];
   __shared__ __align__(16) float ne_s[STAGES][T];   // -eta of the stage's tokens (0 beyond M)
+#ifdef TTT_TRACE
+  __shared__ unsigned tr_s[64 * 16];
+  for (int e = threadIdx.x; e < 64 * 16; e += blockDim.x) tr_s[e] = 0;
+  __syncthreads();
+  if (threadIdx.x == 0) tr_s[15] = (unsigned)clock();
+#endif
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int split = blockIdx.x, slice = blockIdx.y, h = blockIdx.z;
@@ -62,8 +82,8 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
 
   if (tid == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 2); mbar_init(&empty[s], 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 128); }
-    mbar_init(&w_ready, 128);
+    for (int b = 0; b < 2; ++b) { mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 8); }
+    mbar_init(&w_ready, 4);
     mbar_init(&grad_done, 1);
     fence_mbar_init();
   }
@@ -72,6 +92,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   __syncthreads();
   tc_fence_after();
   const uint32_t tb = tmem_base_s;
+  if (tid == 0) TTT_TR(0, 14);
 
   if (warp == 0) {
     // ===================== TMA producer =====================
@@ -81,6 +102,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       for (int i = 0; i < ntiles; ++i) {
         const int s = i % STAGES, it = i / STAGES;
         mbar_wait(&empty[s], (it & 1) ^ 1);
+        TTT_TR(i, 12);
         mbar_arrive_expect_tx(&full[s], 2 * TILE_BYTES);
         uint8_t* dst = smem + s * 2 * TILE_BYTES;
         tma_load_2d(dst, &mapK, &full[s], h * HD, (tile_lo + i) * T);
@@ -97,8 +119,10 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       tc_fence_after();
       auto fwd = [&](int i) {
         const int s = i % STAGES, it = i / STAGES, b = i & 1;
+        TTT_TR(i, 0);
         mbar_wait(&full[s], it & 1);
         tc_fence_after();
+        TTT_TR(i, 1);
         const uint32_t ks = smem_base + s * 2 * TILE_BYTES, vs = ks + TILE_BYTES;
         const uint32_t acc = tb + C_BUF + b * BUF_STRIDE;
 #pragma unroll
@@ -111,26 +135,29 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         for (int k = 0; k < HD / 16; ++k)
           umma_ts(acc + 64, tb + C_W2 + 8 * k, umma_smem_desc_sw128(vs + 32 * k, 16, 1024), idesc_f, k > 0);
         tc_commit(&fwd_full[b]);
+        TTT_TR(i, 2);
       };
       auto grad = [&](int i) {
         const int s = i % STAGES, b = i & 1, n = i >> 1;
         mbar_wait(&epi_done[b], n & 1);
         tc_fence_after();
+        TTT_TR(i, 3);
         const uint32_t ks = smem_base + s * 2 * TILE_BYTES, vs = ks + TILE_BYTES;
         const uint32_t opnd = tb + C_BUF + b * BUF_STRIDE;   // dA | dB | Hd' alias A | B | g
 #pragma unroll
         for (int k = 0; k < T / 16; ++k)
-          umma_ts(tb + C_G1, opnd + 8 * k, umma_smem_desc_sw128(ks + 2048 * k, TILE_BYTES, 1024),
+          umma_ts(tb + C_G1, opnd + 24 * k, umma_smem_desc_sw128(ks + 2048 * k, TILE_BYTES, 1024),
                   idesc_g, (i > 0 || k > 0));
 #pragma unroll
         for (int k = 0; k < T / 16; ++k)
-          umma_ts(tb + C_G3, opnd + 32 + 8 * k, umma_smem_desc_sw128(ks + 2048 * k, TILE_BYTES, 1024),
+          umma_ts(tb + C_G3, opnd + 32 + 24 * k, umma_smem_desc_sw128(ks + 2048 * k, TILE_BYTES, 1024),
                   idesc_g, (i > 0 || k > 0));
 #pragma unroll
         for (int k = 0; k < T / 16; ++k)
-          umma_ts(tb + C_G2, opnd + 64 + 8 * k, umma_smem_desc_sw128(vs + 2048 * k, TILE_BYTES, 1024),
+          umma_ts(tb + C_G2, opnd + 64 + 24 * k, umma_smem_desc_sw128(vs + 2048 * k, TILE_BYTES, 1024),
                   idesc_g, (i > 0 || k > 0));
         tc_commit(&empty[s]);
+        TTT_TR(i, 4);
       };
       if (ntiles > 0) fwd(0);
       for (int i = 0; i < ntiles; ++i) {
@@ -159,74 +186,87 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     const size_t me = (size_t)nh * H * HD;
     const size_t row = ((size_t)h * H + (size_t)slice * HS + j) * HD;
     if (wg == 0) {
-      // weights -> TMEM as A operands: row j of W1^T, W3^T, W2 (64 bf16 = 32 words each)
+      // weights -> TMEM as A operands: row j of W1^T, W3^T, W2 (64 bf16 = 32 words each);
+      // all 24 loads are issued before the first TMEM store
       const uint32_t cols[3] = {C_W1, C_W2, C_W3};
+      uint4 x[3][8];
 #pragma unroll
       for (int mat = 0; mat < 3; ++mat) {
         const uint4* src = reinterpret_cast<const uint4*>(Wb + mat * me + row);
+#pragma unroll
+        for (int v = 0; v < 8; ++v) x[mat][v] = __ldg(src + v);
+      }
+#pragma unroll
+      for (int mat = 0; mat < 3; ++mat) {
         uint32_t r[32];
 #pragma unroll
         for (int v = 0; v < 8; ++v) {
-          const uint4 x = __ldg(src + v);
-          r[4 * v] = x.x; r[4 * v + 1] = x.y; r[4 * v + 2] = x.z; r[4 * v + 3] = x.w;
+          r[4 * v] = x[mat][v].x; r[4 * v + 1] = x[mat][v].y;
+          r[4 * v + 2] = x[mat][v].z; r[4 * v + 3] = x[mat][v].w;
         }
         tmem_st_x32(tb + lane_base + cols[mat], r);
       }
       tc_wait_st();
       tc_fence_before();
-      mbar_arrive(&w_ready);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&w_ready);
     }
     uint64_t loss2 = 0ull;
     const uint64_t HALF2 = pack2(0.5f, 0.5f), NHALF2 = pack2(-0.5f, -0.5f);
-    for (int i = wg; i < ntiles; i += 2) {
+    for (int i = 0; i < ntiles; ++i) {
+      // both warpgroups work on every tile: warpgroup `wg` owns token columns [16 wg, 16 wg + 16)
       const int b = i & 1, n = i >> 1, s = i % STAGES;
       const uint32_t buf = tb + lane_base + C_BUF + b * BUF_STRIDE;
+      if (q == 0 && lane == 0) TTT_TR(i, 5 + wg);
       mbar_wait(&fwd_full[b], n & 1);
       mbar_wait(&full[s], (i / STAGES) & 1);     // direct acquire of the loader's -eta slot
       tc_fence_after();
+      if (q == 0 && lane == 0) TTT_TR(i, 7 + wg);
       const uint2* nes = reinterpret_cast<const uint2*>(&ne_s[s][0]);
+      uint32_t ra[16], rb[16], rg[16];
+      tmem_ld_x16(buf + 16 * wg, ra);
+      tmem_ld_x16(buf + 32 + 16 * wg, rb);
+      tmem_ld_x16(buf + 64 + 16 * wg, rg);
+      tc_wait_ld();
+      uint32_t pa[8], pb[8], ph[8];
 #pragma unroll
-      for (int half = 0; half < 2; ++half) {
-        uint32_t ra[16], rb[16], rg[16];
-        tmem_ld_x16(buf + 16 * half, ra);
-        tmem_ld_x16(buf + 32 + 16 * half, rb);
-        tmem_ld_x16(buf + 64 + 16 * half, rg);
-        tc_wait_ld();
-        uint32_t pa[8], pb[8], ph[8];
-#pragma unroll
-        for (int c = 0; c < 16; c += 2) {
-          const uint64_t a = pack2u(ra[c], ra[c + 1]);
-          const uint64_t bb = pack2u(rb[c], rb[c + 1]);
-          const uint64_t g = pack2u(rg[c], rg[c + 1]);
-          const uint2 nev = nes[8 * half + (c >> 1)];
-          const uint64_t ne = pack2u(nev.x, nev.y);
-          // sigmoid(a) = 0.5 tanh(a/2) + 0.5 on the MUFU; 1 - sigmoid = 0.5 - 0.5 tanh(a/2)
-          float x0, x1;
-          unpack2(fmul2(a, HALF2), x0, x1);
-          const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
-          const uint64_t sg = ffma2(th, HALF2, HALF2);
-          const uint64_t om = ffma2(th, NHALF2, HALF2);
-          const uint64_t S = fmul2(a, sg);                 // SiLU(a)
-          const uint64_t t2 = ffma2(S, om, sg);            // SiLU'(a) = s + S (1 - s)
-          const uint64_t hdv = fmul2(S, bb);               // hidden activation Hd
-          const uint64_t dhd = fmul2(ne, g);               // dHd = (-eta v) W2^T
-          pa[c >> 1] = pack_bf16x2_from2(fmul2(fmul2(dhd, bb), t2));   // dA
-          pb[c >> 1] = pack_bf16x2_from2(fmul2(dhd, S));               // dB
-          ph[c >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));              // Hd' = -eta Hd
-          if (LOSS) loss2 = ffma2(hdv, dhd, loss2);
-        }
-        // bf16 operands overwrite the first 16 columns of their own fp32 sources
-        tmem_st_x8(buf + 8 * half, pa);
-        tmem_st_x8(buf + 32 + 8 * half, pb);
-        tmem_st_x8(buf + 64 + 8 * half, ph);
+      for (int c = 0; c < 16; c += 2) {
+        const uint64_t a = pack2u(ra[c], ra[c + 1]);
+        const uint64_t bb = pack2u(rb[c], rb[c + 1]);
+        const uint64_t g = pack2u(rg[c], rg[c + 1]);
+        const uint2 nev = nes[8 * wg + (c >> 1)];
+        const uint64_t ne = pack2u(nev.x, nev.y);
+        // sigmoid(a) = 0.5 tanh(a/2) + 0.5 on the MUFU; 1 - sigmoid = 0.5 - 0.5 tanh(a/2)
+        float x0, x1;
+        unpack2(fmul2(a, HALF2), x0, x1);
+        const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
+        const uint64_t sg = ffma2(th, HALF2, HALF2);
+        const uint64_t om = ffma2(th, NHALF2, HALF2);
+        const uint64_t S = fmul2(a, sg);                 // SiLU(a)
+        const uint64_t t2 = ffma2(S, om, sg);            // SiLU'(a) = s + S (1 - s)
+        const uint64_t hdv = fmul2(S, bb);               // hidden activation Hd
+        const uint64_t dhd = fmul2(ne, g);               // dHd = (-eta v) W2^T
+        pa[c >> 1] = pack_bf16x2_from2(fmul2(fmul2(dhd, bb), t2));   // dA
+        pb[c >> 1] = pack_bf16x2_from2(fmul2(dhd, S));               // dB
+        ph[c >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));              // Hd' = -eta Hd
+        if (LOSS) loss2 = ffma2(hdv, dhd, loss2);
       }
+      // bf16 operands overwrite fp32 columns this warp itself has just read: tokens [16 wg, +16)
+      // of dA / dB / Hd' go to columns [24 wg, 24 wg + 8) of the A / B / g regions
+      tmem_st_x8(buf + 24 * wg, pa);
+      tmem_st_x8(buf + 32 + 24 * wg, pb);
+      tmem_st_x8(buf + 64 + 24 * wg, ph);
       tc_wait_st();
       tc_fence_before();
-      mbar_arrive(&epi_done[b]);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&epi_done[b]);
+      if (q == 0 && lane == 0) TTT_TR(i, 9 + wg);
     }
     // ---- flush the gradient accumulators: one fp32 partial slice per CTA ----
+    if (warp == 4 && lane == 0) TTT_TR(2, 13);
     mbar_wait(&grad_done, 0);
     tc_fence_after();
+    if (warp == 4 && lane == 0) TTT_TR(2, 14);
     float* Pset = P + (size_t)split * 3 * me;
     auto flush = [&](uint32_t col, int mat, int c0, int ncols) {
       float4* dst = reinterpret_cast<float4*>(Pset + mat * me + row + c0);
@@ -247,6 +287,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     };
     if (wg == 0) { flush(C_G1, 0, 0, 64); flush(C_G2, 1, 0, 32); }
     else         { flush(C_G3, 2, 0, 64); flush(C_G2, 1, 32, 32); }
+    if (warp == 4 && lane == 0) TTT_TR(2, 15);
     if (LOSS) {
       float l0, l1;
       unpack2(loss2, l0, l1);
@@ -265,6 +306,12 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   tc_fence_before();
   __syncthreads();
   if (warp == 0) tmem_dealloc(tb, 512);
+#ifdef TTT_TRACE
+  if (threadIdx.x == 0) tr_s[16 + 15] = (unsigned)clock();
+  __syncthreads();
+  if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0)
+    for (int e = threadIdx.x; e < 64 * 16; e += blockDim.x) g_ttt_trace[e] = tr_s[e];
+#endif
 }
 
 // ------------------------------------------------------------------------------------------------
