@@ -168,15 +168,35 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     }
   } else if (warp == 2) {
     // ===================== learning-rate loader =====================
+    // -eta of tile i (32 tokens = one 128-B line of lr) goes to the stage's shared-memory slot.
+    // The global loads run LRPF tiles ahead of the ring (register double buffer), so their
+    // latency is never on the critical path of a tile.
+    constexpr int LRPF = 8;
     const float* lrh = lr + (size_t)h * M;
-    for (int i = 0; i < ntiles; ++i) {
-      const int s = i % STAGES, it = i / STAGES;
-      const int t = (tile_lo + i) * T + lane;
-      const float v = (t < M) ? -__ldg(lrh + t) : 0.f;
-      mbar_wait(&empty[s], (it & 1) ^ 1);
-      ne_s[s][lane] = v;
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&full[s]);
+    auto ld_batch = [&](int i0, float (&v)[LRPF]) {
+#pragma unroll
+      for (int u = 0; u < LRPF; ++u) {
+        const int t = (tile_lo + i0 + u) * T + lane;
+        v[u] = (i0 + u < ntiles && t < M) ? -__ldg(lrh + t) : 0.f;
+      }
+    };
+    float cur[LRPF], nxt[LRPF];
+    ld_batch(0, cur);
+    for (int i0 = 0; i0 < ntiles; i0 += LRPF) {
+      ld_batch(i0 + LRPF, nxt);
+#pragma unroll
+      for (int u = 0; u < LRPF; ++u) {
+        const int i = i0 + u;
+        if (i < ntiles) {
+          const int s = i % STAGES, it = i / STAGES;
+          mbar_wait(&empty[s], (it & 1) ^ 1);
+          ne_s[s][lane] = cur[u];
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&full[s]);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < LRPF; ++u) cur[u] = nxt[u];
     }
   } else if (warp >= 4) {
     // ===================== epilogue warpgroups =====================
