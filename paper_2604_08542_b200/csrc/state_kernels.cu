@@ -405,7 +405,10 @@ int launch_loss_reduce(ttt_ctx* ctx, int n, float* loss, cudaStream_t s) {
 
 int launch_commit(ttt_ctx* ctx, cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
-  if (c.ns_iters > 0) {
+  if (c.ns_iters > 0 && ns_tc_supported(&c)) {
+    int rc = launch_ns_tc(ctx, s);      // tensor-core NS; folds the partial sets into G itself
+    if (rc != TTT_OK) return rc;
+  } else if (c.ns_iters > 0) {
     int rc = launch_reduce_pending(ctx, s);
     if (rc != TTT_OK) return rc;
     const size_t smem = ((size_t)2 * c.hd * (c.hd + 1) + (size_t)NS_ROWS * (c.hd + 1) +

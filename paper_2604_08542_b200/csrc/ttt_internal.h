@@ -59,6 +59,11 @@ int launch_commit(ttt_ctx* ctx, cudaStream_t s);
 // loss[h] = sum_{r in [0, n)} loss_part[r][h]  (fixed order)
 int launch_loss_reduce(ttt_ctx* ctx, int n, float* loss, cudaStream_t s);
 
+// --- tensor-core Newton-Schulz (ns_tc.cu) ---------------------------------------------------------
+int ns_tc_supported(const ttt_config* cfg);
+// G = NS((G_valid ? G : 0) + sum partials) for all 3*nh matrices; marks G_valid, clears n_partials
+int launch_ns_tc(ttt_ctx* ctx, cudaStream_t s);
+
 // --- f32 path (f32_path.cu) ---------------------------------------------------------------------
 // appends partial-gradient sets [n_partials, n_partials + used); writes loss_part rows [0, loss_rows)
 int f32_accumulate(ttt_ctx* ctx, const float* K, const float* V, const float* lr, int64_t M,

@@ -160,6 +160,28 @@ def test_bf16_gradient_against_oracle():
     gpu.close()
 
 
+@pytest.mark.parametrize("H", [128, 256])
+def test_bf16_newton_schulz_kernel_against_oracle(H):
+    """The tensor-core Newton-Schulz kernel in isolation: W0 - W' after a commit must equal the
+    oracle's NS of the very gradient the GPU holds (ttt_pending_gradient), to split-bf16 accuracy."""
+    from oracle.ttt_oracle import newton_schulz
+    dev = torch.device("cuda", 0)
+    w = _bf16_workload("cfg3", nh=2, hidden=H, tokens_per_frame=300, frames_per_chunk=2, n_frames=2)
+    W1, W2, W3 = ti.fast_weights(w)
+    Q, K, V, lr = ti.TokenStream(w).next_chunk()
+    gpu = _mk(w)
+    gpu.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    gpu.ttt_accumulate(K.to(dev), V.to(dev), lr.to(dev))
+    G = gpu.ttt_pending_gradient().cpu().clone()                 # [3, nh, H, hd], hidden-major
+    gpu.ttt_commit()
+    n1, n2, n3 = (x.cpu().double() for x in gpu.ttt_get_weights())
+    ns = newton_schulz(G.reshape(-1, H, w.hd).numpy(), 5).reshape(3, w.nh, H, w.hd)
+    assert rel_err(W1.double() - n1, np.swapaxes(ns[0], 1, 2)) <= 2e-4
+    assert rel_err(W2.double() - n2, ns[1]) <= 2e-4
+    assert rel_err(W3.double() - n3, np.swapaxes(ns[2], 1, 2)) <= 2e-4
+    gpu.close()
+
+
 def test_bf16_apply_only_and_head_independence():
     dev = torch.device("cuda", 0)
     w = _bf16_workload("cfg2", nh=4, tokens_per_frame=129, frames_per_chunk=3, n_frames=3)
