@@ -15,61 +15,66 @@
 // tcgen05 mapping (hd = 64; all operands in shared memory, 128-byte swizzle, fp32 accumulators in
 // TMEM). X is kept as two bf16 tiles XH, XL [H rows][64], AL follows AH, XL follows XH, so that a
 // 128-row operand is "hi stacked on lo":
-//   Gram   D[128 x 64] = [XH | XL]^T (MN-major A, second 64-wide atom at LBO) . XH  then . XL
-//          rows 0-63 = hi*hi + hi*lo, rows 64-127 = lo*hi + lo*lo;  A = top + bottom
-//   square D[128 x 64] = [AH ; AL] (K-major A, 128 rows) . AH  then . AL;   A A = top + bottom
-//   tall   D_mb[128 x 64] = XH_mb . PH + XH_mb . PL + XL_mb . PH        per 128-row block mb
-// Phases are sequential (each product depends on the previous one): one elected thread issues the
-// MMAs and commits to an mbarrier, all 8 warps run the TMEM -> registers -> split -> shared epilogue.
+//   Gram   D[128 x 128] = [XH | XL]^T . [XH | XL]   (MN-major A and B, second 64-wide atom at LBO)
+//          four 64 x 64 blocks hh, hl / lh, ll in ONE MMA per 16 rows;  A = sum of the four blocks
+//   square D[128 x 128] = [AH ; AL] . [AH ; AL]^T  (K-major, 128 rows each);  A A = sum of the blocks
+//   tall   D_mb[128 x 128] = XH_mb . [PH ; PL]^T, then columns 0-63 += XL_mb . PH^T   per 128-row block
+//          X' = left half + right half
+// SS-mode MMAs with a 64-wide dimension are bound by the shared-memory operand port (128 B/clk),
+// which is why the hi/lo halves are stacked into 128-wide operands instead of issued as three
+// 64-wide products. Phases are sequential (each product depends on the previous one): one elected
+// thread issues the MMAs and commits to an mbarrier, all 16 warps run the TMEM -> registers ->
+// split -> shared epilogue (4 warps per TMEM lane quarter, 16 columns each).
 #include <stdio.h>
 
 #include "tc_common.cuh"
 #include "ttt_internal.h"
 
+#ifdef TTT_TRACE
+__device__ long long g_ns_trace[64];
+extern "C" int ttt_debug_ns_trace(long long* host) {
+  return (int)cudaMemcpyFromSymbol(host, g_ns_trace, sizeof(g_ns_trace));
+}
+#define NS_TR(k) do { if (blockIdx.x == 0 && threadIdx.x == 0 && (k) < 64) g_ns_trace[(k)] = clock64(); } while (0)
+#else
+#define NS_TR(k) do { } while (0)
+#endif
+
 namespace ttt {
 
 namespace nstc {
-constexpr int THREADS = 256;
-constexpr uint32_t C_A = 0;      // Gram accumulator        [128 x 64] fp32
-constexpr uint32_t C_A2 = 64;    // A A accumulator         [128 x 64] fp32
-constexpr uint32_t C_X = 128;    // X Pm accumulators, 64 columns per 128-row block
-constexpr int S_LD = 65;         // fp32 exchange scratch row stride (bank-conflict free)
+constexpr int THREADS = 512;
+constexpr uint32_t C_A = 0;      // Gram accumulator   [128 x 128] fp32
+constexpr uint32_t C_A2 = 128;   // A A accumulator    [128 x 128] fp32
+constexpr uint32_t C_X = 0;      // X Pm accumulators, 128 columns per 128-row block (alias C_A, C_A2)
+constexpr int S_LD = 65;         // fp32 exchange scratch row stride in floats (bank-conflict free)
+constexpr int W_LD = 68;         // fp32 commit staging row stride in floats (16-B aligned rows)
 }  // namespace nstc
 
-// hi/lo split of four fp32 values -> two 8-byte words of bf16
-__device__ __forceinline__ void split4(const float (&v)[4], uint2& hi, uint2& lo) {
-  hi.x = pack_bf16x2(v[0], v[1]);
-  hi.y = pack_bf16x2(v[2], v[3]);
-  float r[4];
-  r[0] = v[0] - __uint_as_float(hi.x << 16);
-  r[1] = v[1] - __uint_as_float(hi.x & 0xffff0000u);
-  r[2] = v[2] - __uint_as_float(hi.y << 16);
-  r[3] = v[3] - __uint_as_float(hi.y & 0xffff0000u);
-  lo.x = pack_bf16x2(r[0], r[1]);
-  lo.y = pack_bf16x2(r[2], r[3]);
+// hi/lo split of eight fp32 values -> one 16-byte chunk of bf16 each
+__device__ __forceinline__ void split8(const float (&v)[8], uint4& hi, uint4& lo) {
+  uint32_t h[4], l[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    h[i] = pack_bf16x2(v[2 * i], v[2 * i + 1]);
+    const float r0 = v[2 * i] - __uint_as_float(h[i] << 16);
+    const float r1 = v[2 * i + 1] - __uint_as_float(h[i] & 0xffff0000u);
+    l[i] = pack_bf16x2(r0, r1);
+  }
+  hi = make_uint4(h[0], h[1], h[2], h[3]);
+  lo = make_uint4(l[0], l[1], l[2], l[3]);
 }
 
-// write 32 consecutive columns [c0, c0+32) of row `row` of a [rows][64] bf16 tile pair (hi, lo)
-// in the 128-byte-swizzled layout (16-byte chunk index ^= row & 7)
-__device__ __forceinline__ void store_row32_split(uint8_t* hi_tile, uint8_t* lo_tile, int row, int c0,
-                                                  const float (&v)[32]) {
-  const uint32_t swz = static_cast<uint32_t>(row & 7);
-#pragma unroll
-  for (int k = 0; k < 4; ++k) {            // 4 chunks of 8 columns
-    const float a[4] = {v[8 * k], v[8 * k + 1], v[8 * k + 2], v[8 * k + 3]};
-    const float b[4] = {v[8 * k + 4], v[8 * k + 5], v[8 * k + 6], v[8 * k + 7]};
-    uint2 ha, la, hb, lb;
-    split4(a, ha, la);
-    split4(b, hb, lb);
-    const uint32_t off = row * 128 + (((c0 >> 3) + k) ^ swz) * 16;
-    *reinterpret_cast<uint4*>(hi_tile + off) = make_uint4(ha.x, ha.y, hb.x, hb.y);
-    *reinterpret_cast<uint4*>(lo_tile + off) = make_uint4(la.x, la.y, lb.x, lb.y);
-  }
+// byte offset of 16-byte chunk `chunk` (8 bf16 columns) of row `row` in a 128-byte-swizzled
+// [rows][64] bf16 tile
+__device__ __forceinline__ uint32_t sw128_off(int row, int chunk) {
+  return static_cast<uint32_t>(row * 128 + ((chunk ^ (row & 7)) << 4));
 }
 
 __global__ void __launch_bounds__(nstc::THREADS, 1)
 ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, size_t set_elems,
-             int use_G, int H, int iters, uint32_t tmem_cols) {
+             int use_G, int H, int iters, uint32_t tmem_cols, float* __restrict__ Wm,
+             __nv_bfloat16* __restrict__ Wb) {
   using namespace nstc;
   constexpr int HD = 64;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -88,26 +93,55 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
   uint8_t* AL = AH + 8192;
   uint8_t* PH = AL + 8192;
   uint8_t* PL = PH + 8192;
-  float* S = reinterpret_cast<float*>(PL + 8192);          // [64][S_LD]
+  float* S = reinterpret_cast<float*>(PL + 8192);          // [128][S_LD]
 
+  NS_TR(0);
   if (tid == 0) { mbar_init(&mma_bar, 1); fence_mbar_init(); }
   if (warp == 0) { tmem_alloc(&tmem_base_s, tmem_cols); tmem_relinquish(); }
+  NS_TR(59);
 
-  // ---- load: g = (use_G ? G : 0) + sum_s P[s], written back to G; Frobenius norm ----
+  // ---- load: g = (use_G ? G : 0) + sum_s P[s] (fixed order), written back to G; Frobenius norm ----
   const size_t mat_off = (size_t)blockIdx.x * H * HD;
   float* X = G + mat_off;
   const int n4 = H * HD / 4;
+  constexpr int LB = 4;                            // float4 loads in flight per thread and set
   float acc = 0.f;
-  for (int e = tid; e < n4; e += THREADS) {
-    float4 g = use_G ? reinterpret_cast<const float4*>(X)[e] : make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int s = 0; s < n_sets; ++s) {
-      const float4 p = reinterpret_cast<const float4*>(P + (size_t)s * set_elems + mat_off)[e];
-      g.x += p.x; g.y += p.y; g.z += p.z; g.w += p.w;
+  for (int e0 = tid; e0 < n4; e0 += THREADS * LB) {
+    float4 g[LB];
+#pragma unroll
+    for (int u = 0; u < LB; ++u) {
+      const int e = e0 + u * THREADS;
+      g[u] = (use_G && e < n4) ? reinterpret_cast<const float4*>(X)[e] : make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    reinterpret_cast<float4*>(X)[e] = g;
-    acc = fmaf(g.x, g.x, acc); acc = fmaf(g.y, g.y, acc);
-    acc = fmaf(g.z, g.z, acc); acc = fmaf(g.w, g.w, acc);
+    for (int s0 = 0; s0 < n_sets; s0 += 4) {       // 4 sets x LB loads in flight, summed in set order
+      float4 p[4][LB];
+#pragma unroll
+      for (int ds = 0; ds < 4; ++ds) {
+        const float4* ps = reinterpret_cast<const float4*>(P + (size_t)(s0 + ds) * set_elems + mat_off);
+#pragma unroll
+        for (int u = 0; u < LB; ++u) {
+          const int e = e0 + u * THREADS;
+          p[ds][u] = (s0 + ds < n_sets && e < n4) ? __ldcg(ps + e) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+      }
+#pragma unroll
+      for (int ds = 0; ds < 4; ++ds)
+#pragma unroll
+        for (int u = 0; u < LB; ++u) {
+          g[u].x += p[ds][u].x; g[u].y += p[ds][u].y; g[u].z += p[ds][u].z; g[u].w += p[ds][u].w;
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < LB; ++u) {
+      const int e = e0 + u * THREADS;
+      if (e < n4) {
+        reinterpret_cast<float4*>(X)[e] = g[u];
+        acc = fmaf(g[u].x, g[u].x, acc); acc = fmaf(g[u].y, g[u].y, acc);
+        acc = fmaf(g[u].z, g[u].z, acc); acc = fmaf(g[u].w, g[u].w, acc);
+      }
+    }
   }
+  NS_TR(60);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
   if (lane == 0) red[warp] = acc;
@@ -122,53 +156,80 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
   }
   __syncthreads();
   const float scale = s_scale;
-  for (int e = tid; e < n4; e += THREADS) {      // same thread re-reads what it wrote
-    const float4 g = reinterpret_cast<const float4*>(X)[e];
-    const float v[4] = {g.x * scale, g.y * scale, g.z * scale, g.w * scale};
-    uint2 hi, lo;
-    split4(v, hi, lo);
-    const int row = e >> 4, c = (e & 15) * 4;    // 16 float4 per 64-wide row
-    const uint32_t off = row * 128 + (((c >> 3) ^ (row & 7)) * 16) + (c & 7) * 2;
-    *reinterpret_cast<uint2*>(XH + off) = hi;
-    *reinterpret_cast<uint2*>(XL + off) = lo;
+  NS_TR(61);
+  for (int e0 = tid; e0 < n4; e0 += THREADS * LB) {   // same thread re-reads what it wrote
+    float4 g[LB];
+#pragma unroll
+    for (int u = 0; u < LB; ++u) {
+      const int e = e0 + u * THREADS;
+      g[u] = e < n4 ? reinterpret_cast<const float4*>(X)[e] : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+#pragma unroll
+    for (int u = 0; u < LB; ++u) {
+      const int e = e0 + u * THREADS;
+      if (e < n4) {
+        const float v0 = g[u].x * scale, v1 = g[u].y * scale, v2 = g[u].z * scale, v3 = g[u].w * scale;
+        uint2 hi, lo;
+        hi.x = pack_bf16x2(v0, v1);
+        hi.y = pack_bf16x2(v2, v3);
+        lo.x = pack_bf16x2(v0 - __uint_as_float(hi.x << 16), v1 - __uint_as_float(hi.x & 0xffff0000u));
+        lo.y = pack_bf16x2(v2 - __uint_as_float(hi.y << 16), v3 - __uint_as_float(hi.y & 0xffff0000u));
+        const int row = e >> 4, c = (e & 15) * 4;    // 16 float4 per 64-wide row
+        const uint32_t off = sw128_off(row, c >> 3) + (c & 7) * 2;
+        *reinterpret_cast<uint2*>(XH + off) = hi;
+        *reinterpret_cast<uint2*>(XL + off) = lo;
+      }
+    }
   }
   fence_proxy_async_smem();
   __syncthreads();
+  NS_TR(1);
 
-  constexpr uint32_t idesc_gram = umma_idesc_bf16(128, 64, 1, 1);   // A, B MN-major
-  constexpr uint32_t idesc_kk = umma_idesc_bf16(128, 64, 0, 0);     // A, B K-major
-  const uint32_t xh = smem_u32(XH), xl = smem_u32(XL), ah = smem_u32(AH), al = smem_u32(AL),
-                 ph = smem_u32(PH), pl = smem_u32(PL);
-  const int q = warp & 3, ch = warp >> 2;                     // TMEM lane quarter, column half
+  constexpr uint32_t idesc_gram = umma_idesc_bf16(128, 128, 1, 1);  // A, B MN-major, hi | lo atoms
+  constexpr uint32_t idesc_k128 = umma_idesc_bf16(128, 128, 0, 0);  // A, B K-major, 128 rows each
+  constexpr uint32_t idesc_k64 = umma_idesc_bf16(128, 64, 0, 0);
+  // shared-memory matrix descriptors; an address step of b bytes is +(b >> 4) on the descriptor
+  const uint64_t d_x_mn = umma_smem_desc_sw128(smem_u32(XH), x_bytes, 1024);    // MN-major, 2nd atom = XL
+  const uint64_t d_xh_k = umma_smem_desc_sw128(smem_u32(XH), 16, 1024);         // K-major
+  const uint64_t d_xl_k = umma_smem_desc_sw128(smem_u32(XL), 16, 1024);
+  const uint64_t d_a = umma_smem_desc_sw128(smem_u32(AH), 16, 1024);            // 128 rows: AH then AL
+  const uint64_t d_p = umma_smem_desc_sw128(smem_u32(PH), 16, 1024);            // 128 rows: PH then PL
+  const int q = warp & 3, cs = warp >> 2;                     // TMEM lane quarter, 16-column group
   const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
-  const int c0 = 32 * ch;
+  const int trow = q * 32 + lane;                             // accumulator row this thread reads
+  const int frow = tid & 63, fch = tid >> 6;                  // fold mapping: row, 8-column chunk
   const int nblk = H / 128;
   const float ca = 3.4445f, cb = -4.7750f, cc = 2.0315f;
   uint32_t phase = 0;
-  float Areg[32];
+  float Areg[8];
 
-  // top (rows 0-63) + bottom (rows 64-127) of a [128 x 64] accumulator; result valid for q < 2
-  auto fold_halves = [&](uint32_t col, float (&out)[32]) {
-    uint32_t r[32];
-    tmem_ld_x32(tb + lane_base + col + c0, r);
+  // sum of the four 64 x 64 blocks of a [128 x 128] accumulator -> 8 values (frow, 8 fch + j)
+  auto fold_blocks = [&](uint32_t col, float (&out)[8]) {
+    uint32_t r0[16], r1[16];
+    NS_TR(52);
+    tmem_ld_x16(tb + lane_base + col + 16 * cs, r0);
+    tmem_ld_x16(tb + lane_base + col + 64 + 16 * cs, r1);
     tc_wait_ld();
-    if (q >= 2) {
-      float* dst = S + ((q - 2) * 32 + lane) * S_LD + c0;
+    NS_TR(53);
+    float* dst = S + trow * S_LD + 16 * cs;
 #pragma unroll
-      for (int j = 0; j < 32; ++j) dst[j] = __uint_as_float(r[j]);
-    }
+    for (int j = 0; j < 16; ++j) dst[j] = __uint_as_float(r0[j]) + __uint_as_float(r1[j]);
+    NS_TR(54);
     __syncthreads();
-    if (q < 2) {
-      const float* src = S + (q * 32 + lane) * S_LD + c0;
+    NS_TR(55);
+    const float* top = S + frow * S_LD + 8 * fch;
+    const float* bot = top + 64 * S_LD;
 #pragma unroll
-      for (int j = 0; j < 32; ++j) out[j] = __uint_as_float(r[j]) + src[j];
-    }
+    for (int j = 0; j < 8; ++j) out[j] = top[j] + bot[j];
   };
   auto end_phase = [&]() {
+    NS_TR(56);
     fence_proxy_async_smem();
+    NS_TR(57);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
+    NS_TR(58);
   };
   auto wait_mma = [&]() {
     mbar_wait(&mma_bar, phase & 1);
@@ -178,81 +239,134 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
 
   for (int it = 0; it < iters; ++it) {
     // ---------------- A = X^T X ----------------
-    if (tid == 0) {
-      for (int ks = 0; ks < H / 16; ++ks) {
-        const uint64_t a = umma_smem_desc_sw128(xh + 2048 * ks, x_bytes, 1024);
-        umma_ss(tb + C_A, a, umma_smem_desc_sw128(xh + 2048 * ks, x_bytes, 1024), idesc_gram, ks > 0);
-        umma_ss(tb + C_A, a, umma_smem_desc_sw128(xl + 2048 * ks, x_bytes, 1024), idesc_gram, 1);
+    if (warp == 0) {
+      if (elect_one()) {
+        uint64_t d = d_x_mn;                                // +2048 B per 16-row K step
+        for (int ks = 0; ks < H / 16; ++ks, d += 128) umma_ss(tb + C_A, d, d, idesc_gram, ks > 0);
+        tc_commit(&mma_bar);
       }
-      tc_commit(&mma_bar);
+      __syncwarp();
     }
+    NS_TR(2 + it * 8);
     wait_mma();
-    fold_halves(C_A, Areg);
-    if (q < 2) store_row32_split(AH, AL, q * 32 + lane, c0, Areg);
-    end_phase();
-    // ---------------- Pm = a I + b A + c A A ----------------
-    if (tid == 0) {
-#pragma unroll
-      for (int k = 0; k < HD / 16; ++k) {
-        const uint64_t a = umma_smem_desc_sw128(ah + 32 * k, 16, 1024);   // 128 rows: AH then AL
-        umma_ss(tb + C_A2, a, umma_smem_desc_sw128(ah + 32 * k, 16, 1024), idesc_kk, k > 0);
-        umma_ss(tb + C_A2, a, umma_smem_desc_sw128(al + 32 * k, 16, 1024), idesc_kk, 1);
-      }
-      tc_commit(&mma_bar);
-    }
-    wait_mma();
+    NS_TR(3 + it * 8);
+    fold_blocks(C_A, Areg);
     {
-      float A2[32];
-      fold_halves(C_A2, A2);
-      if (q < 2) {
-        const int row = q * 32 + lane;
-#pragma unroll
-        for (int j = 0; j < 32; ++j) {
-          float p = fmaf(cc, A2[j], cb * Areg[j]);
-          if (c0 + j == row) p += ca;
-          A2[j] = p;
-        }
-        store_row32_split(PH, PL, row, c0, A2);
-      }
+      uint4 hi, lo;
+      split8(Areg, hi, lo);
+      *reinterpret_cast<uint4*>(AH + sw128_off(frow, fch)) = hi;
+      *reinterpret_cast<uint4*>(AL + sw128_off(frow, fch)) = lo;
     }
     end_phase();
-    // ---------------- X <- X Pm ----------------
-    if (tid == 0) {
-      for (int mb = 0; mb < nblk; ++mb) {
-        const uint32_t d = tb + C_X + 64 * mb;
-        const uint32_t xhb = xh + mb * (128 * 128), xlb = xl + mb * (128 * 128);
+    NS_TR(4 + it * 8);
+    // ---------------- Pm = a I + b A + c A A ----------------
+    if (warp == 0) {
+      if (elect_one()) {
 #pragma unroll
-        for (int k = 0; k < HD / 16; ++k) {
-          const uint64_t a_hi = umma_smem_desc_sw128(xhb + 32 * k, 16, 1024);
-          const uint64_t b_hi = umma_smem_desc_sw128(ph + 32 * k, 16, 1024);
-          umma_ss(d, a_hi, b_hi, idesc_kk, k > 0);
-          umma_ss(d, a_hi, umma_smem_desc_sw128(pl + 32 * k, 16, 1024), idesc_kk, 1);
-          umma_ss(d, umma_smem_desc_sw128(xlb + 32 * k, 16, 1024), b_hi, idesc_kk, 1);
-        }
+        for (int k = 0; k < HD / 16; ++k)                   // +32 B per 16-column K step
+          umma_ss(tb + C_A2, d_a + 2 * k, d_a + 2 * k, idesc_k128, k > 0);
+        tc_commit(&mma_bar);
       }
-      tc_commit(&mma_bar);
+      __syncwarp();
     }
     wait_mma();
+    NS_TR(5 + it * 8);
+    {
+      float pm[8];
+      fold_blocks(C_A2, pm);
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        float p = fmaf(cc, pm[j], cb * Areg[j]);
+        if (8 * fch + j == frow) p += ca;
+        pm[j] = p;
+      }
+      uint4 hi, lo;
+      split8(pm, hi, lo);
+      *reinterpret_cast<uint4*>(PH + sw128_off(frow, fch)) = hi;
+      *reinterpret_cast<uint4*>(PL + sw128_off(frow, fch)) = lo;
+    }
+    end_phase();
+    NS_TR(6 + it * 8);
+    // ---------------- X <- X Pm ----------------
+    if (warp == 0) {
+      if (elect_one()) {
+        for (int mb = 0; mb < nblk; ++mb) {
+          const uint32_t d = tb + C_X + 128 * mb;
+          const uint64_t a_h = d_xh_k + mb * 1024, a_l = d_xl_k + mb * 1024;   // 16 KB per 128-row block
+#pragma unroll
+          for (int k = 0; k < HD / 16; ++k) {
+            umma_ss(d, a_h + 2 * k, d_p + 2 * k, idesc_k128, k > 0);   // [XH PH^T | XH PL^T]
+            umma_ss(d, a_l + 2 * k, d_p + 2 * k, idesc_k64, 1);        // left half += XL PH^T
+          }
+        }
+        tc_commit(&mma_bar);
+      }
+      __syncwarp();
+    }
+    NS_TR(7 + it * 8);
+    wait_mma();
+    NS_TR(8 + it * 8);
+    const bool last = it == iters - 1;
+    float* stage = reinterpret_cast<float*>(smem);            // last iteration: fp32 [H][W_LD]
     for (int mb = 0; mb < nblk; ++mb) {
-      uint32_t r[32];
-      tmem_ld_x32(tb + lane_base + C_X + 64 * mb + c0, r);
+      uint32_t r0[16], r1[16];
+      tmem_ld_x16(tb + lane_base + C_X + 128 * mb + 16 * cs, r0);
+      tmem_ld_x16(tb + lane_base + C_X + 128 * mb + 64 + 16 * cs, r1);
       tc_wait_ld();
-      const int row = mb * 128 + q * 32 + lane;
-      if (it == iters - 1) {
-        float4* dst = reinterpret_cast<float4*>(X + (size_t)row * HD + c0);
+      const int row = mb * 128 + trow;
+      float f[16];
 #pragma unroll
-        for (int v = 0; v < 8; ++v)
-          dst[v] = make_float4(__uint_as_float(r[4 * v]), __uint_as_float(r[4 * v + 1]),
-                               __uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3]));
+      for (int j = 0; j < 16; ++j) f[j] = __uint_as_float(r0[j]) + __uint_as_float(r1[j]);
+      if (!last) {
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          const float v[8] = {f[8 * k], f[8 * k + 1], f[8 * k + 2], f[8 * k + 3],
+                              f[8 * k + 4], f[8 * k + 5], f[8 * k + 6], f[8 * k + 7]};
+          uint4 hi, lo;
+          split8(v, hi, lo);
+          *reinterpret_cast<uint4*>(XH + sw128_off(row, 2 * cs + k)) = hi;
+          *reinterpret_cast<uint4*>(XL + sw128_off(row, 2 * cs + k)) = lo;
+        }
       } else {
-        float f[32];
+        // all MMAs that read the operand tiles have completed: reuse them as the fp32 staging
+        float4* dst = reinterpret_cast<float4*>(stage + (size_t)row * W_LD + 16 * cs);
 #pragma unroll
-        for (int j = 0; j < 32; ++j) f[j] = __uint_as_float(r[j]);
-        store_row32_split(XH, XL, row, c0, f);
+        for (int v = 0; v < 4; ++v) dst[v] = make_float4(f[4 * v], f[4 * v + 1], f[4 * v + 2], f[4 * v + 3]);
       }
     }
     end_phase();
+    NS_TR(9 + it * 8);
   }
+  // ---- coalesced write-out: fused commit W <- W - NS(g) (Eq. 8) or NS(g) -> G ----
+  {
+    const float* stage = reinterpret_cast<const float*>(smem);
+    constexpr int WB = 4;
+    for (int e0 = tid; e0 < n4; e0 += THREADS * WB) {
+      float4 w[WB];
+#pragma unroll
+      for (int u = 0; u < WB; ++u) {
+        const int e = e0 + u * THREADS;
+        w[u] = (Wm != nullptr && e < n4) ? reinterpret_cast<const float4*>(Wm + mat_off)[e]
+                                         : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int u = 0; u < WB; ++u) {
+        const int e = e0 + u * THREADS;
+        if (e >= n4) continue;
+        const int row = e >> 4, c = (e & 15) * 4;
+        const float4 x = *reinterpret_cast<const float4*>(stage + (size_t)row * W_LD + c);
+        if (Wm != nullptr) {
+          w[u].x -= x.x; w[u].y -= x.y; w[u].z -= x.z; w[u].w -= x.w;
+          reinterpret_cast<float4*>(Wm + mat_off)[e] = w[u];
+          reinterpret_cast<uint2*>(Wb + mat_off)[e] =
+              make_uint2(pack_bf16x2(w[u].x, w[u].y), pack_bf16x2(w[u].z, w[u].w));
+        } else {
+          reinterpret_cast<float4*>(X)[e] = x;
+        }
+      }
+    }
+  }
+  NS_TR(50);
   if (warp == 0) tmem_dealloc(tb, tmem_cols);
 }
 
@@ -261,24 +375,29 @@ int ns_tc_supported(const ttt_config* cfg) {
          cfg->hidden >= 128 && cfg->hidden <= 512 && !cfg->linear_fast_weight;
 }
 
-// In-place NS of all 3*nh matrices of the pending gradient; folds the partial sets into G first.
-int launch_ns_tc(ttt_ctx* ctx, cudaStream_t s) {
+// NS of all 3*nh matrices of the pending gradient (the partial sets are folded in first).
+// fuse_commit: also apply W <- W - NS(g) (fp32 master + bf16 copy) and clear the pending set;
+// otherwise NS(g) is left in G (G_valid) for the commit kernel.
+int launch_ns_tc(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
-  const size_t smem = (size_t)2 * c.hidden * 128 + 4 * 8192 + 64 * nstc::S_LD * sizeof(float) + 1024;
+  size_t smem = (size_t)2 * c.hidden * 128 + 4 * 8192 + 128 * nstc::S_LD * sizeof(float);
+  const size_t stage = (size_t)c.hidden * nstc::W_LD * sizeof(float);
+  if (stage > smem) smem = stage;
+  smem += 1024;
   static size_t attr_smem = 0;
   if (smem > attr_smem) {
     TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ns_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            (int)smem), "ns_tc_kernel smem attr");
     attr_smem = smem;
   }
-  uint32_t cols = 128 + 64 * (c.hidden / 128);
-  uint32_t alloc = 32;
-  while (alloc < cols) alloc <<= 1;
+  const uint32_t alloc = c.hidden <= 256 ? 256 : 512;
   ns_tc_kernel<<<3 * c.nh, nstc::THREADS, smem, s>>>(ctx->G, ctx->partials, ctx->n_partials,
                                                      3 * ctx->mat_elems, ctx->G_valid ? 1 : 0,
-                                                     c.hidden, c.ns_iters, alloc);
+                                                     c.hidden, c.ns_iters, alloc,
+                                                     fuse_commit ? ctx->Wm : nullptr,
+                                                     fuse_commit ? ctx->Wb : nullptr);
   TTT_LAUNCH_CHECK(ctx, "ns_tc_kernel");
-  ctx->G_valid = true;
+  ctx->G_valid = !fuse_commit;
   ctx->n_partials = 0;
   return TTT_OK;
 }

@@ -406,8 +406,9 @@ int launch_loss_reduce(ttt_ctx* ctx, int n, float* loss, cudaStream_t s) {
 int launch_commit(ttt_ctx* ctx, cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
   if (c.ns_iters > 0 && ns_tc_supported(&c)) {
-    int rc = launch_ns_tc(ctx, s);      // tensor-core NS; folds the partial sets into G itself
-    if (rc != TTT_OK) return rc;
+    // tensor-core NS; folds the partial sets itself and, without renorm, commits W <- W - NS(g)
+    int rc = launch_ns_tc(ctx, c.renorm == 0, s);
+    if (rc != TTT_OK || c.renorm == 0) return rc;
   } else if (c.ns_iters > 0) {
     int rc = launch_reduce_pending(ctx, s);
     if (rc != TTT_OK) return rc;

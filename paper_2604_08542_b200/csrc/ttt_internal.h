@@ -61,8 +61,9 @@ int launch_loss_reduce(ttt_ctx* ctx, int n, float* loss, cudaStream_t s);
 
 // --- tensor-core Newton-Schulz (ns_tc.cu) ---------------------------------------------------------
 int ns_tc_supported(const ttt_config* cfg);
-// G = NS((G_valid ? G : 0) + sum partials) for all 3*nh matrices; marks G_valid, clears n_partials
-int launch_ns_tc(ttt_ctx* ctx, cudaStream_t s);
+// NS((G_valid ? G : 0) + sum partials) for all 3*nh matrices; fuse_commit: W <- W - NS(.) and the
+// pending set is cleared, else the result is left in G (G_valid)
+int launch_ns_tc(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s);
 
 // --- f32 path (f32_path.cu) ---------------------------------------------------------------------
 // appends partial-gradient sets [n_partials, n_partials + used); writes loss_part rows [0, loss_rows)
