@@ -3,21 +3,34 @@
 //
 // Formulation ("hidden on lanes"): one CTA owns 128 hidden units of one head and a range of tokens.
 // Everything is computed TRANSPOSED so that each MMA has M = 128 hidden units on the TMEM lanes:
-//   forward   A^T  = W1^T K^T,  B^T = W3^T K^T,  g^T = W2 V^T      [128 x T]  (contract over hd)
-//   epilogue  s = sigmoid(A); S = A s; Hd = S B; dHd = -eta g
-//             dA = dHd B (s + S (1 - s)); dB = dHd S; Hd' = -eta Hd            (fp32 -> bf16)
-//   gradient  G1^T += dA^T K,  G3^T += dB^T K,  G2 += Hd'^T V      [128 x hd] (contract over tokens)
-// The A operand of every MMA lives in TMEM (weights: loaded once; dA/dB/Hd': written by the
-// epilogue over their own fp32 sources), the B operand is the K or V token tile that TMA put in
-// shared memory with the 128-byte swizzle; the SAME tile serves the forward MMA as a K-major
-// operand and the gradient MMA as an MN-major operand. Gradient accumulators stay in TMEM for the
-// CTA's whole token range; one fp32 partial per CTA goes to HBM/L2 and is summed in a fixed order
-// by the commit kernel (deterministic, no float atomics).
+//   forward   x^T  = (W1/2)^T K^T,  b^T = W3^T K^T,  g0^T = W2 V^T   [128 x T]  (contract over hd)
+//             g = -eta g0 = dHd (dot-product loss: dL/df = -eta v, Eq. 9)
+//   epilogue  th = tanh(x);  S = x + x th = SiLU(a);  t = (1 + th) + S (1 - th) = 2 SiLU'(a)
+//             dA2 = g b t (= 2 dA);  dB = g S;  Hd' = -eta S b                 (fp32 -> bf16)
+//   gradient  2 G1^T += dA2^T K,  G3^T += dB^T K,  G2 += Hd'^T V     [128 x hd] (contract over tokens)
+// The A operand of every MMA lives in TMEM (weights: loaded once, W1 pre-halved (exact) so the
+// accumulator is the tanh argument; dA2/dB/Hd: written by the epilogue over their own fp32 sources),
+// the B operand is the K or V token tile in shared memory with the 128-byte swizzle; the SAME tile
+// serves the forward MMA as a K-major operand and the gradient MMA as an MN-major operand, so the
+// shared-memory operand traffic is 64 B/clk at tensor peak. Gradient accumulators stay in TMEM for
+// the CTA's whole token range; one fp32 partial per CTA goes to L2 and is summed in a fixed order
+// by the commit (deterministic, no float atomics). The factor 2 of G1 is removed at the flush.
 //
-// Warp roles (384 threads): warp 0 = TMA producer, warp 1 = MMA issuer, warp 2 = learning-rate
-// loader (-eta of each tile into the stage's shared-memory slot), warps 4-7 / 8-11 = two epilogue
-// warpgroups that alternate token tiles (TMEM accumulators are double-buffered). The epilogue math
-// is packed fp32x2 (FFMA2/FMUL2): two tokens of one hidden unit per instruction.
+// Warp roles (640 threads): warp 0 = TMA producer; warp 1 = forward-MMA issuer; warp 2 = learning-
+// rate loader (-eta of a tile into the stage's shared-memory slot, prefetched ahead of the ring; scaling
+// V in shared memory instead costs a serial read-modify-write + proxy fence per tile); warp 3 = gradient-MMA
+// issuer (two issuers: an mbarrier wait costs ~90 clk even when already complete, and MMA issue
+// blocks at the tensor pipe's pace, so one thread cannot keep the pipe fed); warps 4-19 = two
+// epilogue groups of 8 warps that alternate token tiles (2 warps per TMEM lane quarter, one
+// 16-token K step each; packed fp32x2 math, tanh.approx sigmoid).
+// Pipeline (TMEM is the scarce resource: weights 96 + gradient accumulators 192 columns leave 224):
+// the x | b forward accumulators are double-buffered, g is single-buffered and released first, as
+// soon as an epilogue group has pulled it into registers; the bf16 gradient operands have their own
+// (single) columns, so nothing aliases; forward and gradient MMAs are issued by different warps —
+// the MMAs of tiles i+1, i+2 overlap the epilogue math of tile i.
+// Measured budget per 32-token tile and SM (B200 microbenchmarks): MMA 546 clk (12 x
+// N=32 at 25 clk + 6 x N=64 at 41 clk: ~9 clk fixed cost per tcgen05.mma), epilogue math ~390 clk
+// (MUFU 16/clk: 256; FP32 pipe 128 lanes/clk: 8 ops per element; F2FP packs).
 #include <stdio.h>
 
 #include "tc_common.cuh"
@@ -25,16 +38,32 @@
 
 #ifdef TTT_TRACE   // debug builds only: per-tile clock timeline of CTA (0,0,0), staged in smem
 __device__ long long g_ttt_trace[64 * 16];
+__device__ unsigned long long g_ttt_time[4];      // globaltimer ns + clock64 at start / end of CTA (0,0,0)
+extern "C" int ttt_debug_time(unsigned long long* host) {
+  return (int)cudaMemcpyFromSymbol(host, g_ttt_time, sizeof(g_ttt_time));
+}
+__device__ unsigned g_ttt_trace2[32 * 16 * 4];   // [tile][epilogue warp][got, loaded, math, done]
+#define TTT_TR2(i, w, k) do { if ((i) < 32 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && lane == 0) g_ttt_trace2[((i) * 16 + (w)) * 4 + (k)] = (unsigned)clock(); } while (0)
+extern "C" int ttt_debug_trace2(unsigned* host) {
+  return (int)cudaMemcpyFromSymbol(host, g_ttt_trace2, sizeof(g_ttt_trace2));
+}
+#ifdef TTT_TRACE_LIGHT     // only the start/end stamps: no probes inside the loops
+#define TTT_TR(i, k) do { } while (0)
+#undef TTT_TR2
+#define TTT_TR2(i, w, k) do { } while (0)
+#else
 #define TTT_TR(i, k)                                                                  \
   do {                                                                                \
     if ((i) < 64 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0)            \
       tr_s[(i) * 16 + (k)] = (unsigned)clock();                                       \
   } while (0)
+#endif
 extern "C" int ttt_debug_trace(long long* host) {
   return (int)cudaMemcpyFromSymbol(host, g_ttt_trace, sizeof(g_ttt_trace));
 }
 #else
 #define TTT_TR(i, k) do { } while (0)
+#define TTT_TR2(i, w, k) do { } while (0)
 #endif
 
 namespace ttt {
@@ -42,14 +71,18 @@ namespace ttt {
 namespace upd {
 constexpr int HS = 128;        // hidden units per CTA (MMA M)
 constexpr int T = 32;          // tokens per tile (forward MMA N, gradient MMA K)
-constexpr int STAGES = 6;      // K/V shared-memory ring
-constexpr int THREADS = 384;
+constexpr int STAGES = 10;     // K/V shared-memory ring (ring latency = TMA + F -> E -> G hand-offs)
+constexpr int EPI_WARPS = 16;
+constexpr int THREADS = (4 + EPI_WARPS) * 32;
 constexpr int TILE_BYTES = T * 128;  // one [T x 64] bf16 tile
+constexpr int STAGE_BYTES = 2 * TILE_BYTES;
 
 // TMEM column plan for hd = 64 (512 columns x 128 lanes x 32 bit)
 constexpr uint32_t C_W1 = 0, C_W3 = 32, C_W2 = 64;        // bf16 weights as A operands, 32 cols each
 constexpr uint32_t C_G1 = 96, C_G3 = 160, C_G2 = 224;     // fp32 gradient accumulators, 64 cols each
-constexpr uint32_t C_BUF = 288, BUF_STRIDE = 96;          // two forward buffers: A | B | g, 32 cols each
+constexpr uint32_t C_XB = 288, XB_STRIDE = 64;            // two forward buffers x | b (fp32, 32 cols each)
+constexpr uint32_t C_GG = 416;                            // forward accumulator g (fp32, 32 cols), single
+constexpr uint32_t C_H = 448;                             // bf16 operands dA2 | dB | Hd, 16 cols each, single
 }  // namespace upd
 
 template <bool LOSS>
@@ -63,15 +96,20 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) &
                                              ~static_cast<uintptr_t>(1023));
-  __shared__ uint64_t full[STAGES], empty[STAGES], fwd_full[2], epi_done[2], w_ready, grad_done;
+  __shared__ uint64_t full[STAGES], empty[STAGES], fwd_full[2], xb_free[2], g_free,
+      epi_done[2], opnd_free, w_ready, grad_done;
   __shared__ uint32_t tmem_base_s;
-  __shared__ float loss_red[8];
+  __shared__ float loss_red[EPI_WARPS];
   __shared__ __align__(16) float ne_s[STAGES][T];   // -eta of the stage's tokens (0 beyond M)
 #ifdef TTT_TRACE
   __shared__ unsigned tr_s[64 * 16];
   for (int e = threadIdx.x; e < 64 * 16; e += blockDim.x) tr_s[e] = 0;
   __syncthreads();
   if (threadIdx.x == 0) tr_s[15] = (unsigned)clock();
+  if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) {
+    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    g_ttt_time[0] = t; g_ttt_time[1] = clock64();
+  }
 #endif
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -82,8 +120,12 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
 
   if (tid == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 2); mbar_init(&empty[s], 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 8); }
-    mbar_init(&w_ready, 4);
+    mbar_init(&fwd_full[0], 1);
+    mbar_init(&fwd_full[1], 1);
+    mbar_init(&g_free, EPI_WARPS / 2);
+    mbar_init(&opnd_free, 1);
+    for (int b = 0; b < 2; ++b) { mbar_init(&epi_done[b], EPI_WARPS / 2); mbar_init(&xb_free[b], EPI_WARPS / 2); }
+    mbar_init(&w_ready, EPI_WARPS);
     mbar_init(&grad_done, 1);
     fence_mbar_init();
   }
@@ -103,74 +145,92 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         const int s = i % STAGES, it = i / STAGES;
         mbar_wait(&empty[s], (it & 1) ^ 1);
         TTT_TR(i, 12);
-        mbar_arrive_expect_tx(&full[s], 2 * TILE_BYTES);
-        uint8_t* dst = smem + s * 2 * TILE_BYTES;
+        mbar_arrive_expect_tx(&full[s], STAGE_BYTES);
+        uint8_t* dst = smem + s * STAGE_BYTES;
         tma_load_2d(dst, &mapK, &full[s], h * HD, (tile_lo + i) * T);
         tma_load_2d(dst + TILE_BYTES, &mapV, &full[s], h * HD, (tile_lo + i) * T);
       }
     }
   } else if (warp == 1) {
-    // ===================== MMA issuer =====================
-    if (elect_one()) {
-      constexpr uint32_t idesc_f = umma_idesc_bf16(HS, T, 0, 0);    // B = token tile, K-major
-      constexpr uint32_t idesc_g = umma_idesc_bf16(HS, HD, 0, 1);   // B = token tile, MN-major
-      const uint32_t smem_base = smem_u32(smem);
-      mbar_wait(&w_ready, 0);
-      tc_fence_after();
-      auto fwd = [&](int i) {
-        const int s = i % STAGES, it = i / STAGES, b = i & 1;
-        TTT_TR(i, 0);
-        mbar_wait(&full[s], it & 1);
-        tc_fence_after();
-        TTT_TR(i, 1);
-        const uint32_t ks = smem_base + s * 2 * TILE_BYTES, vs = ks + TILE_BYTES;
-        const uint32_t acc = tb + C_BUF + b * BUF_STRIDE;
-#pragma unroll
-        for (int k = 0; k < HD / 16; ++k)
-          umma_ts(acc, tb + C_W1 + 8 * k, umma_smem_desc_sw128(ks + 32 * k, 16, 1024), idesc_f, k > 0);
-#pragma unroll
-        for (int k = 0; k < HD / 16; ++k)
-          umma_ts(acc + 32, tb + C_W3 + 8 * k, umma_smem_desc_sw128(ks + 32 * k, 16, 1024), idesc_f, k > 0);
-#pragma unroll
-        for (int k = 0; k < HD / 16; ++k)
-          umma_ts(acc + 64, tb + C_W2 + 8 * k, umma_smem_desc_sw128(vs + 32 * k, 16, 1024), idesc_f, k > 0);
-        tc_commit(&fwd_full[b]);
-        TTT_TR(i, 2);
-      };
-      auto grad = [&](int i) {
-        const int s = i % STAGES, b = i & 1, n = i >> 1;
-        mbar_wait(&epi_done[b], n & 1);
-        tc_fence_after();
-        TTT_TR(i, 3);
-        const uint32_t ks = smem_base + s * 2 * TILE_BYTES, vs = ks + TILE_BYTES;
-        const uint32_t opnd = tb + C_BUF + b * BUF_STRIDE;   // dA | dB | Hd' alias A | B | g
-#pragma unroll
-        for (int k = 0; k < T / 16; ++k)
-          umma_ts(tb + C_G1, opnd + 24 * k, umma_smem_desc_sw128(ks + 2048 * k, TILE_BYTES, 1024),
-                  idesc_g, (i > 0 || k > 0));
-#pragma unroll
-        for (int k = 0; k < T / 16; ++k)
-          umma_ts(tb + C_G3, opnd + 32 + 24 * k, umma_smem_desc_sw128(ks + 2048 * k, TILE_BYTES, 1024),
-                  idesc_g, (i > 0 || k > 0));
-#pragma unroll
-        for (int k = 0; k < T / 16; ++k)
-          umma_ts(tb + C_G2, opnd + 64 + 24 * k, umma_smem_desc_sw128(vs + 2048 * k, TILE_BYTES, 1024),
-                  idesc_g, (i > 0 || k > 0));
-        tc_commit(&empty[s]);
-        TTT_TR(i, 4);
-      };
-      if (ntiles > 0) fwd(0);
-      for (int i = 0; i < ntiles; ++i) {
-        if (i + 1 < ntiles) fwd(i + 1);
-        grad(i);
+    // ===================== forward-MMA issuer =====================
+    // Descriptors are built once; a step of b bytes in shared memory is +(b >> 4) on a descriptor.
+    constexpr uint32_t idesc_f = umma_idesc_bf16(HS, T, 0, 0);    // B = token tile, K-major
+    const uint64_t dk_f = umma_smem_desc_sw128(smem_u32(smem), 16, 1024);
+    constexpr uint64_t V_OFF = TILE_BYTES >> 4, ST_OFF = STAGE_BYTES >> 4;
+    mbar_wait(&w_ready, 0);
+    tc_fence_after();
+    for (int i = 0; i < ntiles; ++i) {
+      const int s = i % STAGES, it = i / STAGES;
+      TTT_TR(i, 0);
+      const int b = i & 1, n = i >> 1;
+      uint32_t g_ok;
+      // the three waits of a tile are probed together (an mbarrier probe costs ~90 clk even when the
+      // phase is already complete), then re-waited only if a probe failed
+      {
+        const uint32_t ok0 = mbar_try_wait(&full[s], it & 1);
+        const uint32_t ok1 = n > 0 ? mbar_try_wait(&xb_free[b], (n - 1) & 1) : 1u;
+        const uint32_t ok2 = i > 0 ? mbar_try_wait(&g_free, (i - 1) & 1) : 1u;
+        if (!ok0) mbar_wait(&full[s], it & 1);
+        if (!ok1) mbar_wait(&xb_free[b], (n - 1) & 1);
+        g_ok = ok2;
       }
-      tc_commit(&grad_done);
+      tc_fence_after();
+      TTT_TR(i, 1);
+      const uint64_t dk = dk_f + s * ST_OFF, dv = dk + V_OFF;
+      if (elect_one()) {
+        const uint32_t acc = tb + C_XB + b * XB_STRIDE;
+#pragma unroll
+        for (int k = 0; k < HD / 16; ++k) umma_ts(acc, tb + C_W1 + 8 * k, dk + 2 * k, idesc_f, k > 0);
+#pragma unroll
+        for (int k = 0; k < HD / 16; ++k) umma_ts(acc + 32, tb + C_W3 + 8 * k, dk + 2 * k, idesc_f, k > 0);
+      }
+      __syncwarp();
+      if (!g_ok) { mbar_wait(&g_free, (i - 1) & 1); tc_fence_after(); }   // g of tile i-1 is in registers
+      if (elect_one()) {
+#pragma unroll
+        for (int k = 0; k < HD / 16; ++k) umma_ts(tb + C_GG, tb + C_W2 + 8 * k, dv + 2 * k, idesc_f, k > 0);
+        tc_commit(&fwd_full[b]);   // one barrier per epilogue group: a parity wait only tells the
+                                       // current phase from the previous one
+      }
+      __syncwarp();
+      TTT_TR(i, 2);
     }
+  } else if (warp == 3) {
+    // ===================== gradient-MMA issuer =====================
+    constexpr uint32_t idesc_g = umma_idesc_bf16(HS, HD, 0, 1);   // B = token tile, MN-major
+    const uint64_t dk_g = umma_smem_desc_sw128(smem_u32(smem), TILE_BYTES, 1024);
+    constexpr uint64_t V_OFF = TILE_BYTES >> 4, ST_OFF = STAGE_BYTES >> 4;
+    for (int i = 0; i < ntiles; ++i) {
+      const int s = i % STAGES, b = i & 1, n = i >> 1;
+      mbar_wait(&epi_done[b], n & 1);
+      tc_fence_after();
+      TTT_TR(i, 3);
+      if (elect_one()) {
+        const uint64_t dk = dk_g + s * ST_OFF, dv = dk + V_OFF;
+        const uint32_t opnd = tb + C_H;                      // dA2 | dB | Hd, 8 columns per K step
+#ifndef TTT_EXP_NOGRAD
+#pragma unroll
+        for (int k = 0; k < T / 16; ++k)                     // +2048 B per 16-token K step
+          umma_ts(tb + C_G1, opnd + 8 * k, dk + 128 * k, idesc_g, (i > 0 || k > 0));
+#pragma unroll
+        for (int k = 0; k < T / 16; ++k)
+          umma_ts(tb + C_G3, opnd + 16 + 8 * k, dk + 128 * k, idesc_g, (i > 0 || k > 0));
+#pragma unroll
+        for (int k = 0; k < T / 16; ++k)
+          umma_ts(tb + C_G2, opnd + 32 + 8 * k, dv + 128 * k, idesc_g, (i > 0 || k > 0));
+#endif
+        tc_commit(&empty[s]);          // the tile's forward MMAs completed long ago (epilogue read them)
+        tc_commit(&opnd_free);
+      }
+      __syncwarp();
+      TTT_TR(i, 4);
+    }
+    if (elect_one()) tc_commit(&grad_done);
+    __syncwarp();
   } else if (warp == 2) {
     // ===================== learning-rate loader =====================
-    // -eta of tile i (32 tokens = one 128-B line of lr) goes to the stage's shared-memory slot.
-    // The global loads run LRPF tiles ahead of the ring (register double buffer), so their
-    // latency is never on the critical path of a tile.
+    // -eta of tile i (32 tokens = one 128-B line of lr) goes to the stage's shared-memory slot. The
+    // global loads run LRPF tiles ahead of the ring (register double buffer).
     constexpr int LRPF = 8;
     const float* lrh = lr + (size_t)h * M;
     auto ld_batch = [&](int i0, float (&v)[LRPF]) {
@@ -198,33 +258,36 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
 #pragma unroll
       for (int u = 0; u < LRPF; ++u) cur[u] = nxt[u];
     }
-  } else if (warp >= 4) {
-    // ===================== epilogue warpgroups =====================
-    const int wg = (warp - 4) >> 2, q = warp & 3;
-    const int j = q * 32 + lane;                       // hidden unit within the slice = TMEM lane
+  } else {
+    // ===================== epilogue warps =====================
+    const int ew = warp - 4, q = warp & 3;
+    const int grp = ew >> 3, kh = (ew >> 2) & 1;           // tile parity this warp serves, K step (16 tokens)
+    const int tc = ew >> 2;                                // 16-column group for the weight load / flush
+    const int j = q * 32 + lane;                           // hidden unit within the slice = TMEM lane
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
     const size_t me = (size_t)nh * H * HD;
     const size_t row = ((size_t)h * H + (size_t)slice * HS + j) * HD;
-    if (wg == 0) {
-      // weights -> TMEM as A operands: row j of W1^T, W3^T, W2 (64 bf16 = 32 words each);
-      // all 24 loads are issued before the first TMEM store
+    {
+      // weights -> TMEM as A operands: row j of W1^T / 2, W3^T, W2 (64 bf16 = 32 words each); warp
+      // group tc loads 16-byte chunks 2 tc, 2 tc + 1 of each row (8 words = columns 8 tc .. 8 tc + 7)
       const uint32_t cols[3] = {C_W1, C_W2, C_W3};
-      uint4 x[3][8];
+      uint4 x[3][2];
 #pragma unroll
       for (int mat = 0; mat < 3; ++mat) {
-        const uint4* src = reinterpret_cast<const uint4*>(Wb + mat * me + row);
-#pragma unroll
-        for (int v = 0; v < 8; ++v) x[mat][v] = __ldg(src + v);
+        const uint4* src = reinterpret_cast<const uint4*>(Wb + mat * me + row) + 2 * tc;
+        x[mat][0] = __ldg(src);
+        x[mat][1] = __ldg(src + 1);
       }
 #pragma unroll
       for (int mat = 0; mat < 3; ++mat) {
-        uint32_t r[32];
+        uint32_t r[8] = {x[mat][0].x, x[mat][0].y, x[mat][0].z, x[mat][0].w,
+                         x[mat][1].x, x[mat][1].y, x[mat][1].z, x[mat][1].w};
+        if (mat == 0) {
 #pragma unroll
-        for (int v = 0; v < 8; ++v) {
-          r[4 * v] = x[mat][v].x; r[4 * v + 1] = x[mat][v].y;
-          r[4 * v + 2] = x[mat][v].z; r[4 * v + 3] = x[mat][v].w;
+          for (int e = 0; e < 8; ++e)      // W1 / 2: the accumulator becomes the tanh argument a / 2
+            r[e] = pack_bf16x2(0.5f * __uint_as_float(r[e] << 16), 0.5f * __uint_as_float(r[e] & 0xffff0000u));
         }
-        tmem_st_x32(tb + lane_base + cols[mat], r);
+        tmem_st_x8(tb + lane_base + cols[mat] + 8 * tc, r);
       }
       tc_wait_st();
       tc_fence_before();
@@ -232,93 +295,120 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       if (lane == 0) mbar_arrive(&w_ready);
     }
     uint64_t loss2 = 0ull;
-    const uint64_t HALF2 = pack2(0.5f, 0.5f), NHALF2 = pack2(-0.5f, -0.5f);
-    for (int i = 0; i < ntiles; ++i) {
-      // both warpgroups work on every tile: warpgroup `wg` owns token columns [16 wg, 16 wg + 16)
-      const int b = i & 1, n = i >> 1, s = i % STAGES;
-      const uint32_t buf = tb + lane_base + C_BUF + b * BUF_STRIDE;
-      if (q == 0 && lane == 0) TTT_TR(i, 5 + wg);
-      mbar_wait(&fwd_full[b], n & 1);
-      mbar_wait(&full[s], (i / STAGES) & 1);     // direct acquire of the loader's -eta slot
+    const uint64_t ONE2 = pack2(1.0f, 1.0f), NONE2 = pack2(-1.0f, -1.0f);
+    const uint32_t xbuf = tb + lane_base + C_XB + grp * XB_STRIDE + 16 * kh;
+    const uint32_t gbuf = tb + lane_base + C_GG + 16 * kh;
+    const uint32_t hbuf = tb + lane_base + C_H + 8 * kh;
+    for (int i = grp; i < ntiles; i += 2) {
+      const int n = i >> 1;
+      if (ew == 0 && lane == 0) TTT_TR(i, 5);
+      mbar_wait(&fwd_full[grp], n & 1);
+      mbar_wait(&full[i % STAGES], (i / STAGES) & 1);      // direct acquire of the loader's -eta slot
       tc_fence_after();
-      if (q == 0 && lane == 0) TTT_TR(i, 7 + wg);
-      const uint2* nes = reinterpret_cast<const uint2*>(&ne_s[s][0]);
-      uint32_t ra[16], rb[16], rg[16];
-      tmem_ld_x16(buf + 16 * wg, ra);
-      tmem_ld_x16(buf + 32 + 16 * wg, rb);
-      tmem_ld_x16(buf + 64 + 16 * wg, rg);
+      const uint2* nes = reinterpret_cast<const uint2*>(&ne_s[i % STAGES][16 * kh]);
+      if (ew == 0 && lane == 0) TTT_TR(i, 7);
+      TTT_TR2(i, ew, 0);
+      uint32_t rx[16], rb[16], rg[16];
+#ifdef TTT_EXP_NOTMEM
+      for (int c = 0; c < 16; ++c) { rg[c] = 0x3c000000u + c; rx[c] = 0x3c000000u + i; rb[c] = 0x3d000000u + c; }
+#else
+      tmem_ld_x16(gbuf, rg);                               // g is single-buffered: release it first
+#endif
       tc_wait_ld();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&g_free);
+#ifndef TTT_EXP_NOTMEM
+      tmem_ld_x16(xbuf, rx);
+      tmem_ld_x16(xbuf + 32, rb);
+#endif
+      tc_wait_ld();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&xb_free[grp]);           // forward MMAs of tile i+2 may overwrite x | b
+      if (ew == 0 && lane == 0) TTT_TR(i, 6);
+      TTT_TR2(i, ew, 1);
       uint32_t pa[8], pb[8], ph[8];
 #pragma unroll
       for (int c = 0; c < 16; c += 2) {
-        const uint64_t a = pack2u(ra[c], ra[c + 1]);
+        const uint64_t x = pack2u(rx[c], rx[c + 1]);
         const uint64_t bb = pack2u(rb[c], rb[c + 1]);
-        const uint64_t g = pack2u(rg[c], rg[c + 1]);
-        const uint2 nev = nes[8 * wg + (c >> 1)];
+        const uint2 nev = nes[c >> 1];
         const uint64_t ne = pack2u(nev.x, nev.y);
-        // sigmoid(a) = 0.5 tanh(a/2) + 0.5 on the MUFU; 1 - sigmoid = 0.5 - 0.5 tanh(a/2)
+        const uint64_t g = fmul2(ne, pack2u(rg[c], rg[c + 1]));   // dHd = (-eta v) W2^T
         float x0, x1;
-        unpack2(fmul2(a, HALF2), x0, x1);
+        unpack2(x, x0, x1);
+#ifdef TTT_EXP_NOMATH
+        const uint64_t th = x;
+#else
         const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
-        const uint64_t sg = ffma2(th, HALF2, HALF2);
-        const uint64_t om = ffma2(th, NHALF2, HALF2);
-        const uint64_t S = fmul2(a, sg);                 // SiLU(a)
-        const uint64_t t2 = ffma2(S, om, sg);            // SiLU'(a) = s + S (1 - s)
-        const uint64_t hdv = fmul2(S, bb);               // hidden activation Hd
-        const uint64_t dhd = fmul2(ne, g);               // dHd = (-eta v) W2^T
-        pa[c >> 1] = pack_bf16x2_from2(fmul2(fmul2(dhd, bb), t2));   // dA
-        pb[c >> 1] = pack_bf16x2_from2(fmul2(dhd, S));               // dB
-        ph[c >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));              // Hd' = -eta Hd
-        if (LOSS) loss2 = ffma2(hdv, dhd, loss2);
+#endif
+        const uint64_t S = ffma2(x, th, x);                  // SiLU(a) = a sigmoid(a), a = 2 x
+        const uint64_t p = fadd2(th, ONE2);                  // 2 sigmoid(a)
+        const uint64_t m = ffma2(th, NONE2, ONE2);           // 2 (1 - sigmoid(a))
+        const uint64_t t2 = ffma2(S, m, p);                  // 2 SiLU'(a)
+        const uint64_t hdv = fmul2(S, bb);                   // hidden activation Hd
+        pa[c >> 1] = pack_bf16x2_from2(fmul2(fmul2(g, bb), t2));   // 2 dA
+        pb[c >> 1] = pack_bf16x2_from2(fmul2(g, S));               // dB
+        ph[c >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));            // Hd' = -eta Hd
+        if (LOSS) loss2 = ffma2(hdv, g, loss2);
       }
-      // bf16 operands overwrite fp32 columns this warp itself has just read: tokens [16 wg, +16)
-      // of dA / dB / Hd' go to columns [24 wg, 24 wg + 8) of the A / B / g regions
-      tmem_st_x8(buf + 24 * wg, pa);
-      tmem_st_x8(buf + 32 + 24 * wg, pb);
-      tmem_st_x8(buf + 64 + 24 * wg, ph);
+      if (ew == 0 && lane == 0) TTT_TR(i, 8);
+      TTT_TR2(i, ew, 2);
+      // the operand buffer was last read by the gradient MMAs of tile i - 1
+      if (i > 0) { mbar_wait(&opnd_free, (i - 1) & 1); tc_fence_after(); }
+      if (ew == 0 && lane == 0) TTT_TR(i, 10);
+#ifdef TTT_EXP_NOTMEM
+      if (pa[0] + pb[1] + ph[2] == 0x12345u) tmem_st_x8(hbuf, pa);
+#else
+      tmem_st_x8(hbuf, pa);
+      tmem_st_x8(hbuf + 16, pb);
+      tmem_st_x8(hbuf + 32, ph);
+#endif
       tc_wait_st();
+      if (ew == 0 && lane == 0) TTT_TR(i, 11);
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&epi_done[b]);
-      if (q == 0 && lane == 0) TTT_TR(i, 9 + wg);
+      if (lane == 0) mbar_arrive(&epi_done[grp]);
+      if (ew == 0 && lane == 0) TTT_TR(i, 9);
+      TTT_TR2(i, ew, 3);
     }
     // ---- flush the gradient accumulators: one fp32 partial slice per CTA ----
-    if (warp == 4 && lane == 0) TTT_TR(2, 13);
+    if (ew == 0 && lane == 0) TTT_TR(2, 13);
     mbar_wait(&grad_done, 0);
     tc_fence_after();
-    if (warp == 4 && lane == 0) TTT_TR(2, 14);
+    if (ew == 0 && lane == 0) TTT_TR(3, 13);
     float* Pset = P + (size_t)split * 3 * me;
-    auto flush = [&](uint32_t col, int mat, int c0, int ncols) {
-      float4* dst = reinterpret_cast<float4*>(Pset + mat * me + row + c0);
-      for (int c = 0; c < ncols; c += 16) {
-        uint32_t r[16];
-        if (ntiles > 0) {
-          tmem_ld_x16(tb + lane_base + col + c0 + c, r);
-          tc_wait_ld();
-        } else {
+    const uint32_t gcol[3] = {C_G1, C_G2, C_G3};
 #pragma unroll
-          for (int u = 0; u < 16; ++u) r[u] = 0u;
-        }
+    for (int mat = 0; mat < 3; ++mat) {                    // this warp: columns 16 tc .. 16 tc + 15
+      uint32_t r[16];
+      if (ntiles > 0) {
+        tmem_ld_x16(tb + lane_base + gcol[mat] + 16 * tc, r);
+        tc_wait_ld();
+      } else {
 #pragma unroll
-        for (int v = 0; v < 4; ++v)
-          dst[(c >> 2) + v] = make_float4(__uint_as_float(r[4 * v]), __uint_as_float(r[4 * v + 1]),
-                                          __uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3]));
+        for (int u = 0; u < 16; ++u) r[u] = 0u;
       }
-    };
-    if (wg == 0) { flush(C_G1, 0, 0, 64); flush(C_G2, 1, 0, 32); }
-    else         { flush(C_G3, 2, 0, 64); flush(C_G2, 1, 32, 32); }
-    if (warp == 4 && lane == 0) TTT_TR(2, 15);
+      const float sc = mat == 0 ? 0.5f : 1.0f;             // G1 was accumulated from 2 dA
+      float4* dst = reinterpret_cast<float4*>(Pset + mat * me + row + 16 * tc);
+#pragma unroll
+      for (int v = 0; v < 4; ++v)
+        dst[v] = make_float4(sc * __uint_as_float(r[4 * v]), sc * __uint_as_float(r[4 * v + 1]),
+                             sc * __uint_as_float(r[4 * v + 2]), sc * __uint_as_float(r[4 * v + 3]));
+    }
+    if (ew == 0 && lane == 0) TTT_TR(4, 13);
     if (LOSS) {
       float l0, l1;
       unpack2(loss2, l0, l1);
       float loss = l0 + l1;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) loss += __shfl_xor_sync(0xffffffffu, loss, o);
-      if (lane == 0) loss_red[warp - 4] = loss;
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-      if (warp == 4 && lane == 0) {
+      if (lane == 0) loss_red[ew] = loss;
+      asm volatile("bar.sync 9, 512;" ::: "memory");
+      if (ew == 0 && lane == 0) {
         float t = 0.f;
-        for (int w = 0; w < 8; ++w) t += loss_red[w];
+        for (int w = 0; w < EPI_WARPS; ++w) t += loss_red[w];
         loss_part[((size_t)split * nslices + slice) * nh + h] = t;
       }
     }
@@ -328,6 +418,10 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   if (warp == 0) tmem_dealloc(tb, 512);
 #ifdef TTT_TRACE
   if (threadIdx.x == 0) tr_s[16 + 15] = (unsigned)clock();
+  if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) {
+    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    g_ttt_time[2] = t; g_ttt_time[3] = clock64();
+  }
   __syncthreads();
   if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0)
     for (int e = threadIdx.x; e < 64 * 16; e += blockDim.x) g_ttt_trace[e] = tr_s[e];
@@ -401,7 +495,7 @@ int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V
   if (rc != TTT_OK) return rc;
   rc = make_token_map(ctx, &mapV, V, M, (int64_t)c.nh * c.hd, ld, upd::T);
   if (rc != TTT_OK) return rc;
-  const size_t smem = (size_t)upd::STAGES * 2 * upd::TILE_BYTES + 1024;
+  const size_t smem = (size_t)upd::STAGES * upd::STAGE_BYTES + 1024;
   static bool attr_set = false;
   if (!attr_set) {
     TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_update_kernel<false>,
