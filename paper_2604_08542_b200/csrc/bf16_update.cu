@@ -94,8 +94,9 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   using namespace upd;
   constexpr int HD = 64;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) &
-                                             ~static_cast<uintptr_t>(1023));
+  // 1024-B aligned base, computed on the 32-bit shared-space address (a uniform value)
+  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
   __shared__ uint64_t full[STAGES], empty[STAGES], fwd_full[2], xb_free[2], g_free,
       epi_done[2], opnd_free, w_ready, grad_done;
   __shared__ uint32_t tmem_base_s;
@@ -134,6 +135,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   __syncthreads();
   tc_fence_after();
   const uint32_t tb = tmem_base_s;
+  if (tb != 0) __trap();      // all 512 columns belong to this CTA: the issuers use absolute columns
   if (tid == 0) TTT_TR(0, 14);
 
   if (warp == 0) {
@@ -153,80 +155,76 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     }
   } else if (warp == 1) {
     // ===================== forward-MMA issuer =====================
-    // Descriptors are built once; a step of b bytes in shared memory is +(b >> 4) on a descriptor.
-    constexpr uint32_t idesc_f = umma_idesc_bf16(HS, T, 0, 0);    // B = token tile, K-major
-    const uint64_t dk_f = umma_smem_desc_sw128(smem_u32(smem), 16, 1024);
-    constexpr uint64_t V_OFF = TILE_BYTES >> 4, ST_OFF = STAGE_BYTES >> 4;
-    mbar_wait(&w_ready, 0);
-    tc_fence_after();
-    for (int i = 0; i < ntiles; ++i) {
-      const int s = i % STAGES, it = i / STAGES;
-      TTT_TR(i, 0);
-      const int b = i & 1, n = i >> 1;
-      uint32_t g_ok;
-      // the three waits of a tile are probed together (an mbarrier probe costs ~90 clk even when the
-      // phase is already complete), then re-waited only if a probe failed
-      {
-        const uint32_t ok0 = mbar_try_wait(&full[s], it & 1);
+    // One elected thread runs the whole loop; it is bound by its own serial instruction stream, so
+    // everything it needs per tile is a constant or an increment: the CTA owns all 512 TMEM columns
+    // (base 0, checked above), stage descriptors advance by a fixed step, phases are flipped bits.
+    if (elect_one()) {
+      constexpr uint32_t idesc_f = umma_idesc_bf16(HS, T, 0, 0);    // B = token tile, K-major
+      constexpr uint32_t V_OFF = TILE_BYTES >> 4, ST_OFF = STAGE_BYTES >> 4;   // descriptor steps (16-B units)
+      const uint64_t d0 = umma_smem_desc_sw128(sbase, 16, 1024);
+      mbar_wait(&w_ready, 0);
+      tc_fence_after();
+      int s = 0;
+      uint32_t ph_full = 0;
+      uint64_t dk = d0;
+      for (int i = 0; i < ntiles; ++i) {
+        const int b = i & 1, n = i >> 1;
+        TTT_TR(i, 0);
+        // the waits of a tile are probed together (a probe costs ~90 clk even when the phase is
+        // already complete), then re-waited only if a probe failed
+        const uint32_t ok0 = mbar_try_wait(&full[s], ph_full);
         const uint32_t ok1 = n > 0 ? mbar_try_wait(&xb_free[b], (n - 1) & 1) : 1u;
         const uint32_t ok2 = i > 0 ? mbar_try_wait(&g_free, (i - 1) & 1) : 1u;
-        if (!ok0) mbar_wait(&full[s], it & 1);
+        if (!ok0) mbar_wait(&full[s], ph_full);
         if (!ok1) mbar_wait(&xb_free[b], (n - 1) & 1);
-        g_ok = ok2;
-      }
-      tc_fence_after();
-      TTT_TR(i, 1);
-      const uint64_t dk = dk_f + s * ST_OFF, dv = dk + V_OFF;
-      if (elect_one()) {
-        const uint32_t acc = tb + C_XB + b * XB_STRIDE;
+        tc_fence_after();
+        TTT_TR(i, 1);
+        const uint32_t acc = C_XB + b * XB_STRIDE;
 #pragma unroll
-        for (int k = 0; k < HD / 16; ++k) umma_ts(acc, tb + C_W1 + 8 * k, dk + 2 * k, idesc_f, k > 0);
+        for (int k = 0; k < HD / 16; ++k) umma_ts(acc, C_W1 + 8 * k, dk + 2 * k, idesc_f, k > 0);
 #pragma unroll
-        for (int k = 0; k < HD / 16; ++k) umma_ts(acc + 32, tb + C_W3 + 8 * k, dk + 2 * k, idesc_f, k > 0);
-      }
-      __syncwarp();
-      if (!g_ok) { mbar_wait(&g_free, (i - 1) & 1); tc_fence_after(); }   // g of tile i-1 is in registers
-      if (elect_one()) {
+        for (int k = 0; k < HD / 16; ++k) umma_ts(acc + 32, C_W3 + 8 * k, dk + 2 * k, idesc_f, k > 0);
+        if (!ok2) { mbar_wait(&g_free, (i - 1) & 1); tc_fence_after(); }   // g of tile i-1 is in registers
 #pragma unroll
-        for (int k = 0; k < HD / 16; ++k) umma_ts(tb + C_GG, tb + C_W2 + 8 * k, dv + 2 * k, idesc_f, k > 0);
+        for (int k = 0; k < HD / 16; ++k) umma_ts(C_GG, C_W2 + 8 * k, dk + V_OFF + 2 * k, idesc_f, k > 0);
         tc_commit(&fwd_full[b]);   // one barrier per epilogue group: a parity wait only tells the
-                                       // current phase from the previous one
+                                   // current phase from the previous one
+        TTT_TR(i, 2);
+        if (++s == STAGES) { s = 0; ph_full ^= 1; dk = d0; } else { dk += ST_OFF; }
       }
-      __syncwarp();
-      TTT_TR(i, 2);
     }
   } else if (warp == 3) {
     // ===================== gradient-MMA issuer =====================
-    constexpr uint32_t idesc_g = umma_idesc_bf16(HS, HD, 0, 1);   // B = token tile, MN-major
-    const uint64_t dk_g = umma_smem_desc_sw128(smem_u32(smem), TILE_BYTES, 1024);
-    constexpr uint64_t V_OFF = TILE_BYTES >> 4, ST_OFF = STAGE_BYTES >> 4;
-    for (int i = 0; i < ntiles; ++i) {
-      const int s = i % STAGES, b = i & 1, n = i >> 1;
-      mbar_wait(&epi_done[b], n & 1);
-      tc_fence_after();
-      TTT_TR(i, 3);
-      if (elect_one()) {
-        const uint64_t dk = dk_g + s * ST_OFF, dv = dk + V_OFF;
-        const uint32_t opnd = tb + C_H;                      // dA2 | dB | Hd, 8 columns per K step
+    if (elect_one()) {
+      constexpr uint32_t idesc_g = umma_idesc_bf16(HS, HD, 0, 1);   // B = token tile, MN-major
+      constexpr uint32_t V_OFF = TILE_BYTES >> 4, ST_OFF = STAGE_BYTES >> 4;
+      const uint64_t d0 = umma_smem_desc_sw128(sbase, TILE_BYTES, 1024);
+      int s = 0;
+      uint64_t dk = d0;
+      for (int i = 0; i < ntiles; ++i) {
+        const int b = i & 1, n = i >> 1;
+        mbar_wait(&epi_done[b], n & 1);
+        tc_fence_after();
+        TTT_TR(i, 3);
+        const uint32_t acc_flag = i > 0;
 #ifndef TTT_EXP_NOGRAD
 #pragma unroll
         for (int k = 0; k < T / 16; ++k)                     // +2048 B per 16-token K step
-          umma_ts(tb + C_G1, opnd + 8 * k, dk + 128 * k, idesc_g, (i > 0 || k > 0));
+          umma_ts(C_G1, C_H + 8 * k, dk + 128 * k, idesc_g, acc_flag | k);
 #pragma unroll
         for (int k = 0; k < T / 16; ++k)
-          umma_ts(tb + C_G3, opnd + 16 + 8 * k, dk + 128 * k, idesc_g, (i > 0 || k > 0));
+          umma_ts(C_G3, C_H + 16 + 8 * k, dk + 128 * k, idesc_g, acc_flag | k);
 #pragma unroll
         for (int k = 0; k < T / 16; ++k)
-          umma_ts(tb + C_G2, opnd + 32 + 8 * k, dv + 128 * k, idesc_g, (i > 0 || k > 0));
+          umma_ts(C_G2, C_H + 32 + 8 * k, dk + V_OFF + 128 * k, idesc_g, acc_flag | k);
 #endif
         tc_commit(&empty[s]);          // the tile's forward MMAs completed long ago (epilogue read them)
         tc_commit(&opnd_free);
+        TTT_TR(i, 4);
+        if (++s == STAGES) { s = 0; dk = d0; } else { dk += ST_OFF; }
       }
-      __syncwarp();
-      TTT_TR(i, 4);
+      tc_commit(&grad_done);
     }
-    if (elect_one()) tc_commit(&grad_done);
-    __syncwarp();
   } else if (warp == 2) {
     // ===================== learning-rate loader =====================
     // -eta of tile i (32 tokens = one 128-B line of lr) goes to the stage's shared-memory slot. The
