@@ -42,8 +42,9 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   using namespace app;
   constexpr int HD = 64;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) &
-                                             ~static_cast<uintptr_t>(1023));
+  // 1024-B aligned base, computed on the 32-bit shared-space address (a uniform value)
+  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
   __shared__ uint64_t w_full, fwd_full[2], epi_done[2], q_full[2], q_empty[2], o_full[2], o_empty[2];
   __shared__ uint64_t qr_full[QST], qr_empty[QST];
   __shared__ uint32_t tmem_base_s;
@@ -61,7 +62,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   if (tid == 0) {
     mbar_init(&w_full, 1);
     for (int b = 0; b < 2; ++b) {
-      mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 128);
+      mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 8);
       mbar_init(&q_full[b], 128); mbar_init(&q_empty[b], 1);
       mbar_init(&o_full[b], 1);   mbar_init(&o_empty[b], 128);
     }
@@ -73,6 +74,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   __syncthreads();
   tc_fence_after();
   const uint32_t tb = tmem_base_s;
+  if (tb != 0) __trap();      // all 512 columns belong to this CTA: the issuer uses absolute columns
 
   if (warp == 0) {
     // ===================== TMA producer: weights once, then the Q tiles =====================
@@ -80,11 +82,14 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       tma_prefetch_desc(&mapW);
       tma_prefetch_desc(&mapQ);
       mbar_arrive_expect_tx(&w_full, w_bytes);
-      // smem: [mat][H rows][128 B]; boxes of 64 rows (8 KB)
-      for (int mat = 0; mat < 3; ++mat)
-        for (int r = 0; r < H; r += 64)
-          tma_load_2d_hint(smem + ((size_t)mat * H + r) * 128, &mapW, &w_full, 0,
-                           (mat * nh + h) * H + r, kEvictLast);
+      // smem, boxes of 64 rows (8 KB): per 64-hidden step n [W1^T rows | W3^T rows] back to back
+      // (one 128-row K-major B operand), then the W2 row blocks
+      for (int n = 0; n < nsl; ++n) {
+        tma_load_2d_hint(smem + (size_t)n * 16384, &mapW, &w_full, 0, (0 * nh + h) * H + 64 * n, kEvictLast);
+        tma_load_2d_hint(smem + (size_t)n * 16384 + 8192, &mapW, &w_full, 0, (2 * nh + h) * H + 64 * n, kEvictLast);
+        tma_load_2d_hint(smem + (size_t)nsl * 16384 + (size_t)n * 8192, &mapW, &w_full, 0,
+                         (1 * nh + h) * H + 64 * n, kEvictLast);
+      }
       for (int tl = 0; tl < my_tiles; ++tl) {
         const int rs = tl % QST, it = tl / QST;
         mbar_wait(&qr_empty[rs], (it & 1) ^ 1);
@@ -96,37 +101,40 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (elect_one() && my_tiles > 0) {
-      constexpr uint32_t idesc_f = umma_idesc_bf16(TM, NS, 0, 0);   // B = W1^T / W3^T rows, K-major
-      constexpr uint32_t idesc_d = umma_idesc_bf16(TM, HD, 0, 1);   // B = W2 rows, MN-major
-      const uint32_t w1s = smem_u32(smem), w2s = w1s + H * 128, w3s = w2s + H * 128;
+      // The issuing thread is bound by its own serial instruction stream: absolute TMEM columns,
+      // descriptors that advance by fixed steps, and one 128-wide forward MMA per K step
+      // (Aq | Bq in one accumulator: W1^T and W3^T rows of a step are adjacent in shared memory).
+      constexpr uint32_t idesc_f = umma_idesc_bf16(TM, 2 * NS, 0, 0);  // B = [W1^T ; W3^T] rows, K-major
+      constexpr uint32_t idesc_d = umma_idesc_bf16(TM, HD, 0, 1);      // B = W2 rows, MN-major
+      const uint64_t d13 = umma_smem_desc_sw128(sbase, 16, 1024);
+      const uint64_t d2 = umma_smem_desc_sw128(sbase + nsl * 16384, 8192, 1024);
       mbar_wait(&w_full, 0);
       tc_fence_after();
+      // forward of step st+1 is issued before the down projection of step st
+      int f_tl = 0, f_n = 0;     // (tile, step) of the next forward
+      int d_tl = 0, d_n = 0;     // (tile, step) of the next down projection
       auto fwd = [&](int st) {
-        const int tl = st / nsl, n = st - tl * nsl, fb = st & 1, qb = tl & 1;
-        if (n == 0) { mbar_wait(&q_full[qb], (tl >> 1) & 1); tc_fence_after(); }
-        const uint32_t acc = tb + C_F + fb * 128, qop = tb + C_Q + qb * 32;
-        const uint32_t b1 = w1s + n * (NS * 128), b3 = w3s + n * (NS * 128);
+        const int fb = st & 1, qb = f_tl & 1;
+        if (f_n == 0) { mbar_wait(&q_full[qb], (f_tl >> 1) & 1); tc_fence_after(); }
+        const uint32_t acc = C_F + fb * 128, qop = C_Q + qb * 32;
+        const uint64_t b = d13 + (uint64_t)f_n * 1024;                 // 16 KB per step
 #pragma unroll
-        for (int k = 0; k < HD / 16; ++k)
-          umma_ts(acc, qop + 8 * k, umma_smem_desc_sw128(b1 + 32 * k, 16, 1024), idesc_f, k > 0);
-#pragma unroll
-        for (int k = 0; k < HD / 16; ++k)
-          umma_ts(acc + 64, qop + 8 * k, umma_smem_desc_sw128(b3 + 32 * k, 16, 1024), idesc_f, k > 0);
+        for (int k = 0; k < HD / 16; ++k) umma_ts(acc, qop + 8 * k, b + 2 * k, idesc_f, k > 0);
         tc_commit(&fwd_full[fb]);
-        if (n == nsl - 1) tc_commit(&q_empty[qb]);
+        if (++f_n == nsl) { tc_commit(&q_empty[qb]); f_n = 0; ++f_tl; }
       };
       auto down = [&](int st) {
-        const int tl = st / nsl, n = st - tl * nsl, fb = st & 1, ob = tl & 1;
-        mbar_wait(&epi_done[fb], (st >> 1) & 1);
-        if (n == 0) mbar_wait(&o_empty[ob], ((tl >> 1) & 1) ^ 1);
+        const int fb = st & 1, ob = d_tl & 1;
+        const uint32_t ok = mbar_try_wait(&epi_done[fb], (st >> 1) & 1);
+        if (d_n == 0) mbar_wait(&o_empty[ob], ((d_tl >> 1) & 1) ^ 1);
+        if (!ok) mbar_wait(&epi_done[fb], (st >> 1) & 1);
         tc_fence_after();
-        const uint32_t hq = tb + C_F + fb * 128, oacc = tb + C_O + ob * 64;
-        const uint32_t b2 = w2s + n * (NS * 128);
+        const uint32_t hq = C_F + fb * 128, oacc = C_O + ob * 64;
+        const uint64_t b = d2 + (uint64_t)d_n * 512;                   // 8 KB per step
 #pragma unroll
-        for (int k = 0; k < NS / 16; ++k)
-          umma_ts(oacc, hq + 8 * k, umma_smem_desc_sw128(b2 + 2048 * k, 8192, 1024), idesc_d,
-                  (n > 0 || k > 0));
-        if (n == nsl - 1) tc_commit(&o_full[ob]);
+        for (int k = 0; k < NS / 16; ++k)        // Hq K steps 0,1 at columns 0-15, K steps 2,3 at columns 32-47
+          umma_ts(oacc, hq + 32 * (k >> 1) + 8 * (k & 1), b + 128 * k, idesc_d, (d_n > 0 || k > 0));
+        if (++d_n == nsl) { tc_commit(&o_full[ob]); d_n = 0; ++d_tl; }
       };
       fwd(0);
       for (int st = 0; st < total_steps; ++st) {
@@ -136,36 +144,36 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
     }
   } else if (warp >= 4 && warp < 12) {
     // ===================== SwiGLU epilogue warpgroups =====================
+    // Both warpgroups work on every step (warpgroup wg owns hidden columns [32 wg, 32 wg + 32)), so
+    // consecutive steps run back to back on the MUFU pipe — the bound of this kernel at hd = 64
+    // (one tanh per element: 512 clk per 128 x 64 step at 16/clk against 384 clk of tensor work).
     const int wg = (warp - 4) >> 2, q = warp & 3;
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
     const uint64_t HALF2 = pack2(0.5f, 0.5f);
-    for (int st = wg; st < total_steps; st += 2) {
+    for (int st = 0; st < total_steps; ++st) {
       const int fb = st & 1;
-      const uint32_t buf = tb + lane_base + C_F + fb * 128;
+      const uint32_t buf = lane_base + C_F + fb * 128 + 32 * wg;
       mbar_wait(&fwd_full[fb], (st >> 1) & 1);
       tc_fence_after();
+      uint32_t ra[32], rb[32];
+      tmem_ld_x32(buf, ra);
+      tmem_ld_x32(buf + 64, rb);
+      tc_wait_ld();
+      uint32_t ph[16];
 #pragma unroll
-      for (int part = 0; part < 2; ++part) {     // 32 hidden columns at a time
-        uint32_t ra[32], rb[32];
-        tmem_ld_x32(buf + 32 * part, ra);
-        tmem_ld_x32(buf + 64 + 32 * part, rb);
-        tc_wait_ld();
-        uint32_t ph[16];
-#pragma unroll
-        for (int c = 0; c < 32; c += 2) {
-          const uint64_t a = pack2u(ra[c], ra[c + 1]);
-          const uint64_t bb = pack2u(rb[c], rb[c + 1]);
-          float x0, x1;
-          unpack2(fmul2(a, HALF2), x0, x1);
-          const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
-          const uint64_t sg = ffma2(th, HALF2, HALF2);             // sigmoid(a)
-          ph[c >> 1] = pack_bf16x2_from2(fmul2(fmul2(a, sg), bb));  // Hq = SiLU(a) b
-        }
-        tmem_st_x16(buf + 16 * part, ph);        // Hq (bf16) over the first 32 columns of Aq
+      for (int c = 0; c < 32; c += 2) {
+        const uint64_t hf = fmul2(pack2u(ra[c], ra[c + 1]), HALF2);   // a / 2
+        const uint64_t bb = pack2u(rb[c], rb[c + 1]);
+        float x0, x1;
+        unpack2(hf, x0, x1);
+        const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
+        ph[c >> 1] = pack_bf16x2_from2(fmul2(ffma2(hf, th, hf), bb));  // Hq = SiLU(a) b, SiLU(a) = h + h tanh(h)
       }
+      tmem_st_x16(buf, ph);        // Hq (bf16) over the first 16 of the 32 Aq columns this thread has read
       tc_wait_st();
       tc_fence_before();
-      mbar_arrive(&epi_done[fb]);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&epi_done[fb]);
     }
   } else if (warp >= 12) {
     // ===================== I/O warpgroup =====================
