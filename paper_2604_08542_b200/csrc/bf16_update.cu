@@ -129,6 +129,32 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     mbar_init(&w_ready, EPI_WARPS);
     mbar_init(&grad_done, 1);
     fence_mbar_init();
+    // the first ring of K/V tiles is requested before anything else: the first TMA round trip
+    // (descriptor fetch + HBM) is ~2 us and would otherwise start after the TMEM allocation
+    tma_prefetch_desc(&mapK);
+    tma_prefetch_desc(&mapV);
+    const int npre = min(ntiles, STAGES);
+    for (int i = 0; i < npre; ++i) {
+      mbar_arrive_expect_tx(&full[i], STAGE_BYTES);
+      uint8_t* dst = smem + i * STAGE_BYTES;
+      tma_load_2d(dst, &mapK, &full[i], h * HD, (tile_lo + i) * T);
+      tma_load_2d(dst + TILE_BYTES, &mapV, &full[i], h * HD, (tile_lo + i) * T);
+    }
+  }
+  __syncwarp();
+  // epilogue warps request their share of the bf16 weights now (row j of W1^T, W2, W3^T; 16-byte
+  // chunks 2 tc, 2 tc + 1), so the L2 latency overlaps the TMEM allocation
+  uint4 wpre[3][2];
+  if (warp >= 4) {
+    const int tc_ = (warp - 4) >> 2, j_ = (warp & 3) * 32 + lane;
+    const size_t me_ = (size_t)nh * H * HD;
+    const size_t row_ = ((size_t)h * H + (size_t)slice * HS + j_) * HD;
+#pragma unroll
+    for (int mat = 0; mat < 3; ++mat) {
+      const uint4* src = reinterpret_cast<const uint4*>(Wb + mat * me_ + row_) + 2 * tc_;
+      wpre[mat][0] = __ldg(src);
+      wpre[mat][1] = __ldg(src + 1);
+    }
   }
   if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
   tc_fence_before();
@@ -141,9 +167,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (elect_one()) {
-      tma_prefetch_desc(&mapK);
-      tma_prefetch_desc(&mapV);
-      for (int i = 0; i < ntiles; ++i) {
+      for (int i = STAGES; i < ntiles; ++i) {        // tiles 0 .. STAGES-1 were requested in the prologue
         const int s = i % STAGES, it = i / STAGES;
         mbar_wait(&empty[s], (it & 1) ^ 1);
         TTT_TR(i, 12);
@@ -269,13 +293,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       // weights -> TMEM as A operands: row j of W1^T / 2, W3^T, W2 (64 bf16 = 32 words each); warp
       // group tc loads 16-byte chunks 2 tc, 2 tc + 1 of each row (8 words = columns 8 tc .. 8 tc + 7)
       const uint32_t cols[3] = {C_W1, C_W2, C_W3};
-      uint4 x[3][2];
-#pragma unroll
-      for (int mat = 0; mat < 3; ++mat) {
-        const uint4* src = reinterpret_cast<const uint4*>(Wb + mat * me + row) + 2 * tc;
-        x[mat][0] = __ldg(src);
-        x[mat][1] = __ldg(src + 1);
-      }
+      uint4 (&x)[3][2] = wpre;           // requested before the TMEM allocation barrier
 #pragma unroll
       for (int mat = 0; mat < 3; ++mat) {
         uint32_t r[8] = {x[mat][0].x, x[mat][0].y, x[mat][0].z, x[mat][0].w,
