@@ -90,7 +90,9 @@ __global__ void __launch_bounds__(upd::THREADS, 1)
 bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
                    const __nv_bfloat16* __restrict__ Wb, const float* __restrict__ lr,
                    float* __restrict__ P, float* __restrict__ loss_part, int M, int nh, int H,
-                   int tiles_total, int tiles_per_split) {
+                   int tiles_total, int tiles_per_split, float* __restrict__ Wm,
+                   __nv_bfloat16* __restrict__ Wbw, unsigned* __restrict__ sync_ctr,
+                   unsigned sync_target) {
   using namespace upd;
   constexpr int HD = 64;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -432,6 +434,43 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   tc_fence_before();
   __syncthreads();
   if (warp == 0) tmem_dealloc(tb, 512);
+  if (Wm != nullptr) {
+    // ---- fused commit (plain update, Eq. 8): W <- W - sum_s P[s], summed in split order ----
+    // The `gridDim.x` CTAs that share this (head, slice) meet at a counter in global memory (the
+    // launch is cooperative: all CTAs are resident), then each commits its share of the slice's
+    // 3 x 128 rows: fp32 master + bf16 operand copy. Deterministic: fixed summation order.
+    const int nsplit = gridDim.x;
+    if (tid == 0) {
+      __threadfence();
+      atomicAdd(&sync_ctr[h * nslices + slice], 1u);
+      unsigned v;
+      long long t0 = clock64();
+      do {
+        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(sync_ctr + h * nslices + slice) : "memory");
+        if (clock64() - t0 > TTT_MBAR_TIMEOUT_CYCLES) __trap();
+      } while ((int)(v - sync_target) < 0);
+    }
+    __syncthreads();
+    const size_t me = (size_t)nh * H * HD, set = 3 * me;
+    const size_t row0 = ((size_t)h * H + (size_t)slice * HS) * HD;
+    constexpr int N4 = 3 * HS * HD / 4;                     // float4 per slice
+    const int chunk = (N4 + nsplit - 1) / nsplit;
+    const int e_hi = min(N4, (split + 1) * chunk);
+    for (int e = split * chunk + tid; e < e_hi; e += THREADS) {
+      const int mat = e / (HS * HD / 4), r4 = e % (HS * HD / 4);
+      const size_t off = mat * me + row0 + (size_t)r4 * 4;
+      float4 g = __ldcg(reinterpret_cast<const float4*>(P + off));
+#pragma unroll 4
+      for (int sp = 1; sp < nsplit; ++sp) {
+        const float4 p = __ldcg(reinterpret_cast<const float4*>(P + (size_t)sp * set + off));
+        g.x += p.x; g.y += p.y; g.z += p.z; g.w += p.w;
+      }
+      float4 w = *reinterpret_cast<const float4*>(Wm + off);
+      w.x -= g.x; w.y -= g.y; w.z -= g.z; w.w -= g.w;
+      *reinterpret_cast<float4*>(Wm + off) = w;
+      *reinterpret_cast<uint2*>(Wbw + off) = make_uint2(pack_bf16x2(w.x, w.y), pack_bf16x2(w.z, w.w));
+    }
+  }
 #ifdef TTT_TRACE
   if (threadIdx.x == 0) tr_s[16 + 15] = (unsigned)clock();
   if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) {
@@ -501,7 +540,7 @@ int bf16_supported(const ttt_config* cfg, char* why, size_t why_len) {
 }
 
 int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V, const float* lr,
-                    int64_t M, int64_t ld, bool want_loss, int* used, int* loss_rows,
+                    int64_t M, int64_t ld, bool want_loss, bool fuse_commit, int* used, int* loss_rows,
                     cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
   int tiles, tps, splits;
@@ -525,18 +564,26 @@ int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V
   const int nslices = c.hidden / upd::HS;
   float* P = ctx->partials + (size_t)ctx->n_partials * 3 * ctx->mat_elems;
   dim3 grid(splits, nslices, c.nh);
-  if (want_loss)
-    bf16_update_kernel<true><<<grid, upd::THREADS, smem, s>>>(mapK, mapV, ctx->Wb, lr, P,
-                                                             ctx->loss_part, (int)M, c.nh,
-                                                             c.hidden, tiles, tps);
-  else
-    bf16_update_kernel<false><<<grid, upd::THREADS, smem, s>>>(mapK, mapV, ctx->Wb, lr, P,
-                                                              ctx->loss_part, (int)M, c.nh,
-                                                              c.hidden, tiles, tps);
+  // fused commit: the CTAs of a (head, slice) group wait on one another, so they must all be
+  // resident -> cooperative launch (fails instead of deadlocking if the device cannot hold them)
+  fuse_commit = fuse_commit && (int)(grid.x * grid.y * grid.z) <= ctx->sm_count;
+  const __nv_bfloat16* Wb = ctx->Wb;
+  float* loss_part = ctx->loss_part;
+  int Mi = (int)M, nh = c.nh, H = c.hidden;
+  float* Wm = fuse_commit ? ctx->Wm : nullptr;
+  __nv_bfloat16* Wbw = fuse_commit ? ctx->Wb : nullptr;
+  unsigned* ctr = ctx->sync_ctr;
+  if (fuse_commit) ctx->sync_target += (unsigned)splits;
+  unsigned target = ctx->sync_target;
+  void* args[] = {&mapK, &mapV, &Wb, &lr, &P, &loss_part, &Mi, &nh, &H, &tiles, &tps, &Wm, &Wbw, &ctr, &target};
+  const void* fn = want_loss ? (const void*)bf16_update_kernel<true> : (const void*)bf16_update_kernel<false>;
+  cudaError_t e = fuse_commit ? cudaLaunchCooperativeKernel(fn, grid, dim3(upd::THREADS), args, smem, s)
+                              : cudaLaunchKernel(fn, grid, dim3(upd::THREADS), args, smem, s);
+  if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, "bf16_update_kernel launch", e);
   TTT_LAUNCH_CHECK(ctx, "bf16_update_kernel");
-  *used = splits;
+  *used = fuse_commit ? 0 : splits;
   *loss_rows = splits * nslices;
-  return TTT_OK;
+  return fuse_commit ? 1 : TTT_OK;     // 1 = gradient already committed by the kernel
 }
 
 }  // namespace ttt

@@ -34,8 +34,10 @@ int check_tokens(ttt_ctx* ctx, int64_t M, int64_t ld) {
   return TTT_OK;
 }
 
+// commit_now: the caller will commit right after (ttt_update / ttt_chunk_step); returns 1 if the
+// accumulate kernel has already committed (fused path), TTT_OK if a commit is still due
 int do_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, int64_t M,
-                  int64_t ld, float* loss, cudaStream_t s) {
+                  int64_t ld, float* loss, cudaStream_t s, bool commit_now = false) {
   const bool bf16 = ctx->cfg.act_dtype == TTT_BF16;
   const int need = bf16 ? bf16_partials_needed(ctx, M) : f32_partials_needed(ctx, M);
   if (need > ctx->cap_partials)
@@ -46,17 +48,23 @@ int do_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, i
     if (rc != TTT_OK) return rc;
   }
   int used = 0, loss_rows = 0, rc;
+  const bool fuse = commit_now && bf16 && ctx->cfg.ns_iters == 0 && ctx->cfg.renorm == 0 &&
+                    ctx->n_partials == 0 && !ctx->G_valid;
   if (bf16)
     rc = bf16_accumulate(ctx, static_cast<const __nv_bfloat16*>(K),
-                         static_cast<const __nv_bfloat16*>(V), lr, M, ld, loss != nullptr, &used,
-                         &loss_rows, s);
+                         static_cast<const __nv_bfloat16*>(V), lr, M, ld, loss != nullptr, fuse,
+                         &used, &loss_rows, s);
   else
     rc = f32_accumulate(ctx, static_cast<const float*>(K), static_cast<const float*>(V), lr, M, ld,
                         loss != nullptr, &used, &loss_rows, s);
-  if (rc != TTT_OK) return rc;
+  if (rc < 0) return rc;
+  const int committed = rc;
   ctx->n_partials += used;
-  if (loss != nullptr) return launch_loss_reduce(ctx, loss_rows, loss, s);
-  return TTT_OK;
+  if (loss != nullptr) {
+    rc = launch_loss_reduce(ctx, loss_rows, loss, s);
+    if (rc != TTT_OK) return rc;
+  }
+  return committed;
 }
 
 int do_apply(ttt_ctx* ctx, const void* Q, void* O, int64_t M, int64_t ld, cudaStream_t s) {
@@ -141,6 +149,11 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
   alloc((void**)&ctx->G, set * sizeof(float));
   alloc((void**)&ctx->partials, (size_t)ctx->cap_partials * set * sizeof(float));
   alloc((void**)&ctx->loss_part, (size_t)ctx->cap_loss_rows * cfg->nh * sizeof(float));
+  if (bf16) {
+    const size_t nctr = (size_t)cfg->nh * ((cfg->hidden + 127) / 128);
+    alloc((void**)&ctx->sync_ctr, nctr * sizeof(unsigned));
+    if (ok && cudaMemset(ctx->sync_ctr, 0, nctr * sizeof(unsigned)) != cudaSuccess) ok = false;
+  }
   if (!bf16) {
     const size_t act = (size_t)cfg->nh * cfg->max_tokens * cfg->hidden * sizeof(float);
     for (int i = 0; i < 3; ++i) alloc((void**)&ctx->act[i], act);
@@ -167,7 +180,7 @@ void ttt_destroy(ttt_ctx* ctx) {
   cudaSetDevice(ctx->cfg.device);
   cudaDeviceSynchronize();
   cudaFree(ctx->Wm); cudaFree(ctx->Wb); cudaFree(ctx->n0); cudaFree(ctx->colsq);
-  cudaFree(ctx->G); cudaFree(ctx->partials); cudaFree(ctx->loss_part); cudaFree(ctx->loss_blk);
+  cudaFree(ctx->G); cudaFree(ctx->partials); cudaFree(ctx->loss_part); cudaFree(ctx->loss_blk); cudaFree(ctx->sync_ctr);
   for (int i = 0; i < 3; ++i) cudaFree(ctx->act[i]);
   delete ctx;
 }
@@ -188,7 +201,8 @@ int ttt_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, 
   if (!ctx) return TTT_ERR_ARG;
   int rc = check_update_args(ctx, K, V, lr, M, ld);
   if (rc != TTT_OK || M == 0) return rc;
-  return do_accumulate(ctx, K, V, lr, M, ld, loss, static_cast<cudaStream_t>(stream));
+  rc = do_accumulate(ctx, K, V, lr, M, ld, loss, static_cast<cudaStream_t>(stream));
+  return rc < 0 ? rc : TTT_OK;
 }
 
 int ttt_commit(ttt_ctx* ctx, void* stream) {
@@ -216,9 +230,9 @@ int ttt_update(ttt_ctx* ctx, const void* K, const void* V, const float* lr, int6
   int rc = check_update_args(ctx, K, V, lr, M, ld);
   if (rc != TTT_OK || M == 0) return rc;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  rc = do_accumulate(ctx, K, V, lr, M, ld, loss, s);
-  if (rc != TTT_OK) return rc;
-  return launch_commit(ctx, s);
+  rc = do_accumulate(ctx, K, V, lr, M, ld, loss, s, true);
+  if (rc < 0) return rc;
+  return rc == 1 ? TTT_OK : launch_commit(ctx, s);
 }
 
 int ttt_apply(ttt_ctx* ctx, const void* Q, void* O, int64_t M, int64_t ld, void* stream) {
@@ -236,10 +250,12 @@ int ttt_chunk_step(ttt_ctx* ctx, const void* Q, const void* K, const void* V, co
   rc = check_apply_args(ctx, Q, O, M, ld);
   if (rc != TTT_OK || M == 0) return rc;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  rc = do_accumulate(ctx, K, V, lr, M, ld, loss, s);
-  if (rc != TTT_OK) return rc;
-  rc = launch_commit(ctx, s);
-  if (rc != TTT_OK) return rc;
+  rc = do_accumulate(ctx, K, V, lr, M, ld, loss, s, true);
+  if (rc < 0) return rc;
+  if (rc != 1) {
+    rc = launch_commit(ctx, s);
+    if (rc != TTT_OK) return rc;
+  }
   return do_apply(ctx, Q, O, M, ld, s);
 }
 

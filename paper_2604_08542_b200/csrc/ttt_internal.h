@@ -41,6 +41,10 @@ struct ttt_ctx {
   // f32 path workspaces: three [nh][max_tokens][H] fp32 activation buffers
   float* act[3];
 
+  // bf16 path: group-barrier counters of the fused commit ([nh][hidden/128]) and their running target
+  unsigned* sync_ctr;
+  unsigned sync_target;
+
   // bf16 path: driver entry point for cuTensorMapEncodeTiled
   void* encode_tiled;
 };
@@ -73,9 +77,11 @@ int f32_apply(ttt_ctx* ctx, const float* Q, float* O, int64_t M, int64_t ld, cud
 int f32_partials_needed(const ttt_ctx* ctx, int64_t M);
 
 // --- bf16 tensor-core path (bf16_update.cu / bf16_apply.cu) -------------------------------------
+// fuse_commit: also apply W <- W - gradient inside the kernel (plain update, nothing pending);
+// returns 1 (instead of TTT_OK) when it did, negative on error
 int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V, const float* lr,
-                    int64_t M, int64_t ld, bool want_loss, int* used, int* loss_rows,
-                    cudaStream_t s);
+                    int64_t M, int64_t ld, bool want_loss, bool fuse_commit, int* used,
+                    int* loss_rows, cudaStream_t s);
 int bf16_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
                cudaStream_t s);
 int bf16_partials_needed(const ttt_ctx* ctx, int64_t M);
