@@ -268,3 +268,49 @@ def test_error_codes_and_empty_chunk():
     t.ttt_chunk_step(Q[:0], Q[:0], Q[:0], lr[:, :0].contiguous())
     assert t.launch_count() == n0
     t.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# full BASELINE.json sizes, in the launch configuration bench.py times (all heads, full chunks);
+# the oracle checks a head subset (heads are independent units, so this is exact per head)
+# ------------------------------------------------------------------------------------------------
+def _full_size_stream(name, n_chunks, heads):
+    dev = torch.device("cuda", 0)
+    w = ti.CONFIGS[name]
+    W1, W2, W3 = ti.fast_weights(w)
+    cols = torch.cat([torch.arange(h * w.hd, (h + 1) * w.hd) for h in heads])
+    ora = OracleTTT(W1[heads], W2[heads], W3[heads], ns_iters=w.ns_iters, renorm=w.renorm)
+    gpu = _mk(w)
+    gpu.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    errs = []
+    for c, (Q, K, V, lr) in enumerate(ti.TokenStream(w)):
+        if c >= n_chunks:
+            break
+        O = gpu.ttt_chunk_step(Q.to(dev), K.to(dev), V.to(dev), lr.to(dev))
+        O_ref, _ = ora.chunk_step(Q[:, cols].contiguous(), K[:, cols].contiguous(),
+                                  V[:, cols].contiguous(), lr[heads].contiguous())
+        errs.append(rel_err(O[:, cols.to(dev)].float().cpu(), O_ref))
+    g = [x.cpu()[heads] for x in gpu.ttt_get_weights()]
+    errs_w = [rel_err(g[0], ora.W1), rel_err(g[1], ora.W2), rel_err(g[2], ora.W3)]
+    gpu.close()
+    return errs, errs_w
+
+
+def test_cfg2_full_size_sampled_heads():
+    """BASELINE.json:configs[1] exactly (16 heads x 64, H 128, 10 992 tokens, L2-normalised K)."""
+    errs, errs_w = _full_size_stream("cfg2", 1, [0, 7, 15])
+    assert max(errs) <= TOL_BF16 and max(errs_w) <= TOL_BF16, (errs, errs_w)
+
+
+def test_cfg3_full_size_sampled_heads():
+    """BASELINE.json:configs[2] exactly: 8 chunks x 10 992 tokens, H 256, Newton-Schulz, rho 0.9."""
+    errs, errs_w = _full_size_stream("cfg3", 8, [0, 15])
+    assert errs[-1] <= TOL_BF16 and max(errs) <= TOL_BF16, errs
+    assert max(errs_w) <= TOL_BF16, errs_w
+
+
+def test_cfg4_full_size_first_chunks_sampled_head():
+    """BASELINE.json:configs[3] shape (43 968-token chunks, renorm, L2-K); first 2 of the 63 chunks
+    (the float64 oracle needs ~3 s per head and chunk at this size)."""
+    errs, errs_w = _full_size_stream("cfg4", 2, [3])
+    assert max(errs) <= TOL_BF16 and max(errs_w) <= TOL_BF16, (errs, errs_w)
