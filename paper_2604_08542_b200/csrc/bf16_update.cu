@@ -158,6 +158,16 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       wpre[mat][1] = __ldg(src + 1);
     }
   }
+  // ... and the learning-rate loader its first batch (cold HBM latency off the first tile's path)
+  constexpr int LRPF = 8;
+  float lr_pre[LRPF];
+  if (warp == 2) {
+#pragma unroll
+    for (int u = 0; u < LRPF; ++u) {
+      const int t = (tile_lo + u) * T + lane;
+      lr_pre[u] = (u < ntiles && t < M) ? -__ldg(lr + (size_t)h * M + t) : 0.f;
+    }
+  }
   if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
   tc_fence_before();
   __syncthreads();
@@ -255,7 +265,6 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     // ===================== learning-rate loader =====================
     // -eta of tile i (32 tokens = one 128-B line of lr) goes to the stage's shared-memory slot. The
     // global loads run LRPF tiles ahead of the ring (register double buffer).
-    constexpr int LRPF = 8;
     const float* lrh = lr + (size_t)h * M;
     auto ld_batch = [&](int i0, float (&v)[LRPF]) {
 #pragma unroll
@@ -265,7 +274,8 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       }
     };
     float cur[LRPF], nxt[LRPF];
-    ld_batch(0, cur);
+#pragma unroll
+    for (int u = 0; u < LRPF; ++u) cur[u] = lr_pre[u];       // requested before the allocation barrier
     for (int i0 = 0; i0 < ntiles; i0 += LRPF) {
       ld_batch(i0 + LRPF, nxt);
 #pragma unroll
@@ -273,10 +283,11 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         const int i = i0 + u;
         if (i < ntiles) {
           const int s = i % STAGES, it = i / STAGES;
-          mbar_wait(&empty[s], (it & 1) ^ 1);
+          if (it > 0) mbar_wait(&empty[s], (it & 1) ^ 1);
           ne_s[s][lane] = cur[u];
           __syncwarp();
           if (lane == 0) mbar_arrive(&full[s]);
+
         }
       }
 #pragma unroll
