@@ -73,6 +73,9 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  // programmatic dependent launch: everything above overlapped the tail of the preceding kernel
+  // (the commit that produces the weights); nothing below may run before it has completed
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   const uint32_t tb = tmem_base_s;
   if (tb != 0) __trap();      // all 512 columns belong to this CTA: the issuer uses absolute columns
 
@@ -267,7 +270,19 @@ int bf16_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M
     attr_smem = smem;
   }
   dim3 grid(per_head, c.nh);
-  bf16_apply_kernel<<<grid, app::THREADS, smem, s>>>(mapW, mapQ, mapO, c.nh, c.hidden, tiles);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(app::THREADS);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  int nh = c.nh, H = c.hidden, ntl = tiles;
+  cudaError_t e = cudaLaunchKernelEx(&cfg, bf16_apply_kernel, mapW, mapQ, mapO, nh, H, ntl);
+  if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, "bf16_apply_kernel launch", e);
   TTT_LAUNCH_CHECK(ctx, "bf16_apply_kernel");
   return TTT_OK;
 }

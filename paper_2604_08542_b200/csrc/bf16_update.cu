@@ -402,6 +402,8 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       if (ew == 0 && lane == 0) TTT_TR(i, 9);
       TTT_TR2(i, ew, 3);
     }
+    // a dependent kernel (PDL) may be scheduled from here on; it still waits for this grid to finish
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // ---- flush the gradient accumulators: one fp32 partial slice per CTA ----
     if (ew == 0 && lane == 0) TTT_TR(2, 13);
     mbar_wait(&grad_done, 0);
