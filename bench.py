@@ -242,10 +242,9 @@ def run_ours(args, w, rank, local_rank, world):
         12.0 * M * w.d * w.hidden / (k_ms[0] * 1e-3) / 1e12
     app_tflops = flops_per_chunk(w, M, "apply") / (k_ms[2] * 1e-3) / 1e12
     step_tflops = flops_per_chunk(w, M, "step") / (ms_per_step * 1e-3) / 1e12
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", f"traffic_{w.name}.json")
-    if os.path.exists(tp):
-        traffic = json.load(open(tp)).get("bf16_update_kernel_dram_bytes_per_launch")
+    # dram__bytes_read.sum + dram__bytes_write.sum of bf16_update_kernel, one launch, from the
+    # `ncu --set full` captures summarised in profiles/r01b_ncu_full.md (None = not captured)
+    traffic = {"cfg2": 48123136 + 486912, "cfg4": 184645632 + 3801600}.get(w.name)
     # (the per-kernel pass calls ttt_accumulate / ttt_commit / ttt_apply separately; inside
     #  ttt_chunk_step the plain commit is fused into the update kernel's tail)
     roofline = {"kernel": "bf16_update_kernel" if w.act_dtype == "bf16" else "f32 path",
