@@ -32,8 +32,9 @@ constexpr int QST = 4;         // Q tile ring stages
 constexpr int TILE_BYTES = TM * 128;   // one [128 x 64] bf16 tile
 // TMEM column plan for hd = 64
 constexpr uint32_t C_Q = 0;      // 2 x 32 cols: Q operand (bf16)
-constexpr uint32_t C_O = 64;     // 2 x 64 cols: O accumulator (fp32)
-constexpr uint32_t C_F = 192;    // 2 x 128 cols: Aq (64) | Bq (64) forward accumulators (fp32)
+constexpr uint32_t C_O = 64;     // 64 cols: O accumulator (fp32), single
+constexpr uint32_t C_F = 128;    // 3 x 128 cols: Aq (64) | Bq (64) forward accumulators (fp32)
+constexpr int NF = 3;            // forward buffers: two in the epilogue (one per warpgroup) + one in the MMAs
 }  // namespace app
 
 __global__ void __launch_bounds__(app::THREADS, 1)
@@ -45,7 +46,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   // 1024-B aligned base, computed on the 32-bit shared-space address (a uniform value)
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
-  __shared__ uint64_t w_full, fwd_full[2], epi_done[2], q_full[2], q_empty[2], o_full[2], o_empty[2];
+  __shared__ uint64_t w_full, fwd_full[NF], epi_done[NF], q_full[2], q_empty[2], o_full, o_empty;
   __shared__ uint64_t qr_full[QST], qr_empty[QST];
   __shared__ uint32_t tmem_base_s;
 
@@ -61,11 +62,10 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
 
   if (tid == 0) {
     mbar_init(&w_full, 1);
-    for (int b = 0; b < 2; ++b) {
-      mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 8);
-      mbar_init(&q_full[b], 128); mbar_init(&q_empty[b], 1);
-      mbar_init(&o_full[b], 1);   mbar_init(&o_empty[b], 128);
-    }
+    for (int b = 0; b < NF; ++b) { mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 4); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&q_full[b], 128); mbar_init(&q_empty[b], 1); }
+    mbar_init(&o_full, 1);
+    mbar_init(&o_empty, 128);
     for (int s = 0; s < QST; ++s) { mbar_init(&qr_full[s], 1); mbar_init(&qr_empty[s], 128); }
     fence_mbar_init();
   }
@@ -116,63 +116,73 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       // forward of step st+1 is issued before the down projection of step st
       int f_tl = 0, f_n = 0;     // (tile, step) of the next forward
       int d_tl = 0, d_n = 0;     // (tile, step) of the next down projection
-      auto fwd = [&](int st) {
-        const int fb = st & 1, qb = f_tl & 1;
+      int f_fb = 0, d_fb = 0;    // forward buffer (st % NF) and its phase bit (st / NF) & 1
+      uint32_t f_ph = 0, d_ph = 0;
+      auto fwd = [&]() {
+        const int qb = f_tl & 1;
         if (f_n == 0) { mbar_wait(&q_full[qb], (f_tl >> 1) & 1); tc_fence_after(); }
-        const uint32_t acc = C_F + fb * 128, qop = C_Q + qb * 32;
+        const uint32_t acc = C_F + f_fb * 128, qop = C_Q + qb * 32;
         const uint64_t b = d13 + (uint64_t)f_n * 1024;                 // 16 KB per step
 #pragma unroll
         for (int k = 0; k < HD / 16; ++k) umma_ts(acc, qop + 8 * k, b + 2 * k, idesc_f, k > 0);
-        tc_commit(&fwd_full[fb]);
+        tc_commit(&fwd_full[f_fb]);
         if (++f_n == nsl) { tc_commit(&q_empty[qb]); f_n = 0; ++f_tl; }
+        if (++f_fb == NF) { f_fb = 0; f_ph ^= 1; }
       };
-      auto down = [&](int st) {
-        const int fb = st & 1, ob = d_tl & 1;
-        const uint32_t ok = mbar_try_wait(&epi_done[fb], (st >> 1) & 1);
-        if (d_n == 0) mbar_wait(&o_empty[ob], ((d_tl >> 1) & 1) ^ 1);
-        if (!ok) mbar_wait(&epi_done[fb], (st >> 1) & 1);
+      auto down = [&]() {
+        const uint32_t ok = mbar_try_wait(&epi_done[d_fb], d_ph);
+        if (d_n == 0 && d_tl > 0) mbar_wait(&o_empty, (d_tl - 1) & 1);   // O of the previous tile is in registers
+        if (!ok) mbar_wait(&epi_done[d_fb], d_ph);
         tc_fence_after();
-        const uint32_t hq = C_F + fb * 128, oacc = C_O + ob * 64;
+        const uint32_t hq = C_F + d_fb * 128;
         const uint64_t b = d2 + (uint64_t)d_n * 512;                   // 8 KB per step
 #pragma unroll
-        for (int k = 0; k < NS / 16; ++k)        // Hq K steps 0,1 at columns 0-15, K steps 2,3 at columns 32-47
-          umma_ts(oacc, hq + 32 * (k >> 1) + 8 * (k & 1), b + 128 * k, idesc_d, (d_n > 0 || k > 0));
-        if (++d_n == nsl) { tc_commit(&o_full[ob]); d_n = 0; ++d_tl; }
+        for (int k = 0; k < NS / 16; ++k)
+          umma_ts(C_O, hq + 8 * k, b + 128 * k, idesc_d, (d_n > 0 || k > 0));
+        if (++d_n == nsl) { tc_commit(&o_full); d_n = 0; ++d_tl; }
+        if (++d_fb == NF) { d_fb = 0; d_ph ^= 1; }
       };
-      fwd(0);
+      // the forward MMAs run two steps ahead of the down projection: one buffer per warpgroup in
+      // the epilogue, the third being filled
+      fwd();
+      if (total_steps > 1) fwd();
       for (int st = 0; st < total_steps; ++st) {
-        if (st + 1 < total_steps) fwd(st + 1);
-        down(st);
+        if (st + 2 < total_steps) fwd();
+        down();
       }
     }
   } else if (warp >= 4 && warp < 12) {
     // ===================== SwiGLU epilogue warpgroups =====================
-    // Both warpgroups work on every step (warpgroup wg owns hidden columns [32 wg, 32 wg + 32)), so
-    // consecutive steps run back to back on the MUFU pipe — the bound of this kernel at hd = 64
-    // (one tanh per element: 512 clk per 128 x 64 step at 16/clk against 384 clk of tensor work).
+    // The two warpgroups alternate steps (three forward buffers keep both fed), so one warpgroup's
+    // TMEM load/store phases overlap the other's MUFU burst — the MUFU pipe is the bound of this
+    // kernel at hd = 64 (one tanh per element: 512 clk per 128 x 64 step at 16/clk against 384 clk
+    // of tensor work).
     const int wg = (warp - 4) >> 2, q = warp & 3;
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
     const uint64_t HALF2 = pack2(0.5f, 0.5f);
-    for (int st = 0; st < total_steps; ++st) {
-      const int fb = st & 1;
-      const uint32_t buf = lane_base + C_F + fb * 128 + 32 * wg;
-      mbar_wait(&fwd_full[fb], (st >> 1) & 1);
+    for (int st = wg; st < total_steps; st += 2) {
+      const int fb = st % NF;
+      const uint32_t buf = lane_base + C_F + fb * 128;
+      mbar_wait(&fwd_full[fb], (st / NF) & 1);
       tc_fence_after();
-      uint32_t ra[32], rb[32];
-      tmem_ld_x32(buf, ra);
-      tmem_ld_x32(buf + 64, rb);
-      tc_wait_ld();
-      uint32_t ph[16];
 #pragma unroll
-      for (int c = 0; c < 32; c += 2) {
-        const uint64_t hf = fmul2(pack2u(ra[c], ra[c + 1]), HALF2);   // a / 2
-        const uint64_t bb = pack2u(rb[c], rb[c + 1]);
-        float x0, x1;
-        unpack2(hf, x0, x1);
-        const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
-        ph[c >> 1] = pack_bf16x2_from2(fmul2(ffma2(hf, th, hf), bb));  // Hq = SiLU(a) b, SiLU(a) = h + h tanh(h)
+      for (int part = 0; part < 2; ++part) {     // 32 hidden columns at a time
+        uint32_t ra[32], rb[32];
+        tmem_ld_x32(buf + 32 * part, ra);
+        tmem_ld_x32(buf + 64 + 32 * part, rb);
+        tc_wait_ld();
+        uint32_t ph[16];
+#pragma unroll
+        for (int c = 0; c < 32; c += 2) {
+          const uint64_t hf = fmul2(pack2u(ra[c], ra[c + 1]), HALF2);   // a / 2
+          const uint64_t bb = pack2u(rb[c], rb[c + 1]);
+          float x0, x1;
+          unpack2(hf, x0, x1);
+          const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
+          ph[c >> 1] = pack_bf16x2_from2(fmul2(ffma2(hf, th, hf), bb));  // Hq = SiLU(a) b, SiLU(a) = h + h tanh(h)
+        }
+        tmem_st_x16(buf + 16 * part, ph);        // Hq (bf16) over Aq columns this thread has already read
       }
-      tmem_st_x16(buf, ph);        // Hq (bf16) over the first 16 of the 32 Aq columns this thread has read
       tc_wait_st();
       tc_fence_before();
       __syncwarp();
@@ -203,15 +213,15 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       mbar_arrive(&q_full[qb]);
     };
     auto store_o = [&](int tl) {
-      const int ob = tl & 1;
-      mbar_wait(&o_full[ob], (tl >> 1) & 1);
+      const int ob = tl & 1;                                   // shared-memory staging buffer only
+      mbar_wait(&o_full, tl & 1);
       tc_fence_after();
       uint32_t ro[64];
-      tmem_ld_x32(tb + lane_base + C_O + ob * 64, *reinterpret_cast<uint32_t(*)[32]>(&ro[0]));
-      tmem_ld_x32(tb + lane_base + C_O + ob * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&ro[32]));
+      tmem_ld_x32(tb + lane_base + C_O, *reinterpret_cast<uint32_t(*)[32]>(&ro[0]));
+      tmem_ld_x32(tb + lane_base + C_O + 32, *reinterpret_cast<uint32_t(*)[32]>(&ro[32]));
       tc_wait_ld();
       tc_fence_before();
-      mbar_arrive(&o_empty[ob]);                               // TMEM buffer is free again
+      mbar_arrive(&o_empty);                                   // the O accumulator is free again
       // staging buffer `ob` was last used by tile tl-2: its TMA store must have read it
       if (tid == 12 * 32) tma_store_wait_read<1>();
       asm volatile("bar.sync 2, 128;" ::: "memory");
