@@ -27,7 +27,8 @@ int make_token_map(ttt_ctx* ctx, CUtensorMap* map, const void* base, int64_t row
 namespace app {
 constexpr int TM = 128;        // tokens per tile (MMA M)
 constexpr int NS = 64;         // hidden units per step
-constexpr int THREADS = 512;
+constexpr int THREADS = 768;    // 4 control warps, 16 epilogue warps, 4 I/O warps
+constexpr int IO_WARP0 = 20;
 constexpr int QST = 4;         // Q tile ring stages
 constexpr int TILE_BYTES = TM * 128;   // one [128 x 64] bf16 tile
 // TMEM column plan for hd = 64
@@ -62,7 +63,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
 
   if (tid == 0) {
     mbar_init(&w_full, 1);
-    for (int b = 0; b < NF; ++b) { mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 4); }
+    for (int b = 0; b < NF; ++b) { mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 8); }
     for (int b = 0; b < 2; ++b) { mbar_init(&q_full[b], 128); mbar_init(&q_empty[b], 1); }
     mbar_init(&o_full, 1);
     mbar_init(&o_empty, 128);
@@ -137,8 +138,8 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
         const uint32_t hq = C_F + d_fb * 128;
         const uint64_t b = d2 + (uint64_t)d_n * 512;                   // 8 KB per step
 #pragma unroll
-        for (int k = 0; k < NS / 16; ++k)
-          umma_ts(C_O, hq + 8 * k, b + 128 * k, idesc_d, (d_n > 0 || k > 0));
+        for (int k = 0; k < NS / 16; ++k)        // Hq K steps 0,1 at columns 0-15, K steps 2,3 at columns 32-47
+          umma_ts(C_O, hq + 32 * (k >> 1) + 8 * (k & 1), b + 128 * k, idesc_d, (d_n > 0 || k > 0));
         if (++d_n == nsl) { tc_commit(&o_full); d_n = 0; ++d_tl; }
         if (++d_fb == NF) { d_fb = 0; d_ph ^= 1; }
       };
@@ -151,29 +152,32 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
         down();
       }
     }
-  } else if (warp >= 4 && warp < 12) {
+  } else if (warp >= 4 && warp < IO_WARP0) {
     // ===================== SwiGLU epilogue warpgroups =====================
     // The two warpgroups alternate steps (three forward buffers keep both fed), so one warpgroup's
     // TMEM load/store phases overlap the other's MUFU burst — the MUFU pipe is the bound of this
     // kernel at hd = 64 (one tanh per element: 512 clk per 128 x 64 step at 16/clk against 384 clk
     // of tensor work).
-    const int wg = (warp - 4) >> 2, q = warp & 3;
+    // Four warpgroups: pair (wgp & 1) serves the steps of that parity, half (wgp >> 1) owns 32 of
+    // the step's 64 hidden columns — four epilogue warps per scheduler, two per step in flight.
+    const int wgp = (warp - 4) >> 2, q = warp & 3;
+    const int par = wgp & 1, half = wgp >> 1;
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
     const uint64_t HALF2 = pack2(0.5f, 0.5f);
-    for (int st = wg; st < total_steps; st += 2) {
+    for (int st = par; st < total_steps; st += 2) {
       const int fb = st % NF;
-      const uint32_t buf = lane_base + C_F + fb * 128;
+      const uint32_t buf = lane_base + C_F + fb * 128 + 32 * half;   // Aq columns; Bq 64 further
       mbar_wait(&fwd_full[fb], (st / NF) & 1);
       tc_fence_after();
 #pragma unroll
-      for (int part = 0; part < 2; ++part) {     // 32 hidden columns at a time
-        uint32_t ra[32], rb[32];
-        tmem_ld_x32(buf + 32 * part, ra);
-        tmem_ld_x32(buf + 64 + 32 * part, rb);
+      for (int part = 0; part < 2; ++part) {     // 16 hidden columns at a time
+        uint32_t ra[16], rb[16];
+        tmem_ld_x16(buf + 16 * part, ra);
+        tmem_ld_x16(buf + 64 + 16 * part, rb);
         tc_wait_ld();
-        uint32_t ph[16];
+        uint32_t ph[8];
 #pragma unroll
-        for (int c = 0; c < 32; c += 2) {
+        for (int c = 0; c < 16; c += 2) {
           const uint64_t hf = fmul2(pack2u(ra[c], ra[c + 1]), HALF2);   // a / 2
           const uint64_t bb = pack2u(rb[c], rb[c + 1]);
           float x0, x1;
@@ -181,14 +185,14 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
           const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
           ph[c >> 1] = pack_bf16x2_from2(fmul2(ffma2(hf, th, hf), bb));  // Hq = SiLU(a) b, SiLU(a) = h + h tanh(h)
         }
-        tmem_st_x16(buf + 16 * part, ph);        // Hq (bf16) over Aq columns this thread has already read
+        tmem_st_x8(buf + 8 * part, ph);          // Hq (bf16) over Aq columns this thread has already read
       }
       tc_wait_st();
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&epi_done[fb]);
     }
-  } else if (warp >= 12) {
+  } else if (warp >= IO_WARP0) {
     // ===================== I/O warpgroup =====================
     const int q = warp & 3;
     const int r = q * 32 + lane;                               // token row within the tile
@@ -223,7 +227,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       tc_fence_before();
       mbar_arrive(&o_empty);                                   // the O accumulator is free again
       // staging buffer `ob` was last used by tile tl-2: its TMA store must have read it
-      if (tid == 12 * 32) tma_store_wait_read<1>();
+      if (tid == IO_WARP0 * 32) tma_store_wait_read<1>();
       asm volatile("bar.sync 2, 128;" ::: "memory");
       uint8_t* rowp = o_stage + ob * TILE_BYTES + r * 128;
 #pragma unroll
@@ -237,7 +241,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       }
       fence_proxy_async_smem();
       asm volatile("bar.sync 2, 128;" ::: "memory");
-      if (tid == 12 * 32) {
+      if (tid == IO_WARP0 * 32) {
         tma_store_2d(&mapO, o_stage + ob * TILE_BYTES, h * HD,
                      ((int)blockIdx.x + tl * (int)gridDim.x) * TM);
         tma_store_commit();
@@ -249,7 +253,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       store_o(tl);
       if (tl + 2 < my_tiles) load_q(tl + 2);
     }
-    if (tid == 12 * 32) tma_store_wait<0>();
+    if (tid == IO_WARP0 * 32) tma_store_wait<0>();
   }
   tc_fence_before();
   __syncthreads();
