@@ -542,13 +542,16 @@ int bf16_partials_needed(const ttt_ctx* ctx, int64_t M) {
   return s;
 }
 
+int bf16_tensor_path(const ttt_config* cfg) {
+  return cfg->hd == 64 && (cfg->hidden == 128 || cfg->hidden == 256) && !cfg->linear_fast_weight;
+}
+
+// bf16 token tensors are accepted for every shape the fp32 path takes; shapes outside the tcgen05
+// kernels' set (hd = 64, hidden 128 | 256) run on the fp32 CUDA-core kernels behind a bf16 <-> fp32
+// conversion (same semantics, fp32 arithmetic).
 int bf16_supported(const ttt_config* cfg, char* why, size_t why_len) {
-  if (cfg->hd != 64) { snprintf(why, why_len, "bf16 path: hd must be 64 (got %d)", cfg->hd); return 0; }
-  if (cfg->hidden % 128 != 0 || cfg->hidden < 128 || cfg->hidden > 256) {
-    snprintf(why, why_len, "bf16 path: hidden must be 128 or 256 (got %d)", cfg->hidden);
-    return 0;
-  }
   if (cfg->linear_fast_weight) { snprintf(why, why_len, "bf16 path: linear test mode is f32-only"); return 0; }
+  if (cfg->hd % 8 != 0) { snprintf(why, why_len, "bf16 path: hd must be a multiple of 8 (got %d)", cfg->hd); return 0; }
   return 1;
 }
 

@@ -205,6 +205,51 @@ f32_out_kernel(const float* __restrict__ Hq, const float* __restrict__ Wm, float
   }
 }
 
+// bf16 <-> fp32 conversion of token tensors (bf16 I/O on this path): 8 elements per thread
+__global__ void bf16_to_f32_kernel(const __nv_bfloat16* __restrict__ src, long ld, float* __restrict__ dst,
+                                   long M, int cols) {
+  const long e = ((long)blockIdx.x * blockDim.x + threadIdx.x) * 8;
+  if (e >= M * cols) return;
+  const long r = e / cols, c = e % cols;
+  const uint4 x = *reinterpret_cast<const uint4*>(src + r * ld + c);
+  const uint32_t w[4] = {x.x, x.y, x.z, x.w};
+  float4 a, b;
+  a.x = __uint_as_float(w[0] << 16); a.y = __uint_as_float(w[0] & 0xffff0000u);
+  a.z = __uint_as_float(w[1] << 16); a.w = __uint_as_float(w[1] & 0xffff0000u);
+  b.x = __uint_as_float(w[2] << 16); b.y = __uint_as_float(w[2] & 0xffff0000u);
+  b.z = __uint_as_float(w[3] << 16); b.w = __uint_as_float(w[3] & 0xffff0000u);
+  reinterpret_cast<float4*>(dst + e)[0] = a;
+  reinterpret_cast<float4*>(dst + e)[1] = b;
+}
+__global__ void f32_to_bf16_kernel(const float* __restrict__ src, __nv_bfloat16* __restrict__ dst, long ld,
+                                   long M, int cols) {
+  const long e = ((long)blockIdx.x * blockDim.x + threadIdx.x) * 8;
+  if (e >= M * cols) return;
+  const long r = e / cols, c = e % cols;
+  const float4 a = reinterpret_cast<const float4*>(src + e)[0], b = reinterpret_cast<const float4*>(src + e)[1];
+  __nv_bfloat162 p0 = __floats2bfloat162_rn(a.x, a.y), p1 = __floats2bfloat162_rn(a.z, a.w),
+                 p2 = __floats2bfloat162_rn(b.x, b.y), p3 = __floats2bfloat162_rn(b.z, b.w);
+  uint4 o;
+  o.x = *reinterpret_cast<uint32_t*>(&p0); o.y = *reinterpret_cast<uint32_t*>(&p1);
+  o.z = *reinterpret_cast<uint32_t*>(&p2); o.w = *reinterpret_cast<uint32_t*>(&p3);
+  *reinterpret_cast<uint4*>(dst + r * ld + c) = o;
+}
+
+int launch_bf16_to_f32(ttt_ctx* ctx, const __nv_bfloat16* src, int64_t ld, float* dst, int64_t M, cudaStream_t s) {
+  const int cols = ctx->cfg.nh * ctx->cfg.hd;
+  const long n8 = (long)M * cols / 8;
+  bf16_to_f32_kernel<<<(unsigned)((n8 + 255) / 256), 256, 0, s>>>(src, ld, dst, M, cols);
+  TTT_LAUNCH_CHECK(ctx, "bf16_to_f32_kernel");
+  return TTT_OK;
+}
+int launch_f32_to_bf16(ttt_ctx* ctx, const float* src, __nv_bfloat16* dst, int64_t ld, int64_t M, cudaStream_t s) {
+  const int cols = ctx->cfg.nh * ctx->cfg.hd;
+  const long n8 = (long)M * cols / 8;
+  f32_to_bf16_kernel<<<(unsigned)((n8 + 255) / 256), 256, 0, s>>>(src, dst, ld, M, cols);
+  TTT_LAUNCH_CHECK(ctx, "f32_to_bf16_kernel");
+  return TTT_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 static int f32_splits(const ttt_ctx* ctx, int64_t M, int* tokens_per_split) {
   // token ranges are multiples of the 64-token fwd tile so loss partials map onto splits

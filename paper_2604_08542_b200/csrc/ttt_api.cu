@@ -38,7 +38,14 @@ int check_tokens(ttt_ctx* ctx, int64_t M, int64_t ld) {
 // accumulate kernel has already committed (fused path), TTT_OK if a commit is still due
 int do_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, int64_t M,
                   int64_t ld, float* loss, cudaStream_t s, bool commit_now = false) {
-  const bool bf16 = ctx->cfg.act_dtype == TTT_BF16;
+  const bool bf16 = ctx->cfg.act_dtype == TTT_BF16 && !ctx->bf16_via_f32;
+  if (ctx->bf16_via_f32) {      // bf16 I/O on the fp32 CUDA-core path: convert K, V first
+    const int64_t d = (int64_t)ctx->cfg.nh * ctx->cfg.hd;
+    int rc = launch_bf16_to_f32(ctx, static_cast<const __nv_bfloat16*>(K), ld, ctx->stage[0], M, s);
+    if (rc == TTT_OK) rc = launch_bf16_to_f32(ctx, static_cast<const __nv_bfloat16*>(V), ld, ctx->stage[1], M, s);
+    if (rc != TTT_OK) return rc;
+    K = ctx->stage[0]; V = ctx->stage[1]; ld = d;
+  }
   const int need = bf16 ? bf16_partials_needed(ctx, M) : f32_partials_needed(ctx, M);
   if (need > ctx->cap_partials)
     return fail(ctx, TTT_ERR_SHAPE, "internal: %lld partial sets needed, capacity %lld", need,
@@ -68,6 +75,13 @@ int do_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, i
 }
 
 int do_apply(ttt_ctx* ctx, const void* Q, void* O, int64_t M, int64_t ld, cudaStream_t s) {
+  if (ctx->bf16_via_f32) {
+    const int64_t d = (int64_t)ctx->cfg.nh * ctx->cfg.hd;
+    int rc = launch_bf16_to_f32(ctx, static_cast<const __nv_bfloat16*>(Q), ld, ctx->stage[0], M, s);
+    if (rc == TTT_OK) rc = f32_apply(ctx, ctx->stage[0], ctx->stage[1], M, d, s);
+    if (rc == TTT_OK) rc = launch_f32_to_bf16(ctx, ctx->stage[1], static_cast<__nv_bfloat16*>(O), ld, M, s);
+    return rc;
+  }
   if (ctx->cfg.act_dtype == TTT_BF16)
     return bf16_apply(ctx, static_cast<const __nv_bfloat16*>(Q), static_cast<__nv_bfloat16*>(O), M,
                       ld, s);
@@ -131,7 +145,8 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
   ctx->sm_count = prop.multiProcessorCount;
   ctx->mat_elems = (size_t)cfg->nh * cfg->hidden * cfg->hd;
   const size_t set = 3 * ctx->mat_elems;
-  const bool bf16 = cfg->act_dtype == TTT_BF16;
+  ctx->bf16_via_f32 = cfg->act_dtype == TTT_BF16 && !bf16_tensor_path(cfg);
+  const bool bf16 = cfg->act_dtype == TTT_BF16 && !ctx->bf16_via_f32;
   ctx->cap_partials = 2 * (bf16 ? bf16_partials_needed(ctx, cfg->max_tokens)
                                 : f32_partials_needed(ctx, cfg->max_tokens));
   if (ctx->cap_partials < 4) ctx->cap_partials = 4;
@@ -153,6 +168,11 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
     const size_t nctr = (size_t)cfg->nh * ((cfg->hidden + 127) / 128);
     alloc((void**)&ctx->sync_ctr, nctr * sizeof(unsigned));
     if (ok && cudaMemset(ctx->sync_ctr, 0, nctr * sizeof(unsigned)) != cudaSuccess) ok = false;
+  }
+  if (ctx->bf16_via_f32) {
+    const size_t st = (size_t)cfg->max_tokens * cfg->nh * cfg->hd * sizeof(float);
+    alloc((void**)&ctx->stage[0], st);
+    alloc((void**)&ctx->stage[1], st);
   }
   if (!bf16) {
     const size_t act = (size_t)cfg->nh * cfg->max_tokens * cfg->hidden * sizeof(float);
@@ -180,7 +200,7 @@ void ttt_destroy(ttt_ctx* ctx) {
   cudaSetDevice(ctx->cfg.device);
   cudaDeviceSynchronize();
   cudaFree(ctx->Wm); cudaFree(ctx->Wb); cudaFree(ctx->n0); cudaFree(ctx->colsq);
-  cudaFree(ctx->G); cudaFree(ctx->partials); cudaFree(ctx->loss_part); cudaFree(ctx->loss_blk); cudaFree(ctx->sync_ctr);
+  cudaFree(ctx->G); cudaFree(ctx->partials); cudaFree(ctx->loss_part); cudaFree(ctx->loss_blk); cudaFree(ctx->sync_ctr); cudaFree(ctx->stage[0]); cudaFree(ctx->stage[1]);
   for (int i = 0; i < 3; ++i) cudaFree(ctx->act[i]);
   delete ctx;
 }

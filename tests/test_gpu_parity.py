@@ -141,6 +141,16 @@ def test_bf16_stream_parity(base, kw):
     assert max(errs_l) <= TOL_LOSS_BF16, errs_l
 
 
+def test_bf16_cfg5_shape_runs_on_the_fp32_cuda_core_path():
+    """hd = 128 / H = 512 (BASELINE.json:configs[4] shape, cut down): bf16 I/O through the C ABI; this
+    shape is outside the tcgen05 kernels' set and runs on the fp32 CUDA-core kernels."""
+    w = _bf16_workload("cfg5", nh=2, tokens_per_frame=137, frames_per_chunk=2, n_frames=6)
+    errs_o, errs_w, errs_l = _run_stream(w)
+    assert max(errs_o) <= TOL_BF16, errs_o
+    assert max(errs_w) <= TOL_BF16, errs_w
+    assert max(errs_l) <= TOL_LOSS_BF16, errs_l
+
+
 def test_bf16_gradient_against_oracle():
     """The raw gradient (before the commit) is the most sensitive quantity: compare G1, G2, G3."""
     dev = torch.device("cuda", 0)
@@ -245,7 +255,7 @@ def test_error_codes_and_empty_chunk():
     from paper_2604_08542_b200 import TTT, TTT_BF16, TTT_F32, TTTError
     dev = torch.device("cuda", 0)
     with pytest.raises(TTTError) as e:
-        TTT(2, 48, 128, TTT_BF16)                       # hd not supported on the tensor path
+        TTT(2, 36, 128, TTT_BF16)                       # bf16 token rows need hd % 8 == 0
     assert e.value.status == -5
     t = TTT(2, 64, 128, TTT_BF16, max_tokens=256)
     Q = torch.zeros(64, 128, dtype=torch.bfloat16, device=dev)
