@@ -92,7 +92,8 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
                    float* __restrict__ P, float* __restrict__ loss_part, int M, int nh, int H,
                    int tiles_total, int tiles_per_split, float* __restrict__ Wm,
                    __nv_bfloat16* __restrict__ Wbw, unsigned* __restrict__ sync_ctr,
-                   unsigned sync_target) {
+                   unsigned sync_target, const float* __restrict__ renorm_n0,
+                   float* __restrict__ renorm_colsq) {
   using namespace upd;
   constexpr int HD = 64;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -448,7 +449,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   __syncthreads();
   if (warp == 0) tmem_dealloc(tb, 512);
   if (Wm != nullptr) {
-    // ---- fused commit (plain update, Eq. 8): W <- W - sum_s P[s], summed in split order ----
+    // ---- fused commit (Eq. 8): W <- W - sum_s P[s], summed in split order [+ re-normalisation] ----
     // The `gridDim.x` CTAs that share this (head, slice) meet at a counter in global memory (the
     // launch is cooperative: all CTAs are resident), then each commits its share of the slice's
     // 3 x 128 rows: fp32 master + bf16 operand copy. Deterministic: fixed summation order.
@@ -467,21 +468,58 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     const size_t me = (size_t)nh * H * HD, set = 3 * me;
     const size_t row0 = ((size_t)h * H + (size_t)slice * HS) * HD;
     constexpr int N4 = 3 * HS * HD / 4;                     // float4 per slice
-    const int chunk = (N4 + nsplit - 1) / nsplit;
-    const int e_hi = min(N4, (split + 1) * chunk);
-    for (int e = split * chunk + tid; e < e_hi; e += THREADS) {
-      const int mat = e / (HS * HD / 4), r4 = e % (HS * HD / 4);
+    constexpr int RQ = HD / 4;                              // float4 per row (16 lanes own one row)
+    const int chunk = ((N4 + nsplit - 1) / nsplit + RQ - 1) / RQ * RQ;   // whole rows per CTA
+    const int e_lo = min(N4, split * chunk), e_hi = min(N4, e_lo + chunk);
+    float4 colacc = make_float4(0.f, 0.f, 0.f, 0.f);        // renorm: W2 column sums of squares
+    for (int base = e_lo; base < e_hi; base += THREADS) {   // THREADS % 16 == 0: a lane keeps its columns
+      const int e = base + tid;
+      const bool ok = e < e_hi;
+      const int mat = ok ? e / (HS * HD / 4) : 0, r4 = ok ? e % (HS * HD / 4) : 0;
       const size_t off = mat * me + row0 + (size_t)r4 * 4;
-      float4 g = __ldcg(reinterpret_cast<const float4*>(P + off));
+      float4 w = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (ok) {
+        float4 g = __ldcg(reinterpret_cast<const float4*>(P + off));
 #pragma unroll 4
-      for (int sp = 1; sp < nsplit; ++sp) {
-        const float4 p = __ldcg(reinterpret_cast<const float4*>(P + (size_t)sp * set + off));
-        g.x += p.x; g.y += p.y; g.z += p.z; g.w += p.w;
+        for (int sp = 1; sp < nsplit; ++sp) {
+          const float4 p = __ldcg(reinterpret_cast<const float4*>(P + (size_t)sp * set + off));
+          g.x += p.x; g.y += p.y; g.z += p.z; g.w += p.w;
+        }
+        w = *reinterpret_cast<const float4*>(Wm + off);
+        w.x -= g.x; w.y -= g.y; w.z -= g.z; w.w -= g.w;
       }
-      float4 w = *reinterpret_cast<const float4*>(Wm + off);
-      w.x -= g.x; w.y -= g.y; w.z -= g.z; w.w -= g.w;
-      *reinterpret_cast<float4*>(Wm + off) = w;
-      *reinterpret_cast<uint2*>(Wbw + off) = make_uint2(pack_bf16x2(w.x, w.y), pack_bf16x2(w.z, w.w));
+      if (renorm_n0 != nullptr) {
+        if (mat != 1) {       // W1^T / W3^T: a row is a unit's fan-in vector -> back to its initial norm
+          float sq = w.x * w.x + w.y * w.y + w.z * w.z + w.w * w.w;
+#pragma unroll
+          for (int o = RQ / 2; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+          const int j = slice * HS + r4 / RQ;
+          const float* n0m = renorm_n0 + (mat == 0 ? (size_t)h * H : (size_t)nh * H + (size_t)nh * HD + (size_t)h * H);
+          const float f = ok ? n0m[j] / (sqrtf(sq) + 1e-5f) : 0.f;
+          w.x *= f; w.y *= f; w.z *= f; w.w *= f;
+        } else if (ok) {      // W2: fan-in = column; finished by renorm_w2_kernel from per-CTA partials
+          colacc.x = fmaf(w.x, w.x, colacc.x); colacc.y = fmaf(w.y, w.y, colacc.y);
+          colacc.z = fmaf(w.z, w.z, colacc.z); colacc.w = fmaf(w.w, w.w, colacc.w);
+        }
+      }
+      if (ok) {
+        *reinterpret_cast<float4*>(Wm + off) = w;
+        *reinterpret_cast<uint2*>(Wbw + off) = make_uint2(pack_bf16x2(w.x, w.y), pack_bf16x2(w.z, w.w));
+      }
+    }
+    if (renorm_n0 != nullptr) {
+      float4* cs = reinterpret_cast<float4*>(smem);         // the K/V ring is idle by now
+      cs[tid] = colacc;
+      __syncthreads();
+      if (tid < RQ) {
+        float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int r = 0; r < THREADS / RQ; ++r) {            // fixed order
+          const float4 v = cs[r * RQ + tid];
+          t.x += v.x; t.y += v.y; t.z += v.z; t.w += v.w;
+        }
+        const int nblk = nslices * nsplit;
+        *reinterpret_cast<float4*>(renorm_colsq + ((size_t)h * nblk + slice * nsplit + split) * HD + 4 * tid) = t;
+      }
     }
   }
 #ifdef TTT_TRACE
@@ -591,7 +629,10 @@ int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V
   unsigned* ctr = ctx->sync_ctr;
   if (fuse_commit) ctx->sync_target += (unsigned)splits;
   unsigned target = ctx->sync_target;
-  void* args[] = {&mapK, &mapV, &Wb, &lr, &P, &loss_part, &Mi, &nh, &H, &tiles, &tps, &Wm, &Wbw, &ctr, &target};
+  const float* rn0 = (fuse_commit && c.renorm) ? ctx->n0 : nullptr;
+  float* rcs = ctx->colsq;
+  void* args[] = {&mapK, &mapV, &Wb, &lr, &P, &loss_part, &Mi, &nh, &H, &tiles, &tps, &Wm, &Wbw, &ctr, &target,
+                  &rn0, &rcs};
   const void* fn = want_loss ? (const void*)bf16_update_kernel<true> : (const void*)bf16_update_kernel<false>;
   cudaError_t e = fuse_commit ? cudaLaunchCooperativeKernel(fn, grid, dim3(upd::THREADS), args, smem, s)
                               : cudaLaunchKernel(fn, grid, dim3(upd::THREADS), args, smem, s);
@@ -599,6 +640,10 @@ int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V
   TTT_LAUNCH_CHECK(ctx, "bf16_update_kernel");
   *used = fuse_commit ? 0 : splits;
   *loss_rows = splits * nslices;
+  if (fuse_commit && c.renorm) {       // W2's column fan-in norms span the head's slices: finish them
+    rc = launch_renorm_w2(ctx, nslices * splits, s);
+    if (rc != TTT_OK) return rc;
+  }
   return fuse_commit ? 1 : TTT_OK;     // 1 = gradient already committed by the kernel
 }
 

@@ -403,6 +403,15 @@ int launch_loss_reduce(ttt_ctx* ctx, int n, float* loss, cudaStream_t s) {
   return TTT_OK;
 }
 
+int launch_renorm_w2(ttt_ctx* ctx, int nblk, cudaStream_t s) {
+  const ttt_config& c = ctx->cfg;
+  const int nrow = (c.hidden + CM_ROWS - 1) / CM_ROWS;
+  renorm_w2_kernel<<<dim3(nrow, c.nh), 256, 0, s>>>(ctx->Wm, ctx->Wb, ctx->colsq, ctx->n0, nblk, c.nh,
+                                                    c.hd, c.hidden);
+  TTT_LAUNCH_CHECK(ctx, "renorm_w2_kernel");
+  return TTT_OK;
+}
+
 int launch_commit(ttt_ctx* ctx, cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
   if (c.ns_iters > 0 && ns_tc_supported(&c)) {
@@ -435,9 +444,8 @@ int launch_commit(ttt_ctx* ctx, cudaStream_t s) {
                                                     tpr);
   TTT_LAUNCH_CHECK(ctx, "commit_kernel");
   if (c.renorm) {
-    renorm_w2_kernel<<<dim3(nblk, c.nh), 256, 0, s>>>(ctx->Wm, ctx->Wb, ctx->colsq, ctx->n0, nblk,
-                                                      c.nh, c.hd, c.hidden);
-    TTT_LAUNCH_CHECK(ctx, "renorm_w2_kernel");
+    int rc = launch_renorm_w2(ctx, nblk, s);
+    if (rc != TTT_OK) return rc;
   }
   ctx->G_valid = false;
   ctx->n_partials = 0;

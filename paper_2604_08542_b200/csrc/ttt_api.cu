@@ -55,7 +55,7 @@ int do_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, i
     if (rc != TTT_OK) return rc;
   }
   int used = 0, loss_rows = 0, rc;
-  const bool fuse = commit_now && bf16 && ctx->cfg.ns_iters == 0 && ctx->cfg.renorm == 0 &&
+  const bool fuse = commit_now && bf16 && ctx->cfg.ns_iters == 0 &&
                     ctx->n_partials == 0 && !ctx->G_valid;
   if (bf16)
     rc = bf16_accumulate(ctx, static_cast<const __nv_bfloat16*>(K),
@@ -151,7 +151,7 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
                                 : f32_partials_needed(ctx, cfg->max_tokens));
   if (ctx->cap_partials < 4) ctx->cap_partials = 4;
   ctx->cap_loss_rows = ctx->cap_partials * ((cfg->hidden + 127) / 128);
-  const int nblk = (cfg->hidden + 15) / 16;
+  const int nblk = (cfg->hidden + 15) / 16 + 160;   // commit row blocks, or (slices x splits) of the fused commit
 
   bool ok = true;
   auto alloc = [&](void** p, size_t bytes) {

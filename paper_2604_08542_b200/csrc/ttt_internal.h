@@ -64,6 +64,8 @@ int launch_get_weights(ttt_ctx* ctx, float* W1, float* W2, float* W3, cudaStream
 int launch_reduce_pending(ttt_ctx* ctx, cudaStream_t s);
 // [NS] -> W -= pending -> [renorm] -> bf16 copy; clears the pending set
 int launch_commit(ttt_ctx* ctx, cudaStream_t s);
+// W2[:, o] *= n0[o] / (||W2[:, o]|| + 1e-5) from `nblk` per-head partial column sums of squares in colsq
+int launch_renorm_w2(ttt_ctx* ctx, int nblk, cudaStream_t s);
 // loss[h] = sum_{r in [0, n)} loss_part[r][h]  (fixed order)
 int launch_loss_reduce(ttt_ctx* ctx, int n, float* loss, cudaStream_t s);
 
