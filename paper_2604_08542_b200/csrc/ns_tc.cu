@@ -23,8 +23,8 @@
 // SS-mode MMAs with a 64-wide dimension are bound by the shared-memory operand port (128 B/clk),
 // which is why the hi/lo halves are stacked into 128-wide operands instead of issued as three
 // 64-wide products. Phases are sequential (each product depends on the previous one): one elected
-// thread issues the MMAs and commits to an mbarrier, all 16 warps run the TMEM -> registers ->
-// split -> shared epilogue (4 warps per TMEM lane quarter, 16 columns each).
+// thread of a dedicated warp issues the MMAs and commits to an mbarrier, 16 worker warps run the
+// TMEM -> registers -> split -> shared epilogue (4 warps per TMEM lane quarter, 16 columns each).
 #include <stdio.h>
 
 #include "tc_common.cuh"
@@ -43,7 +43,8 @@ extern "C" int ttt_debug_ns_trace(long long* host) {
 namespace ttt {
 
 namespace nstc {
-constexpr int THREADS = 512;
+constexpr int THREADS = 512;     // epilogue / load workers (16 warps)
+constexpr int LAUNCH_THREADS = THREADS + 32;   // + a dedicated MMA-issuing warp (warp 16)
 constexpr uint32_t C_A = 0;      // Gram accumulator   [128 x 128] fp32
 constexpr uint32_t C_A2 = 128;   // A A accumulator    [128 x 128] fp32
 constexpr uint32_t C_X = 0;      // X Pm accumulators, 128 columns per 128-row block (alias C_A, C_A2)
@@ -71,7 +72,7 @@ __device__ __forceinline__ uint32_t sw128_off(int row, int chunk) {
   return static_cast<uint32_t>(row * 128 + ((chunk ^ (row & 7)) << 4));
 }
 
-__global__ void __launch_bounds__(nstc::THREADS, 1)
+__global__ void __launch_bounds__(nstc::LAUNCH_THREADS, 1)
 ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, size_t set_elems,
              int use_G, int H, int iters, uint32_t tmem_cols, float* __restrict__ Wm,
              __nv_bfloat16* __restrict__ Wb) {
@@ -86,6 +87,7 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
   __shared__ float s_scale;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const bool issuer = warp == THREADS / 32;    // issues every MMA; takes part in the CTA barriers only
   const uint32_t x_bytes = static_cast<uint32_t>(H) * 128u;
   uint8_t* XH = smem;
   uint8_t* XL = XH + x_bytes;
@@ -106,7 +108,7 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
   const int n4 = H * HD / 4;
   constexpr int LB = 4;                            // float4 loads in flight per thread and set
   float acc = 0.f;
-  for (int e0 = tid; e0 < n4; e0 += THREADS * LB) {
+  for (int e0 = issuer ? n4 : tid; e0 < n4; e0 += THREADS * LB) {
     float4 g[LB];
 #pragma unroll
     for (int u = 0; u < LB; ++u) {
@@ -144,7 +146,7 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
   NS_TR(60);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-  if (lane == 0) red[warp] = acc;
+  if (lane == 0 && !issuer) red[warp] = acc;
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -157,7 +159,7 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
   __syncthreads();
   const float scale = s_scale;
   NS_TR(61);
-  for (int e0 = tid; e0 < n4; e0 += THREADS * LB) {   // same thread re-reads what it wrote
+  for (int e0 = issuer ? n4 : tid; e0 < n4; e0 += THREADS * LB) {   // same thread re-reads what it wrote
     float4 g[LB];
 #pragma unroll
     for (int u = 0; u < LB; ++u) {
@@ -203,55 +205,50 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
   uint32_t phase = 0;
   float Areg[8];
 
-  // sum of the four 64 x 64 blocks of a [128 x 128] accumulator -> 8 values (frow, 8 fch + j)
-  auto fold_blocks = [&](uint32_t col, float (&out)[8]) {
+  // sum of the four 64 x 64 blocks of a [128 x 128] accumulator -> 8 values (frow, 8 fch + j):
+  // part 1 (workers) column halves added, rows exported; CTA barrier; part 2 top + bottom rows
+  auto fold_export = [&](uint32_t col) {
     uint32_t r0[16], r1[16];
-    NS_TR(52);
     tmem_ld_x16(tb + lane_base + col + 16 * cs, r0);
     tmem_ld_x16(tb + lane_base + col + 64 + 16 * cs, r1);
     tc_wait_ld();
-    NS_TR(53);
     float* dst = S + trow * S_LD + 16 * cs;
 #pragma unroll
     for (int j = 0; j < 16; ++j) dst[j] = __uint_as_float(r0[j]) + __uint_as_float(r1[j]);
-    NS_TR(54);
-    __syncthreads();
-    NS_TR(55);
+  };
+  auto fold_import = [&](float (&out)[8]) {
     const float* top = S + frow * S_LD + 8 * fch;
     const float* bot = top + 64 * S_LD;
 #pragma unroll
     for (int j = 0; j < 8; ++j) out[j] = top[j] + bot[j];
   };
   auto end_phase = [&]() {
-    NS_TR(56);
     fence_proxy_async_smem();
-    NS_TR(57);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    NS_TR(58);
   };
   auto wait_mma = [&]() {
     mbar_wait(&mma_bar, phase & 1);
     phase ^= 1;
     tc_fence_after();
   };
+  const uint32_t lead = issuer ? elect_one() : 0u;
 
   for (int it = 0; it < iters; ++it) {
+    const bool last = it == iters - 1;
     // ---------------- A = X^T X ----------------
-    if (warp == 0) {
-      if (elect_one()) {
-        uint64_t d = d_x_mn;                                // +2048 B per 16-row K step
-        for (int ks = 0; ks < H / 16; ++ks, d += 128) umma_ss(tb + C_A, d, d, idesc_gram, ks > 0);
-        tc_commit(&mma_bar);
-      }
-      __syncwarp();
+    if (lead) {
+      uint64_t d = d_x_mn;                                  // +2048 B per 16-row K step
+      for (int ks = 0; ks < H / 16; ++ks, d += 128) umma_ss(tb + C_A, d, d, idesc_gram, ks > 0);
+      tc_commit(&mma_bar);
     }
     NS_TR(2 + it * 8);
-    wait_mma();
+    if (!issuer) { wait_mma(); fold_export(C_A); }
     NS_TR(3 + it * 8);
-    fold_blocks(C_A, Areg);
-    {
+    __syncthreads();
+    if (!issuer) {
+      fold_import(Areg);
       uint4 hi, lo;
       split8(Areg, hi, lo);
       *reinterpret_cast<uint4*>(AH + sw128_off(frow, fch)) = hi;
@@ -260,20 +257,18 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
     end_phase();
     NS_TR(4 + it * 8);
     // ---------------- Pm = a I + b A + c A A ----------------
-    if (warp == 0) {
-      if (elect_one()) {
+    if (lead) {
 #pragma unroll
-        for (int k = 0; k < HD / 16; ++k)                   // +32 B per 16-column K step
-          umma_ss(tb + C_A2, d_a + 2 * k, d_a + 2 * k, idesc_k128, k > 0);
-        tc_commit(&mma_bar);
-      }
-      __syncwarp();
+      for (int k = 0; k < HD / 16; ++k)                     // +32 B per 16-column K step
+        umma_ss(tb + C_A2, d_a + 2 * k, d_a + 2 * k, idesc_k128, k > 0);
+      tc_commit(&mma_bar);
     }
-    wait_mma();
+    if (!issuer) { wait_mma(); fold_export(C_A2); }
     NS_TR(5 + it * 8);
-    {
+    __syncthreads();
+    if (!issuer) {
       float pm[8];
-      fold_blocks(C_A2, pm);
+      fold_import(pm);
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
         float p = fmaf(cc, pm[j], cb * Areg[j]);
@@ -288,52 +283,50 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
     end_phase();
     NS_TR(6 + it * 8);
     // ---------------- X <- X Pm ----------------
-    if (warp == 0) {
-      if (elect_one()) {
-        for (int mb = 0; mb < nblk; ++mb) {
-          const uint32_t d = tb + C_X + 128 * mb;
-          const uint64_t a_h = d_xh_k + mb * 1024, a_l = d_xl_k + mb * 1024;   // 16 KB per 128-row block
+    if (lead) {
+      for (int mb = 0; mb < nblk; ++mb) {
+        const uint32_t d = tb + C_X + 128 * mb;
+        const uint64_t a_h = d_xh_k + mb * 1024, a_l = d_xl_k + mb * 1024;   // 16 KB per 128-row block
 #pragma unroll
-          for (int k = 0; k < HD / 16; ++k) {
-            umma_ss(d, a_h + 2 * k, d_p + 2 * k, idesc_k128, k > 0);   // [XH PH^T | XH PL^T]
-            umma_ss(d, a_l + 2 * k, d_p + 2 * k, idesc_k64, 1);        // left half += XL PH^T
-          }
+        for (int k = 0; k < HD / 16; ++k) {
+          umma_ss(d, a_h + 2 * k, d_p + 2 * k, idesc_k128, k > 0);   // [XH PH^T | XH PL^T]
+          umma_ss(d, a_l + 2 * k, d_p + 2 * k, idesc_k64, 1);        // left half += XL PH^T
         }
-        tc_commit(&mma_bar);
       }
-      __syncwarp();
+      tc_commit(&mma_bar);
     }
     NS_TR(7 + it * 8);
-    wait_mma();
-    NS_TR(8 + it * 8);
-    const bool last = it == iters - 1;
-    float* stage = reinterpret_cast<float*>(smem);            // last iteration: fp32 [H][W_LD]
-    for (int mb = 0; mb < nblk; ++mb) {
-      uint32_t r0[16], r1[16];
-      tmem_ld_x16(tb + lane_base + C_X + 128 * mb + 16 * cs, r0);
-      tmem_ld_x16(tb + lane_base + C_X + 128 * mb + 64 + 16 * cs, r1);
-      tc_wait_ld();
-      const int row = mb * 128 + trow;
-      float f[16];
+    if (!issuer) {
+      wait_mma();
+      float* stage = reinterpret_cast<float*>(smem);          // last iteration: fp32 [H][W_LD]
+      for (int mb = 0; mb < nblk; ++mb) {
+        uint32_t r0[16], r1[16];
+        tmem_ld_x16(tb + lane_base + C_X + 128 * mb + 16 * cs, r0);
+        tmem_ld_x16(tb + lane_base + C_X + 128 * mb + 64 + 16 * cs, r1);
+        tc_wait_ld();
+        const int row = mb * 128 + trow;
+        float f[16];
 #pragma unroll
-      for (int j = 0; j < 16; ++j) f[j] = __uint_as_float(r0[j]) + __uint_as_float(r1[j]);
-      if (!last) {
+        for (int j = 0; j < 16; ++j) f[j] = __uint_as_float(r0[j]) + __uint_as_float(r1[j]);
+        if (!last) {
 #pragma unroll
-        for (int k = 0; k < 2; ++k) {
-          const float v[8] = {f[8 * k], f[8 * k + 1], f[8 * k + 2], f[8 * k + 3],
-                              f[8 * k + 4], f[8 * k + 5], f[8 * k + 6], f[8 * k + 7]};
-          uint4 hi, lo;
-          split8(v, hi, lo);
-          *reinterpret_cast<uint4*>(XH + sw128_off(row, 2 * cs + k)) = hi;
-          *reinterpret_cast<uint4*>(XL + sw128_off(row, 2 * cs + k)) = lo;
+          for (int k = 0; k < 2; ++k) {
+            const float v[8] = {f[8 * k], f[8 * k + 1], f[8 * k + 2], f[8 * k + 3],
+                                f[8 * k + 4], f[8 * k + 5], f[8 * k + 6], f[8 * k + 7]};
+            uint4 hi, lo;
+            split8(v, hi, lo);
+            *reinterpret_cast<uint4*>(XH + sw128_off(row, 2 * cs + k)) = hi;
+            *reinterpret_cast<uint4*>(XL + sw128_off(row, 2 * cs + k)) = lo;
+          }
+        } else {
+          // all MMAs that read the operand tiles have completed: reuse them as the fp32 staging
+          float4* dst = reinterpret_cast<float4*>(stage + (size_t)row * W_LD + 16 * cs);
+#pragma unroll
+          for (int v = 0; v < 4; ++v) dst[v] = make_float4(f[4 * v], f[4 * v + 1], f[4 * v + 2], f[4 * v + 3]);
         }
-      } else {
-        // all MMAs that read the operand tiles have completed: reuse them as the fp32 staging
-        float4* dst = reinterpret_cast<float4*>(stage + (size_t)row * W_LD + 16 * cs);
-#pragma unroll
-        for (int v = 0; v < 4; ++v) dst[v] = make_float4(f[4 * v], f[4 * v + 1], f[4 * v + 2], f[4 * v + 3]);
       }
     }
+    NS_TR(8 + it * 8);
     end_phase();
     NS_TR(9 + it * 8);
   }
@@ -341,7 +334,7 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
   {
     const float* stage = reinterpret_cast<const float*>(smem);
     constexpr int WB = 4;
-    for (int e0 = tid; e0 < n4; e0 += THREADS * WB) {
+    for (int e0 = issuer ? n4 : tid; e0 < n4; e0 += THREADS * WB) {
       float4 w[WB];
 #pragma unroll
       for (int u = 0; u < WB; ++u) {
@@ -391,7 +384,7 @@ int launch_ns_tc(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s) {
     attr_smem = smem;
   }
   const uint32_t alloc = c.hidden <= 256 ? 256 : 512;
-  ns_tc_kernel<<<3 * c.nh, nstc::THREADS, smem, s>>>(ctx->G, ctx->partials, ctx->n_partials,
+  ns_tc_kernel<<<3 * c.nh, nstc::LAUNCH_THREADS, smem, s>>>(ctx->G, ctx->partials, ctx->n_partials,
                                                      3 * ctx->mat_elems, ctx->G_valid ? 1 : 0,
                                                      c.hidden, c.ns_iters, alloc,
                                                      fuse_commit ? ctx->Wm : nullptr,
