@@ -19,6 +19,14 @@
 #include "tc_common.cuh"
 #include "ttt_internal.h"
 
+#ifdef TTT_TRACE
+__device__ long long g_app_trace[16];
+extern "C" int ttt_debug_app_trace(long long* host) { return (int)cudaMemcpyFromSymbol(host, g_app_trace, sizeof(g_app_trace)); }
+#define APP_TR(k) do { if (blockIdx.x == 0 && blockIdx.y == 0) g_app_trace[k] = clock64(); } while (0)
+#else
+#define APP_TR(k) do { } while (0)
+#endif
+
 namespace ttt {
 
 int make_token_map(ttt_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int64_t cols,
@@ -47,11 +55,12 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   // 1024-B aligned base, computed on the 32-bit shared-space address (a uniform value)
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
-  __shared__ uint64_t w_full, fwd_full[NF], epi_done[NF], q_full[2], q_empty[2], o_full, o_empty;
+  __shared__ uint64_t w_full[8], fwd_full[NF], epi_done[NF], q_full[2], q_empty[2], o_full, o_empty;
   __shared__ uint64_t qr_full[QST], qr_empty[QST];
   __shared__ uint32_t tmem_base_s;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  if (tid == 0) APP_TR(0);
   const int h = blockIdx.y;
   const int nsl = H / NS;                                    // steps per tile
   // tiles of this CTA: blockIdx.x, blockIdx.x + gridDim.x, ...
@@ -62,7 +71,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   uint8_t* o_stage = q_ring + QST * TILE_BYTES;              // 2 x 16 KB
 
   if (tid == 0) {
-    mbar_init(&w_full, 1);
+    for (int n = 0; n < 8; ++n) mbar_init(&w_full[n], 1);
     for (int b = 0; b < NF; ++b) { mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 8); }
     for (int b = 0; b < 2; ++b) { mbar_init(&q_full[b], 128); mbar_init(&q_empty[b], 1); }
     mbar_init(&o_full, 1);
@@ -76,7 +85,9 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   tc_fence_after();
   // programmatic dependent launch: everything above overlapped the tail of the preceding kernel
   // (the commit that produces the weights); nothing below may run before it has completed
+  if (tid == 0) APP_TR(1);
   asm volatile("griddepcontrol.wait;" ::: "memory");
+  if (tid == 0) APP_TR(2);
   const uint32_t tb = tmem_base_s;
   if (tb != 0) __trap();      // all 512 columns belong to this CTA: the issuer uses absolute columns
 
@@ -85,16 +96,24 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
     if (elect_one() && my_tiles > 0) {
       tma_prefetch_desc(&mapW);
       tma_prefetch_desc(&mapQ);
-      mbar_arrive_expect_tx(&w_full, w_bytes);
+      // first Q tiles first (they feed the I/O warpgroup's shared -> TMEM copy), then the weights step
+      // by step, each step on its own barrier so the MMAs start when step 0 has landed
+      const int npre = min(my_tiles, QST);
+      for (int tl = 0; tl < npre; ++tl) {
+        mbar_arrive_expect_tx(&qr_full[tl], TILE_BYTES);
+        tma_load_2d_hint(q_ring + tl * TILE_BYTES, &mapQ, &qr_full[tl], h * HD,
+                         ((int)blockIdx.x + tl * (int)gridDim.x) * TM, kEvictFirst);
+      }
       // smem, boxes of 64 rows (8 KB): per 64-hidden step n [W1^T rows | W3^T rows] back to back
       // (one 128-row K-major B operand), then the W2 row blocks
       for (int n = 0; n < nsl; ++n) {
-        tma_load_2d_hint(smem + (size_t)n * 16384, &mapW, &w_full, 0, (0 * nh + h) * H + 64 * n, kEvictLast);
-        tma_load_2d_hint(smem + (size_t)n * 16384 + 8192, &mapW, &w_full, 0, (2 * nh + h) * H + 64 * n, kEvictLast);
-        tma_load_2d_hint(smem + (size_t)nsl * 16384 + (size_t)n * 8192, &mapW, &w_full, 0,
+        mbar_arrive_expect_tx(&w_full[n], 3u * 8192u);
+        tma_load_2d_hint(smem + (size_t)n * 16384, &mapW, &w_full[n], 0, (0 * nh + h) * H + 64 * n, kEvictLast);
+        tma_load_2d_hint(smem + (size_t)n * 16384 + 8192, &mapW, &w_full[n], 0, (2 * nh + h) * H + 64 * n, kEvictLast);
+        tma_load_2d_hint(smem + (size_t)nsl * 16384 + (size_t)n * 8192, &mapW, &w_full[n], 0,
                          (1 * nh + h) * H + 64 * n, kEvictLast);
       }
-      for (int tl = 0; tl < my_tiles; ++tl) {
+      for (int tl = npre; tl < my_tiles; ++tl) {
         const int rs = tl % QST, it = tl / QST;
         mbar_wait(&qr_empty[rs], (it & 1) ^ 1);
         mbar_arrive_expect_tx(&qr_full[rs], TILE_BYTES);
@@ -112,8 +131,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       constexpr uint32_t idesc_d = umma_idesc_bf16(TM, HD, 0, 1);      // B = W2 rows, MN-major
       const uint64_t d13 = umma_smem_desc_sw128(sbase, 16, 1024);
       const uint64_t d2 = umma_smem_desc_sw128(sbase + nsl * 16384, 8192, 1024);
-      mbar_wait(&w_full, 0);
-      tc_fence_after();
+      APP_TR(3);
       // forward of step st+1 is issued before the down projection of step st
       int f_tl = 0, f_n = 0;     // (tile, step) of the next forward
       int d_tl = 0, d_n = 0;     // (tile, step) of the next down projection
@@ -122,6 +140,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       auto fwd = [&]() {
         const int qb = f_tl & 1;
         if (f_n == 0) { mbar_wait(&q_full[qb], (f_tl >> 1) & 1); tc_fence_after(); }
+        if (f_tl == 0) { mbar_wait(&w_full[f_n], 0); tc_fence_after(); }     // this step's weights have landed
         const uint32_t acc = C_F + f_fb * 128, qop = C_Q + qb * 32;
         const uint64_t b = d13 + (uint64_t)f_n * 1024;                 // 16 KB per step
 #pragma unroll
@@ -146,11 +165,14 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       // the forward MMAs run two steps ahead of the down projection: one buffer per warpgroup in
       // the epilogue, the third being filled
       fwd();
+      APP_TR(4);
       if (total_steps > 1) fwd();
       for (int st = 0; st < total_steps; ++st) {
         if (st + 2 < total_steps) fwd();
         down();
+        if (st == 0) APP_TR(5);
       }
+      APP_TR(6);
     }
   } else if (warp >= 4 && warp < IO_WARP0) {
     // ===================== SwiGLU epilogue warpgroups =====================
@@ -253,7 +275,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       store_o(tl);
       if (tl + 2 < my_tiles) load_q(tl + 2);
     }
-    if (tid == IO_WARP0 * 32) tma_store_wait<0>();
+    if (tid == IO_WARP0 * 32) { APP_TR(7); tma_store_wait<0>(); APP_TR(8); }
   }
   tc_fence_before();
   __syncthreads();
