@@ -324,3 +324,32 @@ def test_cfg4_full_size_first_chunks_sampled_head():
     (the float64 oracle needs ~3 s per head and chunk at this size)."""
     errs, errs_w = _full_size_stream("cfg4", 2, [3])
     assert max(errs) <= TOL_BF16 and max(errs_w) <= TOL_BF16, (errs, errs_w)
+
+
+@pytest.mark.parametrize("M", [1, 5, 33, 130])
+def test_bf16_tiny_chunks_strided_rows_and_nonuniform_lr(M):
+    """Edge cases of the tensor path: chunks smaller than one update tile (32) / apply tile (128),
+    token rows with padding (ld > nh*hd), per-token learning rates of both signs and zero."""
+    from paper_2604_08542_b200 import TTT, TTT_BF16
+    dev = torch.device("cuda", 0)
+    nh, hd, H, ld = 2, 64, 128, 2 * 64 + 24
+    g = torch.Generator().manual_seed(100 + M)
+    W1 = torch.randn(nh, hd, H, generator=g) / 8
+    W2 = torch.randn(nh, H, hd, generator=g) / 8
+    W3 = torch.randn(nh, hd, H, generator=g) / 8
+    buf = [torch.randn(M, ld, generator=g).to(torch.bfloat16) for _ in range(3)]
+    Q, K, V = (b[:, :nh * hd] for b in buf)                     # views with row stride ld
+    lr = (torch.rand(nh, M, generator=g) - 0.3) * 0.05
+    lr[:, ::3] = 0.0
+    t = TTT(nh, hd, H, TTT_BF16, max_tokens=256)
+    t.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    dQ, dK, dV = (b.to(dev)[:, :nh * hd] for b in buf)
+    assert dQ.stride(0) == ld
+    loss = torch.zeros(nh, device=dev)
+    O = t.ttt_chunk_step(dQ, dK, dV, lr.to(dev), loss=loss)
+    ora = OracleTTT(W1, W2, W3)
+    O_ref, loss_ref = ora.chunk_step(Q.contiguous(), K.contiguous(), V.contiguous(), lr)
+    assert rel_err(O.float().cpu(), O_ref) <= TOL_BF16
+    assert max(rel_err(a.cpu(), b) for a, b in zip(t.ttt_get_weights(), ora.weights())) <= TOL_BF16
+    assert rel_err(loss.cpu(), loss_ref) <= TOL_LOSS_BF16
+    t.close()
