@@ -100,6 +100,8 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
   NS_TR(0);
   if (tid == 0) { mbar_init(&mma_bar, 1); fence_mbar_init(); }
   if (warp == 0) { tmem_alloc(&tmem_base_s, tmem_cols); tmem_relinquish(); }
+  // programmatic dependent launch: the set-up above overlapped the tail of the gradient kernel
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   NS_TR(59);
 
   // ---- load: g = (use_G ? G : 0) + sum_s P[s] (fixed order), written back to G; Frobenius norm ----
@@ -330,6 +332,7 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
     end_phase();
     NS_TR(9 + it * 8);
   }
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   // ---- coalesced write-out: fused commit W <- W - NS(g) (Eq. 8) or NS(g) -> G ----
   {
     const float* stage = reinterpret_cast<const float*>(smem);
@@ -384,11 +387,24 @@ int launch_ns_tc(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s) {
     attr_smem = smem;
   }
   const uint32_t alloc = c.hidden <= 256 ? 256 : 512;
-  ns_tc_kernel<<<3 * c.nh, nstc::LAUNCH_THREADS, smem, s>>>(ctx->G, ctx->partials, ctx->n_partials,
-                                                     3 * ctx->mat_elems, ctx->G_valid ? 1 : 0,
-                                                     c.hidden, c.ns_iters, alloc,
-                                                     fuse_commit ? ctx->Wm : nullptr,
-                                                     fuse_commit ? ctx->Wb : nullptr);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(3 * c.nh);
+  cfg.blockDim = dim3(nstc::LAUNCH_THREADS);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  float* G = ctx->G;
+  const float* P = ctx->partials;
+  int n_sets = ctx->n_partials, use_G = ctx->G_valid ? 1 : 0, H = c.hidden, iters = c.ns_iters;
+  size_t set_elems = 3 * ctx->mat_elems;
+  float* Wm = fuse_commit ? ctx->Wm : nullptr;
+  __nv_bfloat16* Wb = fuse_commit ? ctx->Wb : nullptr;
+  cudaError_t e = cudaLaunchKernelEx(&cfg, ns_tc_kernel, G, P, n_sets, set_elems, use_G, H, iters, alloc, Wm, Wb);
+  if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, "ns_tc_kernel launch", e);
   TTT_LAUNCH_CHECK(ctx, "ns_tc_kernel");
   ctx->G_valid = !fuse_commit;
   ctx->n_partials = 0;
