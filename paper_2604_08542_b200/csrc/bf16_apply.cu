@@ -35,8 +35,9 @@ int make_token_map(ttt_ctx* ctx, CUtensorMap* map, const void* base, int64_t row
 namespace app {
 constexpr int TM = 128;        // tokens per tile (MMA M)
 constexpr int NS = 64;         // hidden units per step
-constexpr int THREADS = 768;    // 4 control warps, 16 epilogue warps, 4 I/O warps
-constexpr int IO_WARP0 = 20;
+constexpr int THREADS = 896;    // 4 control warps, 16 epilogue warps, 4 O-store warps, 4 Q-load warps
+constexpr int IO_WARP0 = 20;    // O: TMEM -> shared -> TMA store
+constexpr int QL_WARP0 = 24;    // Q: shared -> TMEM (A operand)
 constexpr int QST = 4;         // Q tile ring stages
 constexpr int TILE_BYTES = TM * 128;   // one [128 x 64] bf16 tile
 // TMEM column plan for hd = 64
@@ -269,13 +270,14 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
         tma_store_commit();
       }
     };
-    if (my_tiles > 0) load_q(0);
-    if (my_tiles > 1) load_q(1);
-    for (int tl = 0; tl < my_tiles; ++tl) {
-      store_o(tl);
-      if (tl + 2 < my_tiles) load_q(tl + 2);
+    // separate warpgroups for the two directions: the Q copy of tile tl+2 and the O drain of tile
+    // tl are both on the issuer's critical path (Q operand double-buffered, O accumulator single)
+    if (warp >= QL_WARP0) {
+      for (int tl = 0; tl < my_tiles; ++tl) load_q(tl);
+    } else {
+      for (int tl = 0; tl < my_tiles; ++tl) store_o(tl);
+      if (tid == IO_WARP0 * 32) { APP_TR(7); tma_store_wait<0>(); APP_TR(8); }
     }
-    if (tid == IO_WARP0 * 32) { APP_TR(7); tma_store_wait<0>(); APP_TR(8); }
   }
   tc_fence_before();
   __syncthreads();
