@@ -100,11 +100,12 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       // first Q tiles first (they feed the I/O warpgroup's shared -> TMEM copy), then the weights step
       // by step, each step on its own barrier so the MMAs start when step 0 has landed
       const int npre = min(my_tiles, QST);
-      for (int tl = 0; tl < npre; ++tl) {
+      auto q_load = [&](int tl) {
         mbar_arrive_expect_tx(&qr_full[tl], TILE_BYTES);
         tma_load_2d_hint(q_ring + tl * TILE_BYTES, &mapQ, &qr_full[tl], h * HD,
                          ((int)blockIdx.x + tl * (int)gridDim.x) * TM, kEvictFirst);
-      }
+      };
+      q_load(0);               // what the first MMAs need goes first: Q tile 0, then the weights in step order
       // smem, boxes of 64 rows (8 KB): per 64-hidden step n [W1^T rows | W3^T rows] back to back
       // (one 128-row K-major B operand), then the W2 row blocks
       for (int n = 0; n < nsl; ++n) {
@@ -114,6 +115,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
         tma_load_2d_hint(smem + (size_t)nsl * 16384 + (size_t)n * 8192, &mapW, &w_full[n], 0,
                          (1 * nh + h) * H + 64 * n, kEvictLast);
       }
+      for (int tl = 1; tl < npre; ++tl) q_load(tl);
       for (int tl = npre; tl < my_tiles; ++tl) {
         const int rs = tl % QST, it = tl / QST;
         mbar_wait(&qr_empty[rs], (it & 1) ^ 1);
