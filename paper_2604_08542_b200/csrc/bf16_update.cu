@@ -28,9 +28,12 @@
 // soon as an epilogue group has pulled it into registers; the bf16 gradient operands have their own
 // (single) columns, so nothing aliases; forward and gradient MMAs are issued by different warps —
 // the MMAs of tiles i+1, i+2 overlap the epilogue math of tile i.
-// Measured budget per 32-token tile and SM (B200 microbenchmarks): MMA 546 clk (12 x
-// N=32 at 25 clk + 6 x N=64 at 41 clk: ~9 clk fixed cost per tcgen05.mma), epilogue math ~390 clk
-// (MUFU 16/clk: 256; FP32 pipe 128 lanes/clk: 8 ops per element; F2FP packs).
+// Measured budget per 32-token tile and SM (B200 microbenchmarks): tensor pipe 384 clk
+// when the twelve N=32 and six N=64 MMAs are issued back to back (nominal rate), epilogue math
+// ~390 clk (MUFU 16/clk: 256; FP32 pipe 128 lanes/clk: 10 ops per element; F2FP packs). The kernel
+// runs at ~786 clk per tile: the forward-issuing thread's own instruction stream (~100 dependent
+// scalar instructions per tile around the twelve MMAs) plus the single-buffered g hand-off are the
+// critical path — variants that split or re-home that stream measured slower.
 #include <stdio.h>
 
 #include "tc_common.cuh"
