@@ -244,7 +244,7 @@ def run_ours(args, w, rank, local_rank, world):
     step_tflops = flops_per_chunk(w, M, "step") / (ms_per_step * 1e-3) / 1e12
     # dram__bytes_read.sum + dram__bytes_write.sum of bf16_update_kernel, one launch, from the
     # `ncu --set full` captures summarised in profiles/r01b_ncu_full.md (None = not captured)
-    traffic = {"cfg2": 48123136 + 486912, "cfg4": 184645632 + 3801600}.get(w.name)
+    traffic = {"cfg2": 48133632 + 442880, "cfg4": 187704320 + 6952704}.get(w.name)
     # (the per-kernel pass calls ttt_accumulate / ttt_commit / ttt_apply separately; inside
     #  ttt_chunk_step the plain commit is fused into the update kernel's tail)
     roofline = {"kernel": "bf16_update_kernel" if w.act_dtype == "bf16" else "f32 path",
