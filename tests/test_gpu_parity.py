@@ -353,3 +353,32 @@ def test_bf16_tiny_chunks_strided_rows_and_nonuniform_lr(M):
     assert max(rel_err(a.cpu(), b) for a, b in zip(t.ttt_get_weights(), ora.weights())) <= TOL_BF16
     assert rel_err(loss.cpu(), loss_ref) <= TOL_LOSS_BF16
     t.close()
+
+
+def test_long_stream_is_stable_and_per_chunk_time_is_flat():
+    """Table 5: runtime grows linearly with sequence length, throughput stays flat.
+    For the path this means: per-chunk time does not depend on the chunk index, and the re-normalised
+    recurrence of the long driving-like config (cfg4 flags: L2-K, renorm, rho 0.95) stays finite over
+    all 63 chunks (cut-down tokens per frame so the test runs in seconds)."""
+    dev = torch.device("cuda", 0)
+    w = _bf16_workload("cfg4", tokens_per_frame=64)            # 63 chunks x 2048 tokens, last chunk 1024
+    W1, W2, W3 = (x.to(dev) for x in ti.fast_weights(w))
+    chunks = [tuple(x.to(dev) for x in c) for c in ti.TokenStream(w)]
+    assert len(chunks) == 63 and chunks[-1][0].shape[0] == 16 * 64
+    g = _mk(w)
+    g.ttt_init(W1, W2, W3)
+    for (Q, K, V, lr) in chunks[:3]:                            # warm-up
+        g.ttt_chunk_step(Q, K, V, lr)
+    g.ttt_init(W1, W2, W3)
+    evs = []
+    outs = []
+    for (Q, K, V, lr) in chunks:
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); outs.append(g.ttt_chunk_step(Q, K, V, lr)); b.record()
+        evs.append((a, b))
+    torch.cuda.synchronize()
+    t = np.array([a.elapsed_time(b) for a, b in evs[:-1]])      # full-size chunks only
+    assert all(bool(torch.isfinite(o.float()).all()) for o in outs)
+    assert all(bool(torch.isfinite(x).all()) for x in g.ttt_get_weights())
+    assert np.median(t[40:]) <= 1.25 * np.median(t[:20]), (np.median(t[:20]), np.median(t[40:]))
+    g.close()
