@@ -583,8 +583,11 @@ int bf16_partials_needed(const ttt_ctx* ctx, int64_t M) {
   return s;
 }
 
-int bf16_tensor_path(const ttt_config* cfg) {
+int bf16_apply_tensor_path(const ttt_config* cfg) {
   return cfg->hd == 64 && (cfg->hidden == 128 || cfg->hidden == 256) && !cfg->linear_fast_weight;
+}
+int bf16_update_tensor_path(const ttt_config* cfg) {
+  return bf16_apply_tensor_path(cfg) || bf16_update_wide_supported(cfg);
 }
 
 // bf16 token tensors are accepted for every shape the fp32 path takes; shapes outside the tcgen05
@@ -602,6 +605,13 @@ int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V
   const ttt_config& c = ctx->cfg;
   int tiles, tps, splits;
   update_split(ctx, M, &tiles, &tps, &splits);
+  if (c.hd == 128) {                     // hd = 128: weights in shared memory, no fused commit
+    int rc = bf16_accumulate_wide(ctx, K, V, lr, M, ld, want_loss, tiles, tps, splits, s);
+    if (rc != TTT_OK) return rc;
+    *used = splits;
+    *loss_rows = splits * (c.hidden / upd::HS);
+    return TTT_OK;
+  }
   CUtensorMap mapK, mapV;
   int rc = make_token_map(ctx, &mapK, K, M, (int64_t)c.nh * c.hd, ld, upd::T);
   if (rc != TTT_OK) return rc;

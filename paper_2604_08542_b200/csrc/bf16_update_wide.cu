@@ -1,0 +1,349 @@
+// bf16_update_wide.cu — fused fast-weight gradient kernel for head dimension 128 (tcgen05 / TMEM / TMA).
+//
+// Same computation as bf16_update.cu (Eq. 11-13: forward through the SwiGLU fast weights on
+// the chunk's keys, gradient of the dot-product loss w.r.t. W1, W2, W3 with the per-token learning
+// rate folded in), same orientation (hidden units on the 128 TMEM lanes, tokens on the MMA N / K
+// axis), for hd = 128, where the TMEM budget is different: the three fp32 gradient accumulators of a
+// 128-hidden slice take 3 x 128 = 384 of the 512 columns, so
+//   * the weights stay in shared memory (A operands of SS-mode MMAs, 96 KB per slice),
+//   * the forward accumulators x | b | g of one 32-token tile are single-buffered (96 columns),
+//   * the bf16 operand Hd' of the W2 gradient re-uses the columns of x; the MMA order
+//     b(i+1), g(i+1), gradients(i), x(i+1) keeps the tensor pipe busy while the epilogue of tile i runs
+//     and makes the overwrite of x safe (MMAs of one thread execute in issue order).
+// One CTA = (token split, 128-hidden slice, head); its partial gradients go to one partial set per
+// split, summed in split order by the commit (deterministic, no float atomics).
+#include <stdio.h>
+
+#include "tc_common.cuh"
+#include "ttt_internal.h"
+
+namespace ttt {
+
+int make_token_map(ttt_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int64_t cols,
+                   int64_t ld, int box_rows);   // bf16_update.cu
+
+namespace updw {
+constexpr int HS = 128;        // hidden units per CTA (MMA M)
+constexpr int HD = 128;        // head dimension (forward MMA K, gradient MMA N)
+constexpr int T = 32;          // tokens per tile (forward MMA N, gradient MMA K)
+constexpr int STAGES = 6;      // K/V shared-memory ring
+constexpr int EPI_WARPS = 8;
+constexpr int THREADS = (4 + EPI_WARPS) * 32;
+constexpr int SUB_BYTES = T * 128;          // one [T x 64] bf16 sub-tile (half of hd), 128-B swizzled
+constexpr int TILE_BYTES = 2 * SUB_BYTES;   // K or V tile
+constexpr int STAGE_BYTES = 2 * TILE_BYTES;
+constexpr int WSUB_BYTES = HS * 128;        // one [128 x 64] bf16 weight sub-tile
+constexpr int WMAT_BYTES = 2 * WSUB_BYTES;
+constexpr int W_BYTES = 3 * WMAT_BYTES;
+constexpr size_t SMEM_BYTES = (size_t)W_BYTES + (size_t)STAGES * STAGE_BYTES + 1024;
+
+// TMEM column plan (512 columns x 128 lanes x 32 bit)
+constexpr uint32_t C_G1 = 0, C_G3 = 128, C_G2 = 256;   // fp32 gradient accumulators [hidden][hd]
+constexpr uint32_t C_X = 384, C_B = 416, C_G = 448;    // fp32 forward accumulators [hidden][token]
+constexpr uint32_t C_OA = 480, C_OB = 496;             // bf16 operands 2 dA, dB [hidden][token], 16 cols
+constexpr uint32_t C_OH = C_X;                         // bf16 operand Hd' = -eta Hd, over the dead x
+}  // namespace updw
+
+template <bool LOSS>
+__global__ void __launch_bounds__(updw::THREADS, 1)
+bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
+                        const __grid_constant__ CUtensorMap mapW, const float* __restrict__ lr,
+                        float* __restrict__ P, float* __restrict__ loss_part, int M, int nh, int H,
+                        int tiles_total, int tiles_per_split) {
+  using namespace updw;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
+  uint8_t* ring = smem + W_BYTES;
+  __shared__ uint64_t full[STAGES], empty[STAGES], w_full, fwd_full, xbg_free, opnd_ready, grad_done;
+  __shared__ uint32_t tmem_base_s;
+  __shared__ float loss_red[EPI_WARPS];
+  __shared__ __align__(16) float ne_s[STAGES][T];   // -eta of the stage's tokens (0 beyond M)
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int split = blockIdx.x, slice = blockIdx.y, h = blockIdx.z;
+  const int nslices = gridDim.y;
+  const int tile_lo = split * tiles_per_split;
+  const int ntiles = min(tiles_per_split, tiles_total - tile_lo);
+
+  auto load_stage = [&](int s, int tile) {
+    mbar_arrive_expect_tx(&full[s], STAGE_BYTES);
+    uint8_t* dst = ring + s * STAGE_BYTES;
+    const int row = tile * T;
+    tma_load_2d(dst, &mapK, &full[s], h * HD, row);
+    tma_load_2d(dst + SUB_BYTES, &mapK, &full[s], h * HD + 64, row);
+    tma_load_2d(dst + TILE_BYTES, &mapV, &full[s], h * HD, row);
+    tma_load_2d(dst + TILE_BYTES + SUB_BYTES, &mapV, &full[s], h * HD + 64, row);
+  };
+
+  if (tid == 0) {
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 2); mbar_init(&empty[s], 1); }
+    mbar_init(&w_full, 1);
+    mbar_init(&fwd_full, 1);
+    mbar_init(&xbg_free, 1);
+    mbar_init(&opnd_ready, EPI_WARPS);
+    mbar_init(&grad_done, 1);
+    fence_mbar_init();
+    tma_prefetch_desc(&mapK);
+    tma_prefetch_desc(&mapV);
+    tma_prefetch_desc(&mapW);
+    // weights of the slice: mat m (0 = W1^T, 1 = W2, 2 = W3^T), hd half c -> [128 rows x 64] sub-tile
+    mbar_arrive_expect_tx(&w_full, W_BYTES);
+    for (int m = 0; m < 3; ++m)
+      for (int c = 0; c < 2; ++c)
+        tma_load_2d(smem + m * WMAT_BYTES + c * WSUB_BYTES, &mapW, &w_full, c * 64,
+                    (m * nh + h) * H + slice * HS);
+    const int npre = min(ntiles, STAGES);
+    for (int i = 0; i < npre; ++i) load_stage(i, tile_lo + i);
+  }
+  __syncwarp();
+  constexpr int LRPF = 4;
+  float lr_pre[LRPF];
+  if (warp == 2) {
+#pragma unroll
+    for (int u = 0; u < LRPF; ++u) {
+      const int t = (tile_lo + u) * T + lane;
+      lr_pre[u] = (u < ntiles && t < M) ? -__ldg(lr + (size_t)h * M + t) : 0.f;
+    }
+  }
+  if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tb = tmem_base_s;
+  if (tb != 0) __trap();      // all 512 columns belong to this CTA: the issuer uses absolute columns
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (elect_one()) {
+      for (int i = STAGES; i < ntiles; ++i) {        // tiles 0 .. STAGES-1 were requested in the prologue
+        const int s = i % STAGES, it = i / STAGES;
+        mbar_wait(&empty[s], (it & 1) ^ 1);
+        load_stage(s, tile_lo + i);
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer (forward and gradients) =====================
+    if (elect_one()) {
+      constexpr uint32_t idesc_f = umma_idesc_bf16(HS, T, 0, 0);    // A = weights, B = token tile, K-major
+      constexpr uint32_t idesc_g = umma_idesc_bf16(HS, HD, 0, 1);   // A = TMEM operand, B = token tile, MN-major
+      const uint64_t dw = umma_smem_desc_sw128(sbase, 16, 1024);
+      const uint64_t dr_k = umma_smem_desc_sw128(sbase + W_BYTES, 16, 1024);
+      const uint64_t dr_mn = umma_smem_desc_sw128(sbase + W_BYTES, SUB_BYTES, 1024);   // 2nd hd atom: +SUB_BYTES
+      // forward product of weight matrix m with the K (tile_off 0) or V tile of stage offset st
+      auto forward = [&](int m, uint64_t st, uint32_t dcol) {
+#pragma unroll
+        for (int k = 0; k < HD / 16; ++k) {
+          const uint64_t a = dw + (uint64_t)(m * (WMAT_BYTES >> 4) + (k >> 2) * (WSUB_BYTES >> 4) + (k & 3) * 2);
+          const uint64_t b = dr_k + st + (uint64_t)((k >> 2) * (SUB_BYTES >> 4) + (k & 3) * 2);
+          umma_ss(dcol, a, b, idesc_f, k > 0);
+        }
+      };
+      auto gradients = [&](uint64_t st, uint32_t acc) {
+#pragma unroll
+        for (int k = 0; k < T / 16; ++k) {                   // +2048 B per 16-token K step
+          umma_ts(C_G1, C_OA + 8 * k, dr_mn + st + 128 * k, idesc_g, acc | k);
+          umma_ts(C_G3, C_OB + 8 * k, dr_mn + st + 128 * k, idesc_g, acc | k);
+          umma_ts(C_G2, C_OH + 8 * k, dr_mn + st + (TILE_BYTES >> 4) + 128 * k, idesc_g, acc | k);
+        }
+      };
+      mbar_wait(&w_full, 0);
+      uint64_t st_prev = 0;
+      int s_prev = 0;
+      for (int i = 0; i < ntiles; ++i) {
+        const int s = i % STAGES;
+        const uint64_t st = (uint64_t)s * (STAGE_BYTES >> 4);
+        mbar_wait(&full[s], (i / STAGES) & 1);
+        if (i > 0) mbar_wait(&xbg_free, (i - 1) & 1);          // x | b | g of tile i-1 are in registers
+        tc_fence_after();
+        forward(2, st, C_B);
+        forward(1, st + (TILE_BYTES >> 4), C_G);
+        if (i > 0) {
+          mbar_wait(&opnd_ready, (i - 1) & 1);
+          tc_fence_after();
+          gradients(st_prev, i > 1);
+          tc_commit(&empty[s_prev]);
+        }
+        forward(0, st, C_X);           // after the gradient MMAs that read Hd' from these columns
+        tc_commit(&fwd_full);
+        st_prev = st;
+        s_prev = s;
+      }
+      if (ntiles > 0) {
+        mbar_wait(&opnd_ready, (ntiles - 1) & 1);
+        tc_fence_after();
+        gradients(st_prev, ntiles > 1);
+      }
+      tc_commit(&grad_done);
+    }
+  } else if (warp == 2) {
+    // ===================== learning-rate loader =====================
+    const float* lrh = lr + (size_t)h * M;
+    auto ld_batch = [&](int i0, float (&v)[LRPF]) {
+#pragma unroll
+      for (int u = 0; u < LRPF; ++u) {
+        const int t = (tile_lo + i0 + u) * T + lane;
+        v[u] = (i0 + u < ntiles && t < M) ? -__ldg(lrh + t) : 0.f;
+      }
+    };
+    float cur[LRPF], nxt[LRPF];
+#pragma unroll
+    for (int u = 0; u < LRPF; ++u) cur[u] = lr_pre[u];
+    for (int i0 = 0; i0 < ntiles; i0 += LRPF) {
+      ld_batch(i0 + LRPF, nxt);
+#pragma unroll
+      for (int u = 0; u < LRPF; ++u) {
+        const int i = i0 + u;
+        if (i < ntiles) {
+          const int s = i % STAGES, it = i / STAGES;
+          if (it > 0) mbar_wait(&empty[s], (it & 1) ^ 1);
+          ne_s[s][lane] = cur[u];
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&full[s]);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < LRPF; ++u) cur[u] = nxt[u];
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue warps =====================
+    const int ew = warp - 4, q = warp & 3, kh = ew >> 2;   // lane quadrant, K step (16 tokens) of the tile
+    const int j = q * 32 + lane;                           // hidden unit within the slice = TMEM lane
+    const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
+    uint64_t loss2 = 0ull;
+    const uint64_t ONE2 = pack2(1.0f, 1.0f), NONE2 = pack2(-1.0f, -1.0f), HALF2 = pack2(0.5f, 0.5f);
+    for (int i = 0; i < ntiles; ++i) {
+      const int s = i % STAGES;
+      mbar_wait(&fwd_full, i & 1);
+      mbar_wait(&full[s], (i / STAGES) & 1);               // acquire of the loader's -eta slot
+      tc_fence_after();
+      const uint2* nes = reinterpret_cast<const uint2*>(&ne_s[s][16 * kh]);
+      uint32_t rx[16], rb[16], rg[16];
+      tmem_ld_x16(lane_base + C_X + 16 * kh, rx);
+      tmem_ld_x16(lane_base + C_B + 16 * kh, rb);
+      tmem_ld_x16(lane_base + C_G + 16 * kh, rg);
+      tc_wait_ld();
+      tc_fence_before();
+      asm volatile("bar.sync 1, 256;" ::: "memory");       // every warp holds its x | b | g
+      if (ew == 0 && lane == 0) mbar_arrive(&xbg_free);
+      uint32_t pa[8], pb[8], ph[8];
+#pragma unroll
+      for (int c = 0; c < 16; c += 2) {
+        const uint64_t x = fmul2(pack2u(rx[c], rx[c + 1]), HALF2);   // a / 2
+        const uint64_t bb = pack2u(rb[c], rb[c + 1]);
+        const uint2 nev = nes[c >> 1];
+        const uint64_t ne = pack2u(nev.x, nev.y);
+        const uint64_t g = fmul2(ne, pack2u(rg[c], rg[c + 1]));   // dHd = (-eta v) W2^T
+        float x0, x1;
+        unpack2(x, x0, x1);
+        const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
+        const uint64_t S = ffma2(x, th, x);                  // SiLU(a) = a sigmoid(a), a = 2 x
+        const uint64_t p = fadd2(th, ONE2);                  // 2 sigmoid(a)
+        const uint64_t m = ffma2(th, NONE2, ONE2);           // 2 (1 - sigmoid(a))
+        const uint64_t t2 = ffma2(S, m, p);                  // 2 SiLU'(a)
+        const uint64_t hdv = fmul2(S, bb);                   // hidden activation Hd
+        pa[c >> 1] = pack_bf16x2_from2(fmul2(fmul2(g, bb), t2));   // 2 dA
+        pb[c >> 1] = pack_bf16x2_from2(fmul2(g, S));               // dB
+        ph[c >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));            // Hd' = -eta Hd
+        if (LOSS) loss2 = ffma2(hdv, g, loss2);
+      }
+      // the gradient MMAs of tile i-1 (the last readers of these columns) were issued before the x
+      // MMAs of tile i and are covered by the same commit: they have completed
+      tmem_st_x8(lane_base + C_OA + 8 * kh, pa);
+      tmem_st_x8(lane_base + C_OB + 8 * kh, pb);
+      tmem_st_x8(lane_base + C_OH + 8 * kh, ph);
+      tc_wait_st();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&opnd_ready);
+    }
+    // ---- flush the gradient accumulators: one fp32 partial slice per CTA ----
+    mbar_wait(&grad_done, 0);
+    tc_fence_after();
+    const size_t me = (size_t)nh * H * HD;
+    const size_t row = ((size_t)h * H + (size_t)slice * HS + j) * HD;
+    float* Pset = P + (size_t)split * 3 * me;
+    const uint32_t gcol[3] = {C_G1, C_G2, C_G3};
+#pragma unroll
+    for (int mat = 0; mat < 3; ++mat) {                    // this warp: columns 64 kh .. 64 kh + 63
+      const float sc = mat == 0 ? 0.5f : 1.0f;             // G1 was accumulated from 2 dA
+#pragma unroll
+      for (int cc = 0; cc < 4; ++cc) {
+        uint32_t r[16];
+        if (ntiles > 0) {
+          tmem_ld_x16(lane_base + gcol[mat] + 64 * kh + 16 * cc, r);
+          tc_wait_ld();
+        } else {
+#pragma unroll
+          for (int u = 0; u < 16; ++u) r[u] = 0u;
+        }
+        float4* dst = reinterpret_cast<float4*>(Pset + mat * me + row + 64 * kh + 16 * cc);
+#pragma unroll
+        for (int v = 0; v < 4; ++v)
+          dst[v] = make_float4(sc * __uint_as_float(r[4 * v]), sc * __uint_as_float(r[4 * v + 1]),
+                               sc * __uint_as_float(r[4 * v + 2]), sc * __uint_as_float(r[4 * v + 3]));
+      }
+    }
+    if (LOSS) {
+      float l0, l1;
+      unpack2(loss2, l0, l1);
+      float loss = l0 + l1;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) loss += __shfl_xor_sync(0xffffffffu, loss, o);
+      if (lane == 0) loss_red[ew] = loss;
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      if (ew == 0 && lane == 0) {
+        float t = 0.f;
+        for (int w = 0; w < EPI_WARPS; ++w) t += loss_red[w];
+        loss_part[((size_t)split * nslices + slice) * nh + h] = t;
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tb, 512);
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+int bf16_update_wide_supported(const ttt_config* cfg) {
+  return cfg->hd == updw::HD && cfg->hidden % updw::HS == 0 && !cfg->linear_fast_weight;
+}
+
+// appends `splits` partial-gradient sets; split geometry (tiles of 32 tokens) comes from the caller
+int bf16_accumulate_wide(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V, const float* lr,
+                         int64_t M, int64_t ld, bool want_loss, int tiles, int tps, int splits,
+                         cudaStream_t s) {
+  const ttt_config& c = ctx->cfg;
+  CUtensorMap mapK, mapV, mapW;
+  int rc = make_token_map(ctx, &mapK, K, M, (int64_t)c.nh * c.hd, ld, updw::T);
+  if (rc != TTT_OK) return rc;
+  rc = make_token_map(ctx, &mapV, V, M, (int64_t)c.nh * c.hd, ld, updw::T);
+  if (rc != TTT_OK) return rc;
+  // bf16 operand copy of the weights as one [3 nh H][hd] matrix, boxes of [128 rows][64]
+  rc = make_token_map(ctx, &mapW, ctx->Wb, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, updw::HS);
+  if (rc != TTT_OK) return rc;
+  static bool attr_set = false;
+  if (!attr_set) {
+    TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_update_wide_kernel<false>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)updw::SMEM_BYTES), "bf16_update_wide_kernel smem attr");
+    TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_update_wide_kernel<true>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)updw::SMEM_BYTES), "bf16_update_wide_kernel smem attr");
+    attr_set = true;
+  }
+  float* P = ctx->partials + (size_t)ctx->n_partials * 3 * ctx->mat_elems;
+  dim3 grid(splits, c.hidden / updw::HS, c.nh);
+  if (want_loss)
+    bf16_update_wide_kernel<true><<<grid, updw::THREADS, updw::SMEM_BYTES, s>>>(
+        mapK, mapV, mapW, lr, P, ctx->loss_part, (int)M, c.nh, c.hidden, tiles, tps);
+  else
+    bf16_update_wide_kernel<false><<<grid, updw::THREADS, updw::SMEM_BYTES, s>>>(
+        mapK, mapV, mapW, lr, P, ctx->loss_part, (int)M, c.nh, c.hidden, tiles, tps);
+  TTT_LAUNCH_CHECK(ctx, "bf16_update_wide_kernel");
+  return TTT_OK;
+}
+
+}  // namespace ttt

@@ -38,8 +38,8 @@ int check_tokens(ttt_ctx* ctx, int64_t M, int64_t ld) {
 // accumulate kernel has already committed (fused path), TTT_OK if a commit is still due
 int do_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, int64_t M,
                   int64_t ld, float* loss, cudaStream_t s, bool commit_now = false) {
-  const bool bf16 = ctx->cfg.act_dtype == TTT_BF16 && !ctx->bf16_via_f32;
-  if (ctx->bf16_via_f32) {      // bf16 I/O on the fp32 CUDA-core path: convert K, V first
+  const bool bf16 = ctx->cfg.act_dtype == TTT_BF16 && !ctx->upd_via_f32;
+  if (ctx->upd_via_f32) {      // bf16 I/O on the fp32 CUDA-core path: convert K, V first
     const int64_t d = (int64_t)ctx->cfg.nh * ctx->cfg.hd;
     int rc = launch_bf16_to_f32(ctx, static_cast<const __nv_bfloat16*>(K), ld, ctx->stage[0], M, s);
     if (rc == TTT_OK) rc = launch_bf16_to_f32(ctx, static_cast<const __nv_bfloat16*>(V), ld, ctx->stage[1], M, s);
@@ -75,7 +75,7 @@ int do_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, i
 }
 
 int do_apply(ttt_ctx* ctx, const void* Q, void* O, int64_t M, int64_t ld, cudaStream_t s) {
-  if (ctx->bf16_via_f32) {
+  if (ctx->app_via_f32) {
     const int64_t d = (int64_t)ctx->cfg.nh * ctx->cfg.hd;
     int rc = launch_bf16_to_f32(ctx, static_cast<const __nv_bfloat16*>(Q), ld, ctx->stage[0], M, s);
     if (rc == TTT_OK) rc = f32_apply(ctx, ctx->stage[0], ctx->stage[1], M, d, s);
@@ -145,8 +145,12 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
   ctx->sm_count = prop.multiProcessorCount;
   ctx->mat_elems = (size_t)cfg->nh * cfg->hidden * cfg->hd;
   const size_t set = 3 * ctx->mat_elems;
-  ctx->bf16_via_f32 = cfg->act_dtype == TTT_BF16 && !bf16_tensor_path(cfg);
-  const bool bf16 = cfg->act_dtype == TTT_BF16 && !ctx->bf16_via_f32;
+  const bool is_bf16 = cfg->act_dtype == TTT_BF16;
+  ctx->upd_via_f32 = is_bf16 && !bf16_update_tensor_path(cfg);
+  ctx->app_via_f32 = is_bf16 && !bf16_apply_tensor_path(cfg);
+  const bool bf16 = is_bf16 && !ctx->upd_via_f32;          // update on the tensor cores
+  const bool any_tc = is_bf16 && !(ctx->upd_via_f32 && ctx->app_via_f32);
+  const bool any_f32 = !is_bf16 || ctx->upd_via_f32 || ctx->app_via_f32;
   ctx->cap_partials = 2 * (bf16 ? bf16_partials_needed(ctx, cfg->max_tokens)
                                 : f32_partials_needed(ctx, cfg->max_tokens));
   if (ctx->cap_partials < 4) ctx->cap_partials = 4;
@@ -169,17 +173,18 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
     alloc((void**)&ctx->sync_ctr, nctr * sizeof(unsigned));
     if (ok && cudaMemset(ctx->sync_ctr, 0, nctr * sizeof(unsigned)) != cudaSuccess) ok = false;
   }
-  if (ctx->bf16_via_f32) {
+  if (ctx->upd_via_f32 || ctx->app_via_f32) {
     const size_t st = (size_t)cfg->max_tokens * cfg->nh * cfg->hd * sizeof(float);
     alloc((void**)&ctx->stage[0], st);
     alloc((void**)&ctx->stage[1], st);
   }
-  if (!bf16) {
+  if (any_f32) {
     const size_t act = (size_t)cfg->nh * cfg->max_tokens * cfg->hidden * sizeof(float);
     for (int i = 0; i < 3; ++i) alloc((void**)&ctx->act[i], act);
     alloc((void**)&ctx->loss_blk, (size_t)cfg->nh * ((cfg->max_tokens + 63) / 64) *
                                       ((cfg->hidden + 63) / 64) * sizeof(float));
-  } else {
+  }
+  if (any_tc) {
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ctx->encode_tiled, cudaEnableDefault,
                                 &qres) != cudaSuccess ||

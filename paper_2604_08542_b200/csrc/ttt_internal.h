@@ -42,7 +42,7 @@ struct ttt_ctx {
   float* act[3];
   // bf16 I/O on the fp32 CUDA-core path (shapes the tensor kernels do not cover yet, e.g. hd = 128):
   // two [max_tokens][nh*hd] fp32 staging buffers for the converted token tensors
-  bool bf16_via_f32;
+  bool upd_via_f32, app_via_f32;   // per call family: update (accumulate) / apply
   float* stage[2];
 
   // bf16 path: group-barrier counters of the fused commit ([nh][hidden/128]) and their running target
@@ -92,8 +92,14 @@ int bf16_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M
                cudaStream_t s);
 int bf16_partials_needed(const ttt_ctx* ctx, int64_t M);
 int bf16_supported(const ttt_config* cfg, char* why, size_t why_len);
-// 1 if the tcgen05 kernels cover the shape, 0 if bf16 I/O must go through the fp32 CUDA-core path
-int bf16_tensor_path(const ttt_config* cfg);
+// 1 if a tcgen05 kernel covers the shape, 0 if bf16 I/O must go through the fp32 CUDA-core path
+int bf16_update_tensor_path(const ttt_config* cfg);
+int bf16_apply_tensor_path(const ttt_config* cfg);
+// hd = 128 update kernel (bf16_update_wide.cu)
+int bf16_update_wide_supported(const ttt_config* cfg);
+int bf16_accumulate_wide(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V, const float* lr,
+                         int64_t M, int64_t ld, bool want_loss, int tiles, int tps, int splits,
+                         cudaStream_t s);
 // strided bf16 [M][cols] (row stride ld) <-> dense fp32 [M][cols]
 int launch_bf16_to_f32(ttt_ctx* ctx, const __nv_bfloat16* src, int64_t ld, float* dst, int64_t M, cudaStream_t s);
 int launch_f32_to_bf16(ttt_ctx* ctx, const float* src, __nv_bfloat16* dst, int64_t ld, int64_t M, cudaStream_t s);
