@@ -290,6 +290,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
 int bf16_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
                cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
+  if (c.hd == 128) return bf16_apply_wide(ctx, Q, O, M, ld, s);   // streamed weights
   const int tiles = (int)((M + app::TM - 1) / app::TM);
   int per_head = ctx->sm_count / c.nh;
   if (per_head < 1) per_head = 1;

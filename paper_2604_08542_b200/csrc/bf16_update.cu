@@ -583,11 +583,14 @@ int bf16_partials_needed(const ttt_ctx* ctx, int64_t M) {
   return s;
 }
 
-int bf16_apply_tensor_path(const ttt_config* cfg) {
+static int narrow_tensor_path(const ttt_config* cfg) {
   return cfg->hd == 64 && (cfg->hidden == 128 || cfg->hidden == 256) && !cfg->linear_fast_weight;
 }
+int bf16_apply_tensor_path(const ttt_config* cfg) {
+  return narrow_tensor_path(cfg) || bf16_apply_wide_supported(cfg);
+}
 int bf16_update_tensor_path(const ttt_config* cfg) {
-  return bf16_apply_tensor_path(cfg) || bf16_update_wide_supported(cfg);
+  return narrow_tensor_path(cfg) || bf16_update_wide_supported(cfg);
 }
 
 // bf16 token tensors are accepted for every shape the fp32 path takes; shapes outside the tcgen05

@@ -95,6 +95,10 @@ int bf16_supported(const ttt_config* cfg, char* why, size_t why_len);
 // 1 if a tcgen05 kernel covers the shape, 0 if bf16 I/O must go through the fp32 CUDA-core path
 int bf16_update_tensor_path(const ttt_config* cfg);
 int bf16_apply_tensor_path(const ttt_config* cfg);
+// hd = 128 apply kernel (bf16_apply_wide.cu)
+int bf16_apply_wide_supported(const ttt_config* cfg);
+int bf16_apply_wide(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
+                    cudaStream_t s);
 // hd = 128 update kernel (bf16_update_wide.cu)
 int bf16_update_wide_supported(const ttt_config* cfg);
 int bf16_accumulate_wide(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V, const float* lr,

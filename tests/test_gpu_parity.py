@@ -141,14 +141,42 @@ def test_bf16_stream_parity(base, kw):
     assert max(errs_l) <= TOL_LOSS_BF16, errs_l
 
 
-def test_bf16_cfg5_shape_runs_on_the_fp32_cuda_core_path():
-    """hd = 128 / H = 512 (BASELINE.json:configs[4] shape, cut down): bf16 I/O through the C ABI; this
-    shape is outside the tcgen05 kernels' set and runs on the fp32 CUDA-core kernels."""
+def test_bf16_cfg5_shape_stream():
+    """hd = 128 / H = 512 (BASELINE.json:configs[4] shape, cut down): bf16 I/O through the C ABI on the
+    hd = 128 tensor-core kernels (weights in shared memory / streamed), Newton-Schulz commit."""
     w = _bf16_workload("cfg5", nh=2, tokens_per_frame=137, frames_per_chunk=2, n_frames=6)
     errs_o, errs_w, errs_l = _run_stream(w)
     assert max(errs_o) <= TOL_BF16, errs_o
     assert max(errs_w) <= TOL_BF16, errs_w
     assert max(errs_l) <= TOL_LOSS_BF16, errs_l
+
+
+@pytest.mark.parametrize("M", [5000, 257, 31])
+def test_bf16_wide_head_gradient_and_apply(M):
+    """hd = 128 kernels at a size where a CTA walks many token tiles (update: ring wraps, operand
+    columns re-used) and several (head, tile pair) units (apply: M = 5000 -> 160 units on 148 SMs),
+    with ragged tails: pending gradient, committed weights and apply output against the oracle."""
+    dev = torch.device("cuda", 0)
+    w = _bf16_workload("cfg5", nh=8, tokens_per_frame=M, frames_per_chunk=1, n_frames=1, ns_iters=0)
+    W1, W2, W3 = ti.fast_weights(w)
+    Q, K, V, lr = ti.TokenStream(w).next_chunk()
+    lr = lr * torch.linspace(0.5, 1.5, M)[None, :]              # per-token learning rates differ
+    gpu = _mk(w)
+    gpu.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    gpu.ttt_accumulate(K.to(dev), V.to(dev), lr.to(dev))
+    G = gpu.ttt_pending_gradient().cpu()                        # [3, nh, H, hd] hidden-major
+    ora = OracleTTT(W1, W2, W3)
+    G1, G2, G3, _ = ora.grad(K, V, lr)
+    assert rel_err(G[0].transpose(1, 2), G1) <= 1e-2
+    assert rel_err(G[1], G2) <= 1e-2
+    assert rel_err(G[2].transpose(1, 2), G3) <= 1e-2
+    gpu.ttt_commit()
+    ora.update(K, V, lr)
+    g1, g2, g3 = (x.cpu() for x in gpu.ttt_get_weights())
+    assert max(rel_err(g1, ora.W1), rel_err(g2, ora.W2), rel_err(g3, ora.W3)) <= TOL_BF16
+    O = gpu.ttt_apply(Q.to(dev))
+    assert rel_err(O.float().cpu(), ora.apply(Q)) <= TOL_BF16
+    gpu.close()
 
 
 def test_bf16_gradient_against_oracle():
