@@ -367,6 +367,7 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
 }
 
 int ns_tc_supported(const ttt_config* cfg) {
+  if (ns_tc_wide_supported(cfg)) return 1;
   return cfg->act_dtype == TTT_BF16 && cfg->hd == 64 && cfg->hidden % 128 == 0 &&
          cfg->hidden >= 128 && cfg->hidden <= 512 && !cfg->linear_fast_weight;
 }
@@ -376,6 +377,7 @@ int ns_tc_supported(const ttt_config* cfg) {
 // otherwise NS(g) is left in G (G_valid) for the commit kernel.
 int launch_ns_tc(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
+  if (c.hd == 128) return launch_ns_tc_wide(ctx, fuse_commit, s);
   size_t smem = (size_t)2 * c.hidden * 128 + 4 * 8192 + 128 * nstc::S_LD * sizeof(float);
   const size_t stage = (size_t)c.hidden * nstc::W_LD * sizeof(float);
   if (stage > smem) smem = stage;

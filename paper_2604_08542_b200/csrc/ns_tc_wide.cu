@@ -1,0 +1,342 @@
+// ns_tc_wide.cu — Newton-Schulz orthonormalisation on the tensor cores for head dimension 128
+// (reading R-NS; BASELINE.json configs[4]: 8 heads x 128, hidden 512).
+//
+// Tall form of the iteration on X [H x 128] (hidden-major), as in ns_tc.cu:
+//     X0 = g / (||g||_F + 1e-7);   n times:  A = X^T X;  Pm = a I + b A + c A A;  X <- X Pm
+// with every product as a split-bf16 ("bf16x3") contraction hi*hi + hi*lo + lo*hi, fp32 accumulation.
+//
+// At hd = 128 the hi / lo operand tiles of a whole matrix (256 KB at H = 512) exceed one SM's shared
+// memory, so a matrix is owned by a thread-block cluster of H / 128 CTAs, one 128-row block each:
+//   Gram   every CTA forms the partial A_r = X_r^T X_r of its rows (MN-major operands), exports it as
+//          fp32 to its own shared memory; after a cluster barrier every CTA sums the partials of all
+//          ranks over distributed shared memory in rank order (so all ranks hold bit-identical A);
+//   square A A and Pm are computed redundantly by every rank (128 x 128 x 128, cheap);
+//   tall   X_r <- X_r Pm needs no exchange.
+// The accumulator layout (TMEM lane = row, 32 columns per warp) is also the register layout of A and
+// X, so the folds need no transposition: TMEM -> registers -> hi/lo split -> swizzled operand tiles.
+#include <stdio.h>
+
+#include "tc_common.cuh"
+#include "ttt_internal.h"
+
+namespace ttt {
+
+namespace nsw {
+constexpr int HD = 128;
+constexpr int RB = 128;          // rows of X per CTA
+constexpr int THREADS = 512;     // fold / load workers (16 warps)
+constexpr int LAUNCH_THREADS = THREADS + 32;   // + the MMA-issuing warp (warp 16)
+constexpr int SUB = RB * 128;    // one [128 rows x 64] bf16 sub-tile (16 KB)
+constexpr int TILE = 2 * SUB;    // one [128 x 128] bf16 operand tile
+constexpr int EX_LD = 132;       // fp32 exchange row stride in floats (16-B aligned, conflict-free float4)
+constexpr size_t SMEM_BYTES = 4 * (size_t)TILE + (size_t)RB * EX_LD * sizeof(float) + 1024;
+constexpr uint32_t C_A = 0, C_A2 = 128, C_X = 256;
+}  // namespace nsw
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ void cluster_arrive() {
+  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void cluster_wait() {
+  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t dsmem_addr(uint32_t local_addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ float4 ld_dsmem_f4(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared::cluster.v4.f32 {%0, %1, %2, %3}, [%4];"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ float ld_dsmem_f(uint32_t addr) {
+  float v;
+  asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
+  return v;
+}
+
+// 32 fp32 values of one row (columns 32 cs .. 32 cs + 31) -> hi / lo bf16 into a [128 x 128] operand
+// tile pair stored as two 128-byte-swizzled [128 x 64] sub-tiles
+__device__ __forceinline__ void split_row32(const float (&v)[32], uint8_t* hi_tile, uint8_t* lo_tile,
+                                            int row, int cs) {
+  uint8_t* hs = hi_tile + (cs >> 1) * nsw::SUB;
+  uint8_t* ls = lo_tile + (cs >> 1) * nsw::SUB;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    uint32_t h[4], l[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float a = v[8 * k + 2 * i], b = v[8 * k + 2 * i + 1];
+      h[i] = pack_bf16x2(a, b);
+      l[i] = pack_bf16x2(a - __uint_as_float(h[i] << 16), b - __uint_as_float(h[i] & 0xffff0000u));
+    }
+    const int chunk = (cs & 1) * 4 + k;                    // 16-byte chunk within the 128-byte row
+    const uint32_t off = static_cast<uint32_t>(row * 128 + ((chunk ^ (row & 7)) << 4));
+    *reinterpret_cast<uint4*>(hs + off) = make_uint4(h[0], h[1], h[2], h[3]);
+    *reinterpret_cast<uint4*>(ls + off) = make_uint4(l[0], l[1], l[2], l[3]);
+  }
+}
+
+__global__ void __launch_bounds__(nsw::LAUNCH_THREADS, 1)
+ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, size_t set_elems,
+                  int use_G, int H, int iters, float* __restrict__ Wm, __nv_bfloat16* __restrict__ Wb) {
+  using namespace nsw;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
+  uint8_t* XH = smem;
+  uint8_t* XL = XH + TILE;
+  uint8_t* AH = XL + TILE;             // A, then Pm (hi)
+  uint8_t* AL = AH + TILE;
+  float* EX = reinterpret_cast<float*>(AL + TILE);          // [128][EX_LD] partial Gram of this rank
+  __shared__ uint64_t mma_bar;
+  __shared__ uint32_t tmem_base_s;
+  __shared__ float red[THREADS / 32];
+  __shared__ float s_part;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const bool issuer = warp == THREADS / 32;
+  const uint32_t rank = cluster_ctarank(), nc = gridDim.x;   // the cluster spans the grid's x dimension
+  const int q = warp & 3, cs = (warp >> 2) & 3;              // TMEM lane quarter, 32-column group
+  const int trow = q * 32 + lane;                            // row of the block = TMEM lane
+  const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
+  const size_t off = ((size_t)blockIdx.y * H + (size_t)rank * RB + trow) * HD + 32 * cs;
+
+  if (tid == 0) { mbar_init(&mma_bar, 1); fence_mbar_init(); }
+  if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+
+  // ---- load: g = (use_G ? G : 0) + sum_s P[s] (fixed order); Frobenius norm over the cluster ----
+  float g[32];
+  float acc = 0.f;
+  if (!issuer) {
+#pragma unroll
+    for (int v = 0; v < 8; ++v) {
+      const float4 x = use_G ? reinterpret_cast<const float4*>(G + off)[v] : make_float4(0.f, 0.f, 0.f, 0.f);
+      g[4 * v] = x.x; g[4 * v + 1] = x.y; g[4 * v + 2] = x.z; g[4 * v + 3] = x.w;
+    }
+    for (int s = 0; s < n_sets; ++s) {
+      const float4* ps = reinterpret_cast<const float4*>(P + (size_t)s * set_elems + off);
+      float4 p[8];
+#pragma unroll
+      for (int v = 0; v < 8; ++v) p[v] = __ldcg(ps + v);
+#pragma unroll
+      for (int v = 0; v < 8; ++v) {
+        g[4 * v] += p[v].x; g[4 * v + 1] += p[v].y; g[4 * v + 2] += p[v].z; g[4 * v + 3] += p[v].w;
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < 32; ++j) acc = fmaf(g[j], g[j], acc);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) red[warp] = acc;
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tb = tmem_base_s;
+  if (tid == 0) {
+    float t = 0.f;
+    for (int w = 0; w < THREADS / 32; ++w) t += red[w];
+    s_part = t;
+  }
+  __syncthreads();
+  cluster_arrive();
+  cluster_wait();
+  float scale;
+  {
+    float t = 0.f;
+    for (uint32_t r = 0; r < nc; ++r) t += ld_dsmem_f(dsmem_addr(smem_u32(&s_part), r));   // rank order
+    scale = 1.0f / (sqrtf(t) + 1e-7f);
+  }
+  if (!issuer) {
+#pragma unroll
+    for (int j = 0; j < 32; ++j) g[j] *= scale;
+    split_row32(g, XH, XL, trow, cs);
+  }
+  fence_proxy_async_smem();
+  __syncthreads();
+
+  constexpr uint32_t idesc_mn = umma_idesc_bf16(128, 128, 1, 1);   // A, B MN-major (Gram)
+  constexpr uint32_t idesc_k = umma_idesc_bf16(128, 128, 0, 0);    // A, B K-major
+  const uint64_t d_xh_mn = umma_smem_desc_sw128(smem_u32(XH), SUB, 1024);   // 2nd 64-column atom: +SUB
+  const uint64_t d_xl_mn = umma_smem_desc_sw128(smem_u32(XL), SUB, 1024);
+  const uint64_t d_xh = umma_smem_desc_sw128(smem_u32(XH), 16, 1024);
+  const uint64_t d_xl = umma_smem_desc_sw128(smem_u32(XL), 16, 1024);
+  const uint64_t d_ah = umma_smem_desc_sw128(smem_u32(AH), 16, 1024);
+  const uint64_t d_al = umma_smem_desc_sw128(smem_u32(AL), 16, 1024);
+  const float ca = 3.4445f, cb = -4.7750f, cc = 2.0315f;
+  uint32_t phase = 0;
+  float Areg[32];
+  auto end_phase = [&]() {
+    fence_proxy_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+  };
+  auto wait_mma = [&]() {
+    mbar_wait(&mma_bar, phase & 1);
+    phase ^= 1;
+    tc_fence_after();
+  };
+  // K-major split product D = (AH + AL) (BH + BL)^T without the lo*lo term, 128 x 128 x 128
+  auto product_k = [&](uint32_t dcol, uint64_t ah, uint64_t al, uint64_t bh, uint64_t bl) {
+#pragma unroll
+    for (int k = 0; k < HD / 16; ++k) {
+      const uint64_t o = (uint64_t)((k >> 2) * (SUB >> 4) + (k & 3) * 2);
+      umma_ss(dcol, ah + o, bh + o, idesc_k, k > 0);
+      umma_ss(dcol, ah + o, bl + o, idesc_k, 1);
+      umma_ss(dcol, al + o, bh + o, idesc_k, 1);
+    }
+    tc_commit(&mma_bar);
+  };
+  const uint32_t lead = issuer ? elect_one() : 0u;
+  const uint32_t ex_row = smem_u32(EX + trow * EX_LD + 32 * cs);
+
+  for (int it = 0; it < iters; ++it) {
+    const bool last = it == iters - 1;
+    // ---------------- A = X^T X: partial over this rank's rows, summed over the cluster ----------------
+    if (lead) {
+#pragma unroll
+      for (int ks = 0; ks < RB / 16; ++ks) {               // +2048 B per 16-row K step
+        umma_ss(tb + C_A, d_xh_mn + 128 * ks, d_xh_mn + 128 * ks, idesc_mn, ks > 0);
+        umma_ss(tb + C_A, d_xh_mn + 128 * ks, d_xl_mn + 128 * ks, idesc_mn, 1);
+        umma_ss(tb + C_A, d_xl_mn + 128 * ks, d_xh_mn + 128 * ks, idesc_mn, 1);
+      }
+      tc_commit(&mma_bar);
+    }
+    __syncwarp();
+    if (!issuer) wait_mma();
+    if (it > 0) cluster_wait();        // every rank has read this rank's previous partial
+    if (!issuer) {
+      uint32_t r[32];
+      tmem_ld_x32(tb + lane_base + C_A + 32 * cs, r);
+      tc_wait_ld();
+      float4* dst = reinterpret_cast<float4*>(EX + trow * EX_LD + 32 * cs);
+#pragma unroll
+      for (int v = 0; v < 8; ++v)
+        dst[v] = make_float4(__uint_as_float(r[4 * v]), __uint_as_float(r[4 * v + 1]),
+                             __uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3]));
+    }
+    cluster_arrive();
+    cluster_wait();
+    if (!issuer) {
+#pragma unroll
+      for (int j = 0; j < 32; ++j) Areg[j] = 0.f;
+      for (uint32_t r = 0; r < nc; ++r) {                  // rank order: identical A on every rank
+        const uint32_t src = dsmem_addr(ex_row, r);
+#pragma unroll
+        for (int v = 0; v < 8; ++v) {
+          const float4 x = ld_dsmem_f4(src + 16 * v);
+          Areg[4 * v] += x.x; Areg[4 * v + 1] += x.y; Areg[4 * v + 2] += x.z; Areg[4 * v + 3] += x.w;
+        }
+      }
+      split_row32(Areg, AH, AL, trow, cs);
+    }
+    cluster_arrive();                  // done reading the other ranks' partials
+    end_phase();
+    // ---------------- Pm = a I + b A + c A A (A symmetric: K-major A . A^T) ----------------
+    if (lead) product_k(tb + C_A2, d_ah, d_al, d_ah, d_al);
+    __syncwarp();
+    if (!issuer) {
+      wait_mma();
+      uint32_t r[32];
+      tmem_ld_x32(tb + lane_base + C_A2 + 32 * cs, r);
+      tc_wait_ld();
+      float pm[32];
+#pragma unroll
+      for (int j = 0; j < 32; ++j) {
+        float p = fmaf(cc, __uint_as_float(r[j]), cb * Areg[j]);
+        if (32 * cs + j == trow) p += ca;
+        pm[j] = p;
+      }
+      split_row32(pm, AH, AL, trow, cs);                   // the A tiles are dead: Pm takes their place
+    }
+    end_phase();
+    // ---------------- X <- X Pm (Pm symmetric: K-major X . Pm^T) ----------------
+    if (lead) product_k(tb + C_X, d_xh, d_xl, d_ah, d_al);
+    __syncwarp();
+    if (!issuer) {
+      wait_mma();
+      uint32_t r[32];
+      tmem_ld_x32(tb + lane_base + C_X + 32 * cs, r);
+      tc_wait_ld();
+      float x[32];
+#pragma unroll
+      for (int j = 0; j < 32; ++j) x[j] = __uint_as_float(r[j]);
+      if (!last) {
+        split_row32(x, XH, XL, trow, cs);
+      } else if (Wm != nullptr) {                          // fused commit W <- W - NS(g) (Eq. 8)
+        float4* wm = reinterpret_cast<float4*>(Wm + off);
+        uint4* wb = reinterpret_cast<uint4*>(Wb + off);
+        float w[32];
+#pragma unroll
+        for (int v = 0; v < 8; ++v) {
+          const float4 t = wm[v];
+          w[4 * v] = t.x - x[4 * v]; w[4 * v + 1] = t.y - x[4 * v + 1];
+          w[4 * v + 2] = t.z - x[4 * v + 2]; w[4 * v + 3] = t.w - x[4 * v + 3];
+        }
+#pragma unroll
+        for (int v = 0; v < 8; ++v) wm[v] = make_float4(w[4 * v], w[4 * v + 1], w[4 * v + 2], w[4 * v + 3]);
+#pragma unroll
+        for (int v = 0; v < 4; ++v)
+          wb[v] = make_uint4(pack_bf16x2(w[8 * v], w[8 * v + 1]), pack_bf16x2(w[8 * v + 2], w[8 * v + 3]),
+                             pack_bf16x2(w[8 * v + 4], w[8 * v + 5]), pack_bf16x2(w[8 * v + 6], w[8 * v + 7]));
+      } else {
+        float4* gd = reinterpret_cast<float4*>(G + off);
+#pragma unroll
+        for (int v = 0; v < 8; ++v) gd[v] = make_float4(x[4 * v], x[4 * v + 1], x[4 * v + 2], x[4 * v + 3]);
+      }
+    }
+    end_phase();
+  }
+  if (iters > 0) cluster_wait();       // no rank still reads this CTA's shared memory
+  if (warp == 0) tmem_dealloc(tb, 512);
+}
+
+int ns_tc_wide_supported(const ttt_config* cfg) {
+  return cfg->act_dtype == TTT_BF16 && cfg->hd == nsw::HD && cfg->hidden % nsw::RB == 0 &&
+         cfg->hidden >= 128 && cfg->hidden <= 1024 && !cfg->linear_fast_weight;
+}
+
+int launch_ns_tc_wide(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s) {
+  const ttt_config& c = ctx->cfg;
+  static bool attr_set = false;
+  if (!attr_set) {
+    TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ns_tc_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)nsw::SMEM_BYTES), "ns_tc_wide_kernel smem attr");
+    attr_set = true;
+  }
+  const int nc = c.hidden / nsw::RB;                       // cluster size: one CTA per 128-row block
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(nc, 3 * c.nh);
+  cfg.blockDim = dim3(nsw::LAUNCH_THREADS);
+  cfg.dynamicSmemBytes = nsw::SMEM_BYTES;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = nc;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  float* G = ctx->G;
+  const float* P = ctx->partials;
+  int n_sets = ctx->n_partials, use_G = ctx->G_valid ? 1 : 0, H = c.hidden, iters = c.ns_iters;
+  size_t set_elems = 3 * ctx->mat_elems;
+  float* Wm = fuse_commit ? ctx->Wm : nullptr;
+  __nv_bfloat16* Wb = fuse_commit ? ctx->Wb : nullptr;
+  cudaError_t e = cudaLaunchKernelEx(&cfg, ns_tc_wide_kernel, G, P, n_sets, set_elems, use_G, H, iters, Wm, Wb);
+  if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, "ns_tc_wide_kernel launch", e);
+  TTT_LAUNCH_CHECK(ctx, "ns_tc_wide_kernel");
+  ctx->G_valid = !fuse_commit;
+  ctx->n_partials = 0;
+  return TTT_OK;
+}
+
+}  // namespace ttt

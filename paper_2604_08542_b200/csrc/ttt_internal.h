@@ -74,6 +74,9 @@ int ns_tc_supported(const ttt_config* cfg);
 // NS((G_valid ? G : 0) + sum partials) for all 3*nh matrices; fuse_commit: W <- W - NS(.) and the
 // pending set is cleared, else the result is left in G (G_valid)
 int launch_ns_tc(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s);
+// hd = 128: one thread-block cluster per matrix (ns_tc_wide.cu); reached through the two calls above
+int ns_tc_wide_supported(const ttt_config* cfg);
+int launch_ns_tc_wide(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s);
 
 // --- f32 path (f32_path.cu) ---------------------------------------------------------------------
 // appends partial-gradient sets [n_partials, n_partials + used); writes loss_part rows [0, loss_rows)

@@ -198,13 +198,15 @@ def test_bf16_gradient_against_oracle():
     gpu.close()
 
 
-@pytest.mark.parametrize("H", [128, 256])
-def test_bf16_newton_schulz_kernel_against_oracle(H):
-    """The tensor-core Newton-Schulz kernel in isolation: W0 - W' after a commit must equal the
-    oracle's NS of the very gradient the GPU holds (ttt_pending_gradient), to split-bf16 accuracy."""
+@pytest.mark.parametrize("hd,H", [(64, 128), (64, 256), (128, 128), (128, 256), (128, 512)])
+def test_bf16_newton_schulz_kernel_against_oracle(hd, H):
+    """The tensor-core Newton-Schulz kernels in isolation (hd = 64: one CTA per matrix; hd = 128: a
+    cluster of H / 128 CTAs per matrix): W0 - W' after a commit must equal the oracle's NS of the
+    very gradient the GPU holds (ttt_pending_gradient), to split-bf16 accuracy."""
     from oracle.ttt_oracle import newton_schulz
     dev = torch.device("cuda", 0)
-    w = _bf16_workload("cfg3", nh=2, hidden=H, tokens_per_frame=300, frames_per_chunk=2, n_frames=2)
+    w = _bf16_workload("cfg3", nh=2, hd=hd, hidden=H, tokens_per_frame=300, frames_per_chunk=2,
+                       n_frames=2)
     W1, W2, W3 = ti.fast_weights(w)
     Q, K, V, lr = ti.TokenStream(w).next_chunk()
     gpu = _mk(w)
