@@ -7,17 +7,29 @@
 //
 // At hd = 128 the hi / lo operand tiles of a whole matrix (256 KB at H = 512) exceed one SM's shared
 // memory, so a matrix is owned by a thread-block cluster of H / 128 CTAs, one 128-row block each:
-//   Gram   every CTA forms the partial A_r = X_r^T X_r of its rows (MN-major operands), exports it as
-//          fp32 to its own shared memory; after a cluster barrier every CTA sums the partials of all
-//          ranks over distributed shared memory in rank order (so all ranks hold bit-identical A);
+//   Gram   every CTA forms the partial A_r = X_r^T X_r of its rows (MN-major operands) and writes it as
+//          fp32 to a scratch in global memory (L2); after a cluster barrier every CTA sums the partials
+//          of all ranks in rank order (so all ranks hold bit-identical A). Distributed shared memory
+//          was measured first: ~20 B/clk per SM made the exchange 80 % of the kernel;
 //   square A A and Pm are computed redundantly by every rank (128 x 128 x 128, cheap);
 //   tall   X_r <- X_r Pm needs no exchange.
 // The accumulator layout (TMEM lane = row, 32 columns per warp) is also the register layout of A and
 // X, so the folds need no transposition: TMEM -> registers -> hi/lo split -> swizzled operand tiles.
+// Global traffic (load, exchange, write-out) is coalesced through one padded fp32 staging tile.
 #include <stdio.h>
 
 #include "tc_common.cuh"
 #include "ttt_internal.h"
+
+#ifdef TTT_TRACE
+__device__ long long g_nsw_trace[64];
+extern "C" int ttt_debug_nsw_trace(long long* host) {
+  return (int)cudaMemcpyFromSymbol(host, g_nsw_trace, sizeof(g_nsw_trace));
+}
+#define NSW_TR(k) do { if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && (k) < 64) g_nsw_trace[(k)] = clock64(); } while (0)
+#else
+#define NSW_TR(k) do { } while (0)
+#endif
 
 namespace ttt {
 
@@ -85,7 +97,8 @@ __device__ __forceinline__ void split_row32(const float (&v)[32], uint8_t* hi_ti
 
 __global__ void __launch_bounds__(nsw::LAUNCH_THREADS, 1)
 ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, size_t set_elems,
-                  int use_G, int H, int iters, float* __restrict__ Wm, __nv_bfloat16* __restrict__ Wb) {
+                  int use_G, int H, int iters, float* __restrict__ Wm, __nv_bfloat16* __restrict__ Wb,
+                  float* __restrict__ scratch) {
   using namespace nsw;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -94,7 +107,7 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
   uint8_t* XL = XH + TILE;
   uint8_t* AH = XL + TILE;             // A, then Pm (hi)
   uint8_t* AL = AH + TILE;
-  float* EX = reinterpret_cast<float*>(AL + TILE);          // [128][EX_LD] partial Gram of this rank
+  float* EX = reinterpret_cast<float*>(AL + TILE);          // [128][EX_LD] fp32 staging (row <-> coalesced)
   __shared__ uint64_t mma_bar;
   __shared__ uint32_t tmem_base_s;
   __shared__ float red[THREADS / 32];
@@ -106,32 +119,48 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
   const int q = warp & 3, cs = (warp >> 2) & 3;              // TMEM lane quarter, 32-column group
   const int trow = q * 32 + lane;                            // row of the block = TMEM lane
   const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
-  const size_t off = ((size_t)blockIdx.y * H + (size_t)rank * RB + trow) * HD + 32 * cs;
+  // this rank's [128 x 128] block of the matrix; float4 index e = tid + 512 k <-> (row e / 32, cols 4 (e % 32))
+  const size_t blk = ((size_t)blockIdx.y * H + (size_t)rank * RB) * HD;
+  float* ex_row = EX + trow * EX_LD + 32 * cs;               // row layout: this thread's 32 columns
+  auto ex_co = [&](int k) { const int e = tid + THREADS * k; return EX + (e >> 5) * EX_LD + (e & 31) * 4; };
+  auto worker_bar = [&]() { asm volatile("bar.sync 2, 512;" ::: "memory"); };
+  auto rows_to_ex = [&](const float (&v)[32]) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u)
+      reinterpret_cast<float4*>(ex_row)[u] = make_float4(v[4 * u], v[4 * u + 1], v[4 * u + 2], v[4 * u + 3]);
+  };
+  auto ex_to_rows = [&](float (&v)[32]) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const float4 x = reinterpret_cast<const float4*>(ex_row)[u];
+      v[4 * u] = x.x; v[4 * u + 1] = x.y; v[4 * u + 2] = x.z; v[4 * u + 3] = x.w;
+    }
+  };
 
+  NSW_TR(0);
   if (tid == 0) { mbar_init(&mma_bar, 1); fence_mbar_init(); }
   if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
 
-  // ---- load: g = (use_G ? G : 0) + sum_s P[s] (fixed order); Frobenius norm over the cluster ----
-  float g[32];
+  // ---- load (coalesced): g = (use_G ? G : 0) + sum_s P[s] (fixed order); Frobenius norm over the cluster ----
+  float4 g[8];
   float acc = 0.f;
   if (!issuer) {
 #pragma unroll
-    for (int v = 0; v < 8; ++v) {
-      const float4 x = use_G ? reinterpret_cast<const float4*>(G + off)[v] : make_float4(0.f, 0.f, 0.f, 0.f);
-      g[4 * v] = x.x; g[4 * v + 1] = x.y; g[4 * v + 2] = x.z; g[4 * v + 3] = x.w;
-    }
+    for (int k = 0; k < 8; ++k)
+      g[k] = use_G ? reinterpret_cast<const float4*>(G + blk)[tid + THREADS * k] : make_float4(0.f, 0.f, 0.f, 0.f);
     for (int s = 0; s < n_sets; ++s) {
-      const float4* ps = reinterpret_cast<const float4*>(P + (size_t)s * set_elems + off);
+      const float4* ps = reinterpret_cast<const float4*>(P + (size_t)s * set_elems + blk);
       float4 p[8];
 #pragma unroll
-      for (int v = 0; v < 8; ++v) p[v] = __ldcg(ps + v);
+      for (int k = 0; k < 8; ++k) p[k] = __ldcg(ps + tid + THREADS * k);
 #pragma unroll
-      for (int v = 0; v < 8; ++v) {
-        g[4 * v] += p[v].x; g[4 * v + 1] += p[v].y; g[4 * v + 2] += p[v].z; g[4 * v + 3] += p[v].w;
-      }
+      for (int k = 0; k < 8; ++k) { g[k].x += p[k].x; g[k].y += p[k].y; g[k].z += p[k].z; g[k].w += p[k].w; }
     }
 #pragma unroll
-    for (int j = 0; j < 32; ++j) acc = fmaf(g[j], g[j], acc);
+    for (int k = 0; k < 8; ++k) {
+      acc = fmaf(g[k].x, g[k].x, acc); acc = fmaf(g[k].y, g[k].y, acc);
+      acc = fmaf(g[k].z, g[k].z, acc); acc = fmaf(g[k].w, g[k].w, acc);
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
     if (lane == 0) red[warp] = acc;
@@ -156,11 +185,16 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
   }
   if (!issuer) {
 #pragma unroll
-    for (int j = 0; j < 32; ++j) g[j] *= scale;
-    split_row32(g, XH, XL, trow, cs);
+    for (int k = 0; k < 8; ++k)
+      *reinterpret_cast<float4*>(ex_co(k)) = make_float4(g[k].x * scale, g[k].y * scale, g[k].z * scale, g[k].w * scale);
+    worker_bar();
+    float x[32];
+    ex_to_rows(x);
+    split_row32(x, XH, XL, trow, cs);
   }
   fence_proxy_async_smem();
   __syncthreads();
+  NSW_TR(1);
 
   constexpr uint32_t idesc_mn = umma_idesc_bf16(128, 128, 1, 1);   // A, B MN-major (Gram)
   constexpr uint32_t idesc_k = umma_idesc_bf16(128, 128, 0, 0);    // A, B K-major
@@ -196,7 +230,8 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
     tc_commit(&mma_bar);
   };
   const uint32_t lead = issuer ? elect_one() : 0u;
-  const uint32_t ex_row = smem_u32(EX + trow * EX_LD + 32 * cs);
+  // partial Gram matrices: [matrix][rank][iteration parity][128 x 128] fp32 in global memory (L2)
+  float* sc_mat = scratch + (size_t)blockIdx.y * nc * 2 * RB * HD;
 
   for (int it = 0; it < iters; ++it) {
     const bool last = it == iters - 1;
@@ -211,35 +246,48 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
       tc_commit(&mma_bar);
     }
     __syncwarp();
-    if (!issuer) wait_mma();
-    if (it > 0) cluster_wait();        // every rank has read this rank's previous partial
     if (!issuer) {
-      uint32_t r[32];
-      tmem_ld_x32(tb + lane_base + C_A + 32 * cs, r);
-      tc_wait_ld();
-      float4* dst = reinterpret_cast<float4*>(EX + trow * EX_LD + 32 * cs);
+      wait_mma();
+      NSW_TR(2 + it * 8);
+      float v[32];
+      {
+        uint32_t r[32];
+        tmem_ld_x32(tb + lane_base + C_A + 32 * cs, r);
+        tc_wait_ld();
 #pragma unroll
-      for (int v = 0; v < 8; ++v)
-        dst[v] = make_float4(__uint_as_float(r[4 * v]), __uint_as_float(r[4 * v + 1]),
-                             __uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3]));
-    }
-    cluster_arrive();
-    cluster_wait();
-    if (!issuer) {
-#pragma unroll
-      for (int j = 0; j < 32; ++j) Areg[j] = 0.f;
-      for (uint32_t r = 0; r < nc; ++r) {                  // rank order: identical A on every rank
-        const uint32_t src = dsmem_addr(ex_row, r);
-#pragma unroll
-        for (int v = 0; v < 8; ++v) {
-          const float4 x = ld_dsmem_f4(src + 16 * v);
-          Areg[4 * v] += x.x; Areg[4 * v + 1] += x.y; Areg[4 * v + 2] += x.z; Areg[4 * v + 3] += x.w;
-        }
+        for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
       }
+      rows_to_ex(v);
+      worker_bar();
+      float4* dst = reinterpret_cast<float4*>(sc_mat + ((size_t)rank * 2 + (it & 1)) * RB * HD);
+#pragma unroll
+      for (int k = 0; k < 8; ++k) dst[tid + THREADS * k] = *reinterpret_cast<const float4*>(ex_co(k));
+      __threadfence();
+    }
+    NSW_TR(3 + it * 8);
+    cluster_arrive();                  // release: this rank's partial is in global memory
+    cluster_wait();
+    NSW_TR(4 + it * 8);
+    if (!issuer) {
+      float4 a[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) a[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+      for (uint32_t r = 0; r < nc; ++r) {                  // rank order: identical A on every rank
+        const float4* src = reinterpret_cast<const float4*>(sc_mat + ((size_t)r * 2 + (it & 1)) * RB * HD);
+        float4 p[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) p[k] = __ldcg(src + tid + THREADS * k);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { a[k].x += p[k].x; a[k].y += p[k].y; a[k].z += p[k].z; a[k].w += p[k].w; }
+      }
+#pragma unroll
+      for (int k = 0; k < 8; ++k) *reinterpret_cast<float4*>(ex_co(k)) = a[k];
+      worker_bar();
+      ex_to_rows(Areg);
       split_row32(Areg, AH, AL, trow, cs);
     }
-    cluster_arrive();                  // done reading the other ranks' partials
     end_phase();
+    NSW_TR(5 + it * 8);
     // ---------------- Pm = a I + b A + c A A (A symmetric: K-major A . A^T) ----------------
     if (lead) product_k(tb + C_A2, d_ah, d_al, d_ah, d_al);
     __syncwarp();
@@ -258,44 +306,52 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
       split_row32(pm, AH, AL, trow, cs);                   // the A tiles are dead: Pm takes their place
     }
     end_phase();
+    NSW_TR(6 + it * 8);
     // ---------------- X <- X Pm (Pm symmetric: K-major X . Pm^T) ----------------
     if (lead) product_k(tb + C_X, d_xh, d_xl, d_ah, d_al);
     __syncwarp();
     if (!issuer) {
       wait_mma();
-      uint32_t r[32];
-      tmem_ld_x32(tb + lane_base + C_X + 32 * cs, r);
-      tc_wait_ld();
       float x[32];
+      {
+        uint32_t r[32];
+        tmem_ld_x32(tb + lane_base + C_X + 32 * cs, r);
+        tc_wait_ld();
 #pragma unroll
-      for (int j = 0; j < 32; ++j) x[j] = __uint_as_float(r[j]);
+        for (int j = 0; j < 32; ++j) x[j] = __uint_as_float(r[j]);
+      }
       if (!last) {
         split_row32(x, XH, XL, trow, cs);
-      } else if (Wm != nullptr) {                          // fused commit W <- W - NS(g) (Eq. 8)
-        float4* wm = reinterpret_cast<float4*>(Wm + off);
-        uint4* wb = reinterpret_cast<uint4*>(Wb + off);
-        float w[32];
-#pragma unroll
-        for (int v = 0; v < 8; ++v) {
-          const float4 t = wm[v];
-          w[4 * v] = t.x - x[4 * v]; w[4 * v + 1] = t.y - x[4 * v + 1];
-          w[4 * v + 2] = t.z - x[4 * v + 2]; w[4 * v + 3] = t.w - x[4 * v + 3];
-        }
-#pragma unroll
-        for (int v = 0; v < 8; ++v) wm[v] = make_float4(w[4 * v], w[4 * v + 1], w[4 * v + 2], w[4 * v + 3]);
-#pragma unroll
-        for (int v = 0; v < 4; ++v)
-          wb[v] = make_uint4(pack_bf16x2(w[8 * v], w[8 * v + 1]), pack_bf16x2(w[8 * v + 2], w[8 * v + 3]),
-                             pack_bf16x2(w[8 * v + 4], w[8 * v + 5]), pack_bf16x2(w[8 * v + 6], w[8 * v + 7]));
       } else {
-        float4* gd = reinterpret_cast<float4*>(G + off);
+        // coalesced write-out through the staging tile: fused commit W <- W - NS(g) (Eq. 8), or NS(g) -> G
+        rows_to_ex(x);
+        worker_bar();
+        if (Wm != nullptr) {
+          float4* wm = reinterpret_cast<float4*>(Wm + blk);
+          uint2* wb = reinterpret_cast<uint2*>(Wb + blk);
+          float4 w[8];
 #pragma unroll
-        for (int v = 0; v < 8; ++v) gd[v] = make_float4(x[4 * v], x[4 * v + 1], x[4 * v + 2], x[4 * v + 3]);
+          for (int k = 0; k < 8; ++k) w[k] = wm[tid + THREADS * k];
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            const float4 d = *reinterpret_cast<const float4*>(ex_co(k));
+            w[k].x -= d.x; w[k].y -= d.y; w[k].z -= d.z; w[k].w -= d.w;
+            wm[tid + THREADS * k] = w[k];
+            wb[tid + THREADS * k] = make_uint2(pack_bf16x2(w[k].x, w[k].y), pack_bf16x2(w[k].z, w[k].w));
+          }
+        } else {
+          float4* gd = reinterpret_cast<float4*>(G + blk);
+#pragma unroll
+          for (int k = 0; k < 8; ++k) gd[tid + THREADS * k] = *reinterpret_cast<const float4*>(ex_co(k));
+        }
       }
     }
     end_phase();
+    NSW_TR(7 + it * 8);
   }
-  if (iters > 0) cluster_wait();       // no rank still reads this CTA's shared memory
+  cluster_arrive();                    // no rank may exit while another still reads its s_part
+  cluster_wait();
+  NSW_TR(50);
   if (warp == 0) tmem_dealloc(tb, 512);
 }
 
@@ -331,7 +387,7 @@ int launch_ns_tc_wide(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s) {
   size_t set_elems = 3 * ctx->mat_elems;
   float* Wm = fuse_commit ? ctx->Wm : nullptr;
   __nv_bfloat16* Wb = fuse_commit ? ctx->Wb : nullptr;
-  cudaError_t e = cudaLaunchKernelEx(&cfg, ns_tc_wide_kernel, G, P, n_sets, set_elems, use_G, H, iters, Wm, Wb);
+  cudaError_t e = cudaLaunchKernelEx(&cfg, ns_tc_wide_kernel, G, P, n_sets, set_elems, use_G, H, iters, Wm, Wb, ctx->ns_scratch);
   if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, "ns_tc_wide_kernel launch", e);
   TTT_LAUNCH_CHECK(ctx, "ns_tc_wide_kernel");
   ctx->G_valid = !fuse_commit;

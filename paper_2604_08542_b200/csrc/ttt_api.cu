@@ -173,6 +173,8 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
     alloc((void**)&ctx->sync_ctr, nctr * sizeof(unsigned));
     if (ok && cudaMemset(ctx->sync_ctr, 0, nctr * sizeof(unsigned)) != cudaSuccess) ok = false;
   }
+  if (cfg->ns_iters > 0 && ns_tc_wide_supported(cfg))
+    alloc((void**)&ctx->ns_scratch, (size_t)3 * cfg->nh * (cfg->hidden / 128) * 2 * 128 * 128 * sizeof(float));
   if (ctx->upd_via_f32 || ctx->app_via_f32) {
     const size_t st = (size_t)cfg->max_tokens * cfg->nh * cfg->hd * sizeof(float);
     alloc((void**)&ctx->stage[0], st);
@@ -205,7 +207,7 @@ void ttt_destroy(ttt_ctx* ctx) {
   cudaSetDevice(ctx->cfg.device);
   cudaDeviceSynchronize();
   cudaFree(ctx->Wm); cudaFree(ctx->Wb); cudaFree(ctx->n0); cudaFree(ctx->colsq);
-  cudaFree(ctx->G); cudaFree(ctx->partials); cudaFree(ctx->loss_part); cudaFree(ctx->loss_blk); cudaFree(ctx->sync_ctr); cudaFree(ctx->stage[0]); cudaFree(ctx->stage[1]);
+  cudaFree(ctx->G); cudaFree(ctx->partials); cudaFree(ctx->loss_part); cudaFree(ctx->loss_blk); cudaFree(ctx->sync_ctr); cudaFree(ctx->ns_scratch); cudaFree(ctx->stage[0]); cudaFree(ctx->stage[1]);
   for (int i = 0; i < 3; ++i) cudaFree(ctx->act[i]);
   delete ctx;
 }

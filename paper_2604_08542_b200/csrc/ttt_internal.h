@@ -46,6 +46,8 @@ struct ttt_ctx {
   float* stage[2];
 
   // bf16 path: group-barrier counters of the fused commit ([nh][hidden/128]) and their running target
+  // hd = 128 Newton-Schulz: partial Gram matrices [3 nh][hidden/128][2][128 x 128] fp32
+  float* ns_scratch;
   unsigned* sync_ctr;
   unsigned sync_target;
 
