@@ -55,7 +55,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
   uint8_t* ring = smem + W_BYTES;
-  __shared__ uint64_t full[STAGES], empty[STAGES], w_full, fwd_full, xbg_free, opnd_ready, grad_done;
+  __shared__ uint64_t full[STAGES], empty[STAGES], w_full, fwd_full, xbg_free, opnd_ready, opnd_free, grad_done;
   __shared__ uint32_t tmem_base_s;
   __shared__ float loss_red[EPI_WARPS];
   __shared__ __align__(16) float ne_s[STAGES][T];   // -eta of the stage's tokens (0 beyond M)
@@ -82,6 +82,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
     mbar_init(&fwd_full, 1);
     mbar_init(&xbg_free, 1);
     mbar_init(&opnd_ready, EPI_WARPS);
+    mbar_init(&opnd_free, 1);
     mbar_init(&grad_done, 1);
     fence_mbar_init();
     tma_prefetch_desc(&mapK);
@@ -139,12 +140,18 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
           umma_ss(dcol, a, b, idesc_f, k > 0);
         }
       };
-      auto gradients = [&](uint64_t st, uint32_t acc) {
+      // gradient MMAs of a tile, in two groups: G2 reads Hd' from the x columns and must precede the next
+      // x product; G1 / G3 read their own operand columns and fill the pipe while the epilogue loads x | b | g
+      auto grad_w2 = [&](uint64_t st, uint32_t acc) {
 #pragma unroll
-        for (int k = 0; k < T / 16; ++k) {                   // +2048 B per 16-token K step
+        for (int k = 0; k < T / 16; ++k)                     // +2048 B per 16-token K step
+          umma_ts(C_G2, C_OH + 8 * k, dr_mn + st + (TILE_BYTES >> 4) + 128 * k, idesc_g, acc | k);
+      };
+      auto grad_w13 = [&](uint64_t st, uint32_t acc) {
+#pragma unroll
+        for (int k = 0; k < T / 16; ++k) {
           umma_ts(C_G1, C_OA + 8 * k, dr_mn + st + 128 * k, idesc_g, acc | k);
           umma_ts(C_G3, C_OB + 8 * k, dr_mn + st + 128 * k, idesc_g, acc | k);
-          umma_ts(C_G2, C_OH + 8 * k, dr_mn + st + (TILE_BYTES >> 4) + 128 * k, idesc_g, acc | k);
         }
       };
       mbar_wait(&w_full, 0);
@@ -161,18 +168,23 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
         if (i > 0) {
           mbar_wait(&opnd_ready, (i - 1) & 1);
           tc_fence_after();
-          gradients(st_prev, i > 1);
-          tc_commit(&empty[s_prev]);
+          grad_w2(st_prev, i > 1);
         }
         forward(0, st, C_X);           // after the gradient MMAs that read Hd' from these columns
         tc_commit(&fwd_full);
+        if (i > 0) {
+          grad_w13(st_prev, i > 1);    // runs while the epilogue of tile i loads its accumulators
+          tc_commit(&opnd_free);       // 2 dA | dB operand columns may be overwritten
+          tc_commit(&empty[s_prev]);
+        }
         st_prev = st;
         s_prev = s;
       }
       if (ntiles > 0) {
         mbar_wait(&opnd_ready, (ntiles - 1) & 1);
         tc_fence_after();
-        gradients(st_prev, ntiles > 1);
+        grad_w2(st_prev, ntiles > 1);
+        grad_w13(st_prev, ntiles > 1);
       }
       tc_commit(&grad_done);
     }
@@ -247,8 +259,10 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
         ph[c >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));            // Hd' = -eta Hd
         if (LOSS) loss2 = ffma2(hdv, g, loss2);
       }
-      // the gradient MMAs of tile i-1 (the last readers of these columns) were issued before the x
-      // MMAs of tile i and are covered by the same commit: they have completed
+      // Hd' columns: their last readers (W2-gradient MMAs of tile i-1) were issued before the x MMAs of
+      // tile i and are covered by fwd_full; 2 dA | dB columns: released by the commit after the W1 / W3
+      // gradient MMAs of tile i-1
+      if (i > 0) { mbar_wait(&opnd_free, (i - 1) & 1); tc_fence_after(); }
       tmem_st_x8(lane_base + C_OA + 8 * kh, pa);
       tmem_st_x8(lane_base + C_OB + 8 * kh, pb);
       tmem_st_x8(lane_base + C_OH + 8 * kh, ph);
