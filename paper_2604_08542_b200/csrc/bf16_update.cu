@@ -578,6 +578,7 @@ static void update_split(const ttt_ctx* ctx, int64_t M, int* tiles_total, int* t
 }
 
 int bf16_partials_needed(const ttt_ctx* ctx, int64_t M) {
+  if (ctx->cfg.hd == 128) return bf16_wide_partials_needed(ctx, M);
   int a, b, s;
   update_split(ctx, M, &a, &b, &s);
   return s;
@@ -608,13 +609,8 @@ int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V
   const ttt_config& c = ctx->cfg;
   int tiles, tps, splits;
   update_split(ctx, M, &tiles, &tps, &splits);
-  if (c.hd == 128) {                     // hd = 128: weights in shared memory, no fused commit
-    int rc = bf16_accumulate_wide(ctx, K, V, lr, M, ld, want_loss, tiles, tps, splits, s);
-    if (rc != TTT_OK) return rc;
-    *used = splits;
-    *loss_rows = splits * (c.hidden / upd::HS);
-    return TTT_OK;
-  }
+  if (c.hd == 128)                       // hd = 128: weights in shared memory, no fused commit
+    return bf16_accumulate_wide(ctx, K, V, lr, M, ld, want_loss, used, loss_rows, s);
   CUtensorMap mapK, mapV;
   int rc = make_token_map(ctx, &mapK, K, M, (int64_t)c.nh * c.hd, ld, upd::T);
   if (rc != TTT_OK) return rc;

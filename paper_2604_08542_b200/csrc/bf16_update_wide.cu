@@ -10,8 +10,8 @@
 //   * the bf16 operand Hd' of the W2 gradient re-uses the columns of x; the MMA order
 //     b(i+1), g(i+1), gradients(i), x(i+1) keeps the tensor pipe busy while the epilogue of tile i runs
 //     and makes the overwrite of x safe (MMAs of one thread execute in issue order).
-// One CTA = (token split, 128-hidden slice, head); its partial gradients go to one partial set per
-// split, summed in split order by the commit (deterministic, no float atomics).
+// A CTA works on one (head, 128-hidden slice) pair at a time; its partial gradients go to one partial
+// set per segment, summed in set order by the commit (deterministic, no float atomics).
 #include <stdio.h>
 
 #include "tc_common.cuh"
@@ -44,12 +44,17 @@ constexpr uint32_t C_OA = 480, C_OB = 496;             // bf16 operands 2 dA, dB
 constexpr uint32_t C_OH = C_X;                         // bf16 operand Hd' = -eta Hd, over the dead x
 }  // namespace updw
 
+// Work distribution: the (head, slice) pairs x 32-token tiles form one list of units, pair-major; CTA c
+// of `gridDim.x` takes units [c U / n, (c + 1) U / n) — every SM gets the same amount of work, and a
+// CTA whose range crosses a pair boundary runs one segment per pair (weights reloaded, accumulators
+// flushed in between). Segment j of a pair (in CTA order) writes partial set j; the pair's last
+// segment zero-fills the sets up to `nsets`, so the commit sums the same number of sets everywhere.
 template <bool LOSS>
 __global__ void __launch_bounds__(updw::THREADS, 1)
 bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
                         const __grid_constant__ CUtensorMap mapW, const float* __restrict__ lr,
                         float* __restrict__ P, float* __restrict__ loss_part, int M, int nh, int H,
-                        int tiles_total, int tiles_per_split) {
+                        int tiles_total, int nsets) {
   using namespace updw;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -61,19 +66,35 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
   __shared__ __align__(16) float ne_s[STAGES][T];   // -eta of the stage's tokens (0 beyond M)
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int split = blockIdx.x, slice = blockIdx.y, h = blockIdx.z;
-  const int nslices = gridDim.y;
-  const int tile_lo = split * tiles_per_split;
-  const int ntiles = min(tiles_per_split, tiles_total - tile_lo);
-
-  auto load_stage = [&](int s, int tile) {
+  const int nslices = H / HS;
+  const long long U = (long long)nh * nslices * tiles_total;
+  const long long lo = blockIdx.x * U / gridDim.x, hi = (blockIdx.x + 1) * U / gridDim.x;
+  const int total = (int)(hi - lo);                 // tiles this CTA processes, over all its segments
+  // unit lo + gi -> pair (= h * nslices + slice) and token tile
+  auto locate = [&](int gi, int& pair, int& tile) {
+    const long long u = lo + gi;
+    pair = (int)(u / tiles_total);
+    tile = (int)(u - (long long)pair * tiles_total);
+  };
+  auto load_stage = [&](int gi) {
+    int pair, tile;
+    locate(gi, pair, tile);
+    const int s = gi % STAGES, h = pair / nslices, row = tile * T;
     mbar_arrive_expect_tx(&full[s], STAGE_BYTES);
     uint8_t* dst = ring + s * STAGE_BYTES;
-    const int row = tile * T;
     tma_load_2d(dst, &mapK, &full[s], h * HD, row);
     tma_load_2d(dst + SUB_BYTES, &mapK, &full[s], h * HD + 64, row);
     tma_load_2d(dst + TILE_BYTES, &mapV, &full[s], h * HD, row);
     tma_load_2d(dst + TILE_BYTES + SUB_BYTES, &mapV, &full[s], h * HD + 64, row);
+  };
+  // weights of a pair: mat m (0 = W1^T, 1 = W2, 2 = W3^T), hd half c -> [128 rows x 64] sub-tile
+  auto load_weights = [&](int pair) {
+    const int h = pair / nslices, slice = pair % nslices;
+    mbar_arrive_expect_tx(&w_full, W_BYTES);
+    for (int m = 0; m < 3; ++m)
+      for (int c = 0; c < 2; ++c)
+        tma_load_2d(smem + m * WMAT_BYTES + c * WSUB_BYTES, &mapW, &w_full, c * 64,
+                    (m * nh + h) * H + slice * HS);
   };
 
   if (tid == 0) {
@@ -88,25 +109,11 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
     tma_prefetch_desc(&mapK);
     tma_prefetch_desc(&mapV);
     tma_prefetch_desc(&mapW);
-    // weights of the slice: mat m (0 = W1^T, 1 = W2, 2 = W3^T), hd half c -> [128 rows x 64] sub-tile
-    mbar_arrive_expect_tx(&w_full, W_BYTES);
-    for (int m = 0; m < 3; ++m)
-      for (int c = 0; c < 2; ++c)
-        tma_load_2d(smem + m * WMAT_BYTES + c * WSUB_BYTES, &mapW, &w_full, c * 64,
-                    (m * nh + h) * H + slice * HS);
-    const int npre = min(ntiles, STAGES);
-    for (int i = 0; i < npre; ++i) load_stage(i, tile_lo + i);
+    if (total > 0) load_weights((int)(lo / tiles_total));
+    const int npre = min(total, STAGES);
+    for (int gi = 0; gi < npre; ++gi) load_stage(gi);
   }
   __syncwarp();
-  constexpr int LRPF = 4;
-  float lr_pre[LRPF];
-  if (warp == 2) {
-#pragma unroll
-    for (int u = 0; u < LRPF; ++u) {
-      const int t = (tile_lo + u) * T + lane;
-      lr_pre[u] = (u < ntiles && t < M) ? -__ldg(lr + (size_t)h * M + t) : 0.f;
-    }
-  }
   if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
   tc_fence_before();
   __syncthreads();
@@ -117,10 +124,9 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (elect_one()) {
-      for (int i = STAGES; i < ntiles; ++i) {        // tiles 0 .. STAGES-1 were requested in the prologue
-        const int s = i % STAGES, it = i / STAGES;
-        mbar_wait(&empty[s], (it & 1) ^ 1);
-        load_stage(s, tile_lo + i);
+      for (int gi = STAGES; gi < total; ++gi) {      // tiles 0 .. STAGES-1 were requested in the prologue
+        mbar_wait(&empty[gi % STAGES], ((gi / STAGES) & 1) ^ 1);
+        load_stage(gi);
       }
     }
   } else if (warp == 1) {
@@ -154,60 +160,78 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
           umma_ts(C_G3, C_OB + 8 * k, dr_mn + st + 128 * k, idesc_g, acc | k);
         }
       };
-      mbar_wait(&w_full, 0);
-      uint64_t st_prev = 0;
-      int s_prev = 0;
-      for (int i = 0; i < ntiles; ++i) {
-        const int s = i % STAGES;
-        const uint64_t st = (uint64_t)s * (STAGE_BYTES >> 4);
-        mbar_wait(&full[s], (i / STAGES) & 1);
-        if (i > 0) mbar_wait(&xbg_free, (i - 1) & 1);          // x | b | g of tile i-1 are in registers
-        tc_fence_after();
-        forward(2, st, C_B);
-        forward(1, st + (TILE_BYTES >> 4), C_G);
-        if (i > 0) {
-          mbar_wait(&opnd_ready, (i - 1) & 1);
+      int gi = 0, seg = 0;
+      while (gi < total) {
+        int pair, t0;
+        locate(gi, pair, t0);
+        const int n = min(total - gi, tiles_total - t0);     // tiles of this segment
+        if (seg > 0) {                 // every MMA that read the previous pair's weights has completed
+          mbar_wait(&grad_done, (seg - 1) & 1);
+          load_weights(pair);
+        }
+        mbar_wait(&w_full, seg & 1);
+        uint64_t st_prev = 0;
+        int s_prev = 0;
+        for (int i = 0; i < n; ++i, ++gi) {
+          const int s = gi % STAGES;
+          const uint64_t st = (uint64_t)s * (STAGE_BYTES >> 4);
+          mbar_wait(&full[s], (gi / STAGES) & 1);
+          if (i > 0) mbar_wait(&xbg_free, (gi - 1) & 1);       // x | b | g of the previous tile are in registers
           tc_fence_after();
-          grad_w2(st_prev, i > 1);
+          forward(2, st, C_B);
+          forward(1, st + (TILE_BYTES >> 4), C_G);
+          if (i > 0) {
+            mbar_wait(&opnd_ready, (gi - 1) & 1);
+            tc_fence_after();
+            grad_w2(st_prev, i > 1);
+          }
+          forward(0, st, C_X);           // after the gradient MMAs that read Hd' from these columns
+          tc_commit(&fwd_full);
+          if (i > 0) {
+            grad_w13(st_prev, i > 1);    // runs while the epilogue of tile i loads its accumulators
+            tc_commit(&opnd_free);       // 2 dA | dB operand columns may be overwritten
+            tc_commit(&empty[s_prev]);
+          }
+          st_prev = st;
+          s_prev = s;
         }
-        forward(0, st, C_X);           // after the gradient MMAs that read Hd' from these columns
-        tc_commit(&fwd_full);
-        if (i > 0) {
-          grad_w13(st_prev, i > 1);    // runs while the epilogue of tile i loads its accumulators
-          tc_commit(&opnd_free);       // 2 dA | dB operand columns may be overwritten
-          tc_commit(&empty[s_prev]);
-        }
-        st_prev = st;
-        s_prev = s;
-      }
-      if (ntiles > 0) {
-        mbar_wait(&opnd_ready, (ntiles - 1) & 1);
+        mbar_wait(&opnd_ready, (gi - 1) & 1);
         tc_fence_after();
-        grad_w2(st_prev, ntiles > 1);
-        grad_w13(st_prev, ntiles > 1);
+        grad_w2(st_prev, n > 1);
+        grad_w13(st_prev, n > 1);
+        tc_commit(&opnd_free);
+        tc_commit(&empty[s_prev]);
+        tc_commit(&grad_done);
+        ++seg;
       }
-      tc_commit(&grad_done);
     }
   } else if (warp == 2) {
     // ===================== learning-rate loader =====================
-    const float* lrh = lr + (size_t)h * M;
-    auto ld_batch = [&](int i0, float (&v)[LRPF]) {
+    // -eta of a tile (32 tokens = one 128-B line of lr) goes to the stage's shared-memory slot; the
+    // global loads run LRPF tiles ahead of the ring (register double buffer)
+    constexpr int LRPF = 4;
+    auto ld_batch = [&](int g0, float (&v)[LRPF]) {
 #pragma unroll
       for (int u = 0; u < LRPF; ++u) {
-        const int t = (tile_lo + i0 + u) * T + lane;
-        v[u] = (i0 + u < ntiles && t < M) ? -__ldg(lrh + t) : 0.f;
+        float x = 0.f;
+        if (g0 + u < total) {
+          int pair, tile;
+          locate(g0 + u, pair, tile);
+          const int t = tile * T + lane;
+          if (t < M) x = -__ldg(lr + (size_t)(pair / nslices) * M + t);
+        }
+        v[u] = x;
       }
     };
     float cur[LRPF], nxt[LRPF];
-#pragma unroll
-    for (int u = 0; u < LRPF; ++u) cur[u] = lr_pre[u];
-    for (int i0 = 0; i0 < ntiles; i0 += LRPF) {
-      ld_batch(i0 + LRPF, nxt);
+    ld_batch(0, cur);
+    for (int g0 = 0; g0 < total; g0 += LRPF) {
+      ld_batch(g0 + LRPF, nxt);
 #pragma unroll
       for (int u = 0; u < LRPF; ++u) {
-        const int i = i0 + u;
-        if (i < ntiles) {
-          const int s = i % STAGES, it = i / STAGES;
+        const int gi = g0 + u;
+        if (gi < total) {
+          const int s = gi % STAGES, it = gi / STAGES;
           if (it > 0) mbar_wait(&empty[s], (it & 1) ^ 1);
           ne_s[s][lane] = cur[u];
           __syncwarp();
@@ -222,95 +246,118 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
     const int ew = warp - 4, q = warp & 3, kh = ew >> 2;   // lane quadrant, K step (16 tokens) of the tile
     const int j = q * 32 + lane;                           // hidden unit within the slice = TMEM lane
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
-    uint64_t loss2 = 0ull;
     const uint64_t ONE2 = pack2(1.0f, 1.0f), NONE2 = pack2(-1.0f, -1.0f), HALF2 = pack2(0.5f, 0.5f);
-    for (int i = 0; i < ntiles; ++i) {
-      const int s = i % STAGES;
-      mbar_wait(&fwd_full, i & 1);
-      mbar_wait(&full[s], (i / STAGES) & 1);               // acquire of the loader's -eta slot
-      tc_fence_after();
-      const uint2* nes = reinterpret_cast<const uint2*>(&ne_s[s][16 * kh]);
-      uint32_t rx[16], rb[16], rg[16];
-      tmem_ld_x16(lane_base + C_X + 16 * kh, rx);
-      tmem_ld_x16(lane_base + C_B + 16 * kh, rb);
-      tmem_ld_x16(lane_base + C_G + 16 * kh, rg);
-      tc_wait_ld();
-      tc_fence_before();
-      asm volatile("bar.sync 1, 256;" ::: "memory");       // every warp holds its x | b | g
-      if (ew == 0 && lane == 0) mbar_arrive(&xbg_free);
-      uint32_t pa[8], pb[8], ph[8];
-#pragma unroll
-      for (int c = 0; c < 16; c += 2) {
-        const uint64_t x = fmul2(pack2u(rx[c], rx[c + 1]), HALF2);   // a / 2
-        const uint64_t bb = pack2u(rb[c], rb[c + 1]);
-        const uint2 nev = nes[c >> 1];
-        const uint64_t ne = pack2u(nev.x, nev.y);
-        const uint64_t g = fmul2(ne, pack2u(rg[c], rg[c + 1]));   // dHd = (-eta v) W2^T
-        float x0, x1;
-        unpack2(x, x0, x1);
-        const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
-        const uint64_t S = ffma2(x, th, x);                  // SiLU(a) = a sigmoid(a), a = 2 x
-        const uint64_t p = fadd2(th, ONE2);                  // 2 sigmoid(a)
-        const uint64_t m = ffma2(th, NONE2, ONE2);           // 2 (1 - sigmoid(a))
-        const uint64_t t2 = ffma2(S, m, p);                  // 2 SiLU'(a)
-        const uint64_t hdv = fmul2(S, bb);                   // hidden activation Hd
-        pa[c >> 1] = pack_bf16x2_from2(fmul2(fmul2(g, bb), t2));   // 2 dA
-        pb[c >> 1] = pack_bf16x2_from2(fmul2(g, S));               // dB
-        ph[c >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));            // Hd' = -eta Hd
-        if (LOSS) loss2 = ffma2(hdv, g, loss2);
-      }
-      // Hd' columns: their last readers (W2-gradient MMAs of tile i-1) were issued before the x MMAs of
-      // tile i and are covered by fwd_full; 2 dA | dB columns: released by the commit after the W1 / W3
-      // gradient MMAs of tile i-1
-      if (i > 0) { mbar_wait(&opnd_free, (i - 1) & 1); tc_fence_after(); }
-      tmem_st_x8(lane_base + C_OA + 8 * kh, pa);
-      tmem_st_x8(lane_base + C_OB + 8 * kh, pb);
-      tmem_st_x8(lane_base + C_OH + 8 * kh, ph);
-      tc_wait_st();
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&opnd_ready);
-    }
-    // ---- flush the gradient accumulators: one fp32 partial slice per CTA ----
-    mbar_wait(&grad_done, 0);
-    tc_fence_after();
     const size_t me = (size_t)nh * H * HD;
-    const size_t row = ((size_t)h * H + (size_t)slice * HS + j) * HD;
-    float* Pset = P + (size_t)split * 3 * me;
-    const uint32_t gcol[3] = {C_G1, C_G2, C_G3};
+    int gi = 0, seg = 0;
+    while (gi < total) {
+      int pair, t0;
+      locate(gi, pair, t0);
+      const int n = min(total - gi, tiles_total - t0);
+      uint64_t loss2 = 0ull;
+      for (int i = 0; i < n; ++i, ++gi) {
+        const int s = gi % STAGES;
+        mbar_wait(&fwd_full, gi & 1);
+        mbar_wait(&full[s], (gi / STAGES) & 1);              // acquire of the loader's -eta slot
+        tc_fence_after();
+        const uint2* nes = reinterpret_cast<const uint2*>(&ne_s[s][16 * kh]);
+        uint32_t rx[16], rb[16], rg[16];
+        tmem_ld_x16(lane_base + C_X + 16 * kh, rx);
+        tmem_ld_x16(lane_base + C_B + 16 * kh, rb);
+        tmem_ld_x16(lane_base + C_G + 16 * kh, rg);
+        tc_wait_ld();
+        tc_fence_before();
+        asm volatile("bar.sync 1, 256;" ::: "memory");       // every warp holds its x | b | g
+        if (ew == 0 && lane == 0) mbar_arrive(&xbg_free);
+        uint32_t pa[8], pb[8], ph[8];
 #pragma unroll
-    for (int mat = 0; mat < 3; ++mat) {                    // this warp: columns 64 kh .. 64 kh + 63
-      const float sc = mat == 0 ? 0.5f : 1.0f;             // G1 was accumulated from 2 dA
+        for (int c = 0; c < 16; c += 2) {
+          const uint64_t x = fmul2(pack2u(rx[c], rx[c + 1]), HALF2);   // a / 2
+          const uint64_t bb = pack2u(rb[c], rb[c + 1]);
+          const uint2 nev = nes[c >> 1];
+          const uint64_t ne = pack2u(nev.x, nev.y);
+          const uint64_t g = fmul2(ne, pack2u(rg[c], rg[c + 1]));   // dHd = (-eta v) W2^T
+          float x0, x1;
+          unpack2(x, x0, x1);
+          const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
+          const uint64_t S = ffma2(x, th, x);                  // SiLU(a) = a sigmoid(a), a = 2 x
+          const uint64_t p = fadd2(th, ONE2);                  // 2 sigmoid(a)
+          const uint64_t m = ffma2(th, NONE2, ONE2);           // 2 (1 - sigmoid(a))
+          const uint64_t t2 = ffma2(S, m, p);                  // 2 SiLU'(a)
+          const uint64_t hdv = fmul2(S, bb);                   // hidden activation Hd
+          pa[c >> 1] = pack_bf16x2_from2(fmul2(fmul2(g, bb), t2));   // 2 dA
+          pb[c >> 1] = pack_bf16x2_from2(fmul2(g, S));               // dB
+          ph[c >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));            // Hd' = -eta Hd
+          if (LOSS) loss2 = ffma2(hdv, g, loss2);
+        }
+        // Hd' columns: their last readers (W2-gradient MMAs of the previous tile) were issued before the x
+        // MMAs of this tile and are covered by fwd_full; 2 dA | dB columns: released by the commit after
+        // the W1 / W3 gradient MMAs of the previous tile
+        if (gi > 0) { mbar_wait(&opnd_free, (gi - 1) & 1); tc_fence_after(); }
+        tmem_st_x8(lane_base + C_OA + 8 * kh, pa);
+        tmem_st_x8(lane_base + C_OB + 8 * kh, pb);
+        tmem_st_x8(lane_base + C_OH + 8 * kh, ph);
+        tc_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&opnd_ready);
+      }
+      // ---- flush the segment's gradient accumulators: one fp32 partial slice ----
+      mbar_wait(&grad_done, seg & 1);
+      tc_fence_after();
+      const int h = pair / nslices, slice = pair % nslices;
+      // ordinal of this segment within its pair = this CTA's index among the CTAs that touch the pair
+      int ord;
+      {
+        const long long target = (long long)pair * tiles_total, n_cta = gridDim.x;
+        long long c1 = target * n_cta / U;
+        while (c1 > 0 && (c1 * U) / n_cta > target) --c1;
+        while (((c1 + 1) * U) / n_cta <= target) ++c1;
+        ord = (int)(blockIdx.x - c1);
+      }
+      const bool pair_done = t0 + n == tiles_total;          // zero-fill the sets no segment writes
+      const size_t row = ((size_t)h * H + (size_t)slice * HS + j) * HD;
+      const uint32_t gcol[3] = {C_G1, C_G2, C_G3};
 #pragma unroll
-      for (int cc = 0; cc < 4; ++cc) {
-        uint32_t r[16];
-        if (ntiles > 0) {
+      for (int mat = 0; mat < 3; ++mat) {                    // this warp: columns 64 kh .. 64 kh + 63
+        const float sc = mat == 0 ? 0.5f : 1.0f;             // G1 was accumulated from 2 dA
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc) {
+          uint32_t r[16];
           tmem_ld_x16(lane_base + gcol[mat] + 64 * kh + 16 * cc, r);
           tc_wait_ld();
-        } else {
+          const size_t e = mat * me + row + 64 * kh + 16 * cc;
+          float4* dst = reinterpret_cast<float4*>(P + (size_t)ord * 3 * me + e);
 #pragma unroll
-          for (int u = 0; u < 16; ++u) r[u] = 0u;
+          for (int v = 0; v < 4; ++v)
+            dst[v] = make_float4(sc * __uint_as_float(r[4 * v]), sc * __uint_as_float(r[4 * v + 1]),
+                                 sc * __uint_as_float(r[4 * v + 2]), sc * __uint_as_float(r[4 * v + 3]));
+          if (pair_done)
+            for (int z = ord + 1; z < nsets; ++z) {
+              float4* zd = reinterpret_cast<float4*>(P + (size_t)z * 3 * me + e);
+#pragma unroll
+              for (int v = 0; v < 4; ++v) zd[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
         }
-        float4* dst = reinterpret_cast<float4*>(Pset + mat * me + row + 64 * kh + 16 * cc);
-#pragma unroll
-        for (int v = 0; v < 4; ++v)
-          dst[v] = make_float4(sc * __uint_as_float(r[4 * v]), sc * __uint_as_float(r[4 * v + 1]),
-                               sc * __uint_as_float(r[4 * v + 2]), sc * __uint_as_float(r[4 * v + 3]));
       }
-    }
-    if (LOSS) {
-      float l0, l1;
-      unpack2(loss2, l0, l1);
-      float loss = l0 + l1;
+      tc_fence_before();
+      if (LOSS) {
+        float l0, l1;
+        unpack2(loss2, l0, l1);
+        float loss = l0 + l1;
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) loss += __shfl_xor_sync(0xffffffffu, loss, o);
-      if (lane == 0) loss_red[ew] = loss;
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-      if (ew == 0 && lane == 0) {
-        float t = 0.f;
-        for (int w = 0; w < EPI_WARPS; ++w) t += loss_red[w];
-        loss_part[((size_t)split * nslices + slice) * nh + h] = t;
+        for (int o = 16; o > 0; o >>= 1) loss += __shfl_xor_sync(0xffffffffu, loss, o);
+        if (lane == 0) loss_red[ew] = loss;
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        if (ew == 0 && lane == 0) {
+          float t = 0.f;
+          for (int w = 0; w < EPI_WARPS; ++w) t += loss_red[w];
+          loss_part[((size_t)ord * nslices + slice) * nh + h] = t;
+          if (pair_done)
+            for (int z = ord + 1; z < nsets; ++z) loss_part[((size_t)z * nslices + slice) * nh + h] = 0.f;
+        }
+        asm volatile("bar.sync 1, 256;" ::: "memory");
       }
+      ++seg;
     }
   }
   tc_fence_before();
@@ -325,11 +372,43 @@ int bf16_update_wide_supported(const ttt_config* cfg) {
   return cfg->hd == updw::HD && cfg->hidden % updw::HS == 0 && !cfg->linear_fast_weight;
 }
 
-// appends `splits` partial-gradient sets; split geometry (tiles of 32 tokens) comes from the caller
+// CTAs of the launch and partial sets it writes: units = pairs x tiles spread evenly over the SMs;
+// nsets = the largest number of CTAs whose range touches one (head, slice) pair
+static void wide_geometry(const ttt_ctx* ctx, int64_t M, int* tiles, int* ncta, int* nsets) {
+  const int t = (int)((M + updw::T - 1) / updw::T);
+  const int pairs = ctx->cfg.nh * (ctx->cfg.hidden / updw::HS);
+  const long long U = (long long)pairs * t;
+  int n = ctx->sm_count;
+  if (n > U) n = (int)U;
+  if (n < 1) n = 1;
+  int worst = 1;
+  for (int p = 0; p < pairs && U > 0; ++p) {
+    // first CTA with hi(c) > p t, last CTA with lo(c) < (p + 1) t
+    long long c0 = (long long)p * t * n / U;
+    while (c0 > 0 && (c0 * U) / n > (long long)p * t) --c0;
+    while (((c0 + 1) * U) / n <= (long long)p * t) ++c0;
+    long long c1 = c0;
+    while (c1 + 1 < n && ((c1 + 1) * U) / n < (long long)(p + 1) * t) ++c1;
+    if ((int)(c1 - c0 + 1) > worst) worst = (int)(c1 - c0 + 1);
+  }
+  *tiles = t;
+  *ncta = n;
+  *nsets = worst;
+}
+
+int bf16_wide_partials_needed(const ttt_ctx* ctx, int64_t M) {
+  int t, n, s;
+  wide_geometry(ctx, M, &t, &n, &s);
+  return s;
+}
+
+// appends `*used` partial-gradient sets, `*loss_rows` loss partial rows
 int bf16_accumulate_wide(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V, const float* lr,
-                         int64_t M, int64_t ld, bool want_loss, int tiles, int tps, int splits,
+                         int64_t M, int64_t ld, bool want_loss, int* used, int* loss_rows,
                          cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
+  int tiles, ncta, nsets;
+  wide_geometry(ctx, M, &tiles, &ncta, &nsets);
   CUtensorMap mapK, mapV, mapW;
   int rc = make_token_map(ctx, &mapK, K, M, (int64_t)c.nh * c.hd, ld, updw::T);
   if (rc != TTT_OK) return rc;
@@ -349,14 +428,15 @@ int bf16_accumulate_wide(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat
     attr_set = true;
   }
   float* P = ctx->partials + (size_t)ctx->n_partials * 3 * ctx->mat_elems;
-  dim3 grid(splits, c.hidden / updw::HS, c.nh);
   if (want_loss)
-    bf16_update_wide_kernel<true><<<grid, updw::THREADS, updw::SMEM_BYTES, s>>>(
-        mapK, mapV, mapW, lr, P, ctx->loss_part, (int)M, c.nh, c.hidden, tiles, tps);
+    bf16_update_wide_kernel<true><<<ncta, updw::THREADS, updw::SMEM_BYTES, s>>>(
+        mapK, mapV, mapW, lr, P, ctx->loss_part, (int)M, c.nh, c.hidden, tiles, nsets);
   else
-    bf16_update_wide_kernel<false><<<grid, updw::THREADS, updw::SMEM_BYTES, s>>>(
-        mapK, mapV, mapW, lr, P, ctx->loss_part, (int)M, c.nh, c.hidden, tiles, tps);
+    bf16_update_wide_kernel<false><<<ncta, updw::THREADS, updw::SMEM_BYTES, s>>>(
+        mapK, mapV, mapW, lr, P, ctx->loss_part, (int)M, c.nh, c.hidden, tiles, nsets);
   TTT_LAUNCH_CHECK(ctx, "bf16_update_wide_kernel");
+  *used = nsets;
+  *loss_rows = nsets * (c.hidden / updw::HS);
   return TTT_OK;
 }
 

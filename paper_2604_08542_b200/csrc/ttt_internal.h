@@ -107,8 +107,9 @@ int bf16_apply_wide(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int6
 // hd = 128 update kernel (bf16_update_wide.cu)
 int bf16_update_wide_supported(const ttt_config* cfg);
 int bf16_accumulate_wide(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V, const float* lr,
-                         int64_t M, int64_t ld, bool want_loss, int tiles, int tps, int splits,
+                         int64_t M, int64_t ld, bool want_loss, int* used, int* loss_rows,
                          cudaStream_t s);
+int bf16_wide_partials_needed(const ttt_ctx* ctx, int64_t M);
 // strided bf16 [M][cols] (row stride ld) <-> dense fp32 [M][cols]
 int launch_bf16_to_f32(ttt_ctx* ctx, const __nv_bfloat16* src, int64_t ld, float* dst, int64_t M, cudaStream_t s);
 int launch_f32_to_bf16(ttt_ctx* ctx, const float* src, __nv_bfloat16* dst, int64_t ld, int64_t M, cudaStream_t s);
