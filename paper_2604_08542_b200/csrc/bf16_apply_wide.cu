@@ -75,6 +75,8 @@ bf16_apply_wide_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_co
   tc_fence_after();
   const uint32_t tb = tmem_base_s;
   if (tb != 0) __trap();      // all 512 columns belong to this CTA: absolute columns below
+  // programmatic dependent launch: everything above overlapped the tail of the commit kernel
+  asm volatile("griddepcontrol.wait;" ::: "memory");
 
   if (warp == 0) {
     // ===================== TMA producer =====================
@@ -248,8 +250,19 @@ int bf16_apply_wide(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int6
   }
   int grid = c.nh * npairs;
   if (grid > ctx->sm_count) grid = ctx->sm_count;      // persistent CTAs, units round-robin
-  bf16_apply_wide_kernel<<<grid, appw::THREADS, appw::SMEM_BYTES, s>>>(mapW, mapQ, O, (int)M, ld, c.nh,
-                                                                      c.hidden, npairs);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(appw::THREADS);
+  cfg.dynamicSmemBytes = appw::SMEM_BYTES;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  int Mi = (int)M, nh = c.nh, H = c.hidden;
+  cudaError_t e = cudaLaunchKernelEx(&cfg, bf16_apply_wide_kernel, mapW, mapQ, O, Mi, ld, nh, H, npairs);
+  if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, "bf16_apply_wide_kernel launch", e);
   TTT_LAUNCH_CHECK(ctx, "bf16_apply_wide_kernel");
   return TTT_OK;
 }

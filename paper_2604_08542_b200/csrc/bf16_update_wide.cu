@@ -301,6 +301,8 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
         __syncwarp();
         if (lane == 0) mbar_arrive(&opnd_ready);
       }
+      // a dependent kernel (PDL) may be scheduled from here on; it still waits for this grid to finish
+      if (gi >= total) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
       // ---- flush the segment's gradient accumulators: one fp32 partial slice ----
       mbar_wait(&grad_done, seg & 1);
       tc_fence_after();

@@ -140,6 +140,8 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
   NSW_TR(0);
   if (tid == 0) { mbar_init(&mma_bar, 1); fence_mbar_init(); }
   if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  // programmatic dependent launch: the set-up above overlapped the tail of the gradient kernel
+  asm volatile("griddepcontrol.wait;" ::: "memory");
 
   // ---- load (coalesced): g = (use_G ? G : 0) + sum_s P[s] (fixed order); Frobenius norm over the cluster ----
   float4 g[8];
@@ -323,6 +325,7 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
       if (!last) {
         split_row32(x, XH, XL, trow, cs);
       } else {
+        asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
         // coalesced write-out through the staging tile: fused commit W <- W - NS(g) (Eq. 8), or NS(g) -> G
         rows_to_ex(x);
         worker_bar();
@@ -374,13 +377,15 @@ int launch_ns_tc_wide(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s) {
   cfg.blockDim = dim3(nsw::LAUNCH_THREADS);
   cfg.dynamicSmemBytes = nsw::SMEM_BYTES;
   cfg.stream = s;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = nc;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = 1;
+  cfg.numAttrs = 2;
   float* G = ctx->G;
   const float* P = ctx->partials;
   int n_sets = ctx->n_partials, use_G = ctx->G_valid ? 1 : 0, H = c.hidden, iters = c.ns_iters;
