@@ -247,7 +247,9 @@ def run_ours(args, w, rank, local_rank, world):
     traffic = {"cfg2": 48133632 + 442880, "cfg4": 187704320 + 6952704}.get(w.name)
     # (the per-kernel pass calls ttt_accumulate / ttt_commit / ttt_apply separately; inside
     #  ttt_chunk_step the plain commit is fused into the update kernel's tail)
-    roofline = {"kernel": "bf16_update_kernel" if w.act_dtype == "bf16" else "f32 path",
+    upd_kernel = ("bf16_update_wide_kernel" if w.hd == 128 else "bf16_update_kernel") \
+        if w.act_dtype == "bf16" else "f32 path"
+    roofline = {"kernel": upd_kernel,
                 "bound": "tensor", "achieved": upd_tflops, "peak": peaks["bf16_tflops"],
                 "unit": "TFLOP/s", "frac": upd_tflops / peaks["bf16_tflops"], "traffic": traffic,
                 "peak_source": peaks["source"] + ", burst figure (step is tens of microseconds)",

@@ -70,7 +70,9 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
   const long long U = (long long)nh * nslices * tiles_total;
   const long long lo = blockIdx.x * U / gridDim.x, hi = (blockIdx.x + 1) * U / gridDim.x;
   const int total = (int)(hi - lo);                 // tiles this CTA processes, over all its segments
-  // unit lo + gi -> pair (= h * nslices + slice) and token tile
+  // unit lo + gi -> pair (= slice * nh + h) and token tile. Slice-major pairs: when nh divides the
+  // CTAs-per-pair pattern (config 5: 4.625 CTAs per pair, nh = 8) the slices of one head walk the
+  // same token tiles at the same time, so K / V come from DRAM once and from L2 three times
   auto locate = [&](int gi, int& pair, int& tile) {
     const long long u = lo + gi;
     pair = (int)(u / tiles_total);
@@ -79,7 +81,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
   auto load_stage = [&](int gi) {
     int pair, tile;
     locate(gi, pair, tile);
-    const int s = gi % STAGES, h = pair / nslices, row = tile * T;
+    const int s = gi % STAGES, h = pair % nh, row = tile * T;
     mbar_arrive_expect_tx(&full[s], STAGE_BYTES);
     uint8_t* dst = ring + s * STAGE_BYTES;
     tma_load_2d(dst, &mapK, &full[s], h * HD, row);
@@ -89,7 +91,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
   };
   // weights of a pair: mat m (0 = W1^T, 1 = W2, 2 = W3^T), hd half c -> [128 rows x 64] sub-tile
   auto load_weights = [&](int pair) {
-    const int h = pair / nslices, slice = pair % nslices;
+    const int h = pair % nh, slice = pair / nh;
     mbar_arrive_expect_tx(&w_full, W_BYTES);
     for (int m = 0; m < 3; ++m)
       for (int c = 0; c < 2; ++c)
@@ -218,7 +220,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
           int pair, tile;
           locate(g0 + u, pair, tile);
           const int t = tile * T + lane;
-          if (t < M) x = -__ldg(lr + (size_t)(pair / nslices) * M + t);
+          if (t < M) x = -__ldg(lr + (size_t)(pair % nh) * M + t);
         }
         v[u] = x;
       }
@@ -306,7 +308,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
       // ---- flush the segment's gradient accumulators: one fp32 partial slice ----
       mbar_wait(&grad_done, seg & 1);
       tc_fence_after();
-      const int h = pair / nslices, slice = pair % nslices;
+      const int h = pair % nh, slice = pair / nh;
       // ordinal of this segment within its pair = this CTA's index among the CTAs that touch the pair
       int ord;
       {
