@@ -51,15 +51,16 @@ typedef enum {
 
 typedef enum {
   TTT_F32 = 0,  /* Q,K,V,O fp32; every contraction in fp32 FFMA (parity config 1, tol 1e-4)   */
-  TTT_BF16 = 1  /* Q,K,V,O bf16, fp32 master weights. hd = 64 and hidden 128|256: tcgen05 bf16
-                   MMAs with fp32 accumulation; other shapes (hd % 8 == 0, e.g. hd = 128): the fp32
-                   CUDA-core kernels behind a bf16 <-> fp32 conversion (same semantics)        */
+  TTT_BF16 = 1  /* Q,K,V,O bf16, fp32 master weights. hd = 64 with hidden 128|256 and hd = 128 with
+                   hidden a multiple of 128: tcgen05 bf16 MMAs with fp32 accumulation; other shapes
+                   (hd % 8 == 0): the fp32 CUDA-core kernels behind a bf16 <-> fp32 conversion
+                   (same semantics)                                                             */
 } ttt_dtype;
 
 typedef struct {
   int32_t nh;                 /* heads (independent fast-weight sets, Eq. 13)    */
   int32_t hd;                 /* head dimension <= 128; bf16: multiple of 8; f32: multiple of 4 */
-  int32_t hidden;             /* H = hd*k, multiple of 4 (tensor path: 128 or 256)             */
+  int32_t hidden;             /* H = hd*k, multiple of 4 (tensor paths: see ttt_dtype)           */
   int32_t act_dtype;          /* ttt_dtype of Q,K,V,O                                          */
   int32_t ns_iters;           /* 0 = plain gradient step (Eq. 8); n>0 = n Newton-Schulz iters  */
   int32_t renorm;             /* 0/1: restore each unit's fan-in 2-norm of ttt_init after update */
