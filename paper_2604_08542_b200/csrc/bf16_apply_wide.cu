@@ -3,15 +3,19 @@
 //
 // Tokens on the 128 TMEM lanes as in bf16_apply.cu. At hd = 128 a head's weights (3 x H x 128 bf16,
 // 393 KB at H = 512) no longer fit in shared memory, so they are streamed: a persistent CTA takes
-// units of (head, two 128-token tiles), keeps the two Q tiles in shared memory and both O
+// units of (head, two 128-token tiles), keeps both Q tiles in shared memory and both O
 // accumulators in TMEM, and walks the hidden dimension in steps of 64 units through a ring of
 // weight stages ([W1^T | W3^T] rows as one N = 128 B operand, W2 rows as the MN-major B operand of
 // the down projection). Every streamed weight byte is used by 256 tokens.
-//   TMEM: O(0) | O(1) fp32 [128 x 128] at columns 0 / 128, forward accumulators x | b of tile t at
-//   256 + 128 t; the bf16 hidden activation Hq (A operand of the down MMAs) overwrites the first 32
-//   columns of its own x once every epilogue warp holds its x | b in registers.
+//   TMEM (512 columns): O(t) fp32 [128 x 128] at 128 t; forward accumulators x | b of tile t
+//   (64 + 64 columns) at 256 + 128 t; the bf16 hidden activation Hq (A operand of the down MMAs)
+//   overwrites the first 32 columns of its own x once every epilogue warp of the tile holds its
+//   x | b in registers. (Q as a TMEM operand with 32-hidden steps was built and measured: the
+//   F -> epilogue -> D -> F chain of a tile is latency-bound and the shorter steps lose, 147 vs 131 us.)
 //   MMA order per step n: D(0,n) F(0,n+1) D(1,n) F(1,n+1) — the forward MMAs of one tile run while
-//   the epilogue works on the other tile; in-order execution makes the re-use of x safe.
+//   the other tile's epilogue works; in-order execution makes the re-use of x safe.
+//   Warps: TMA producer, MMA issuer, two epilogue groups of 8 warps, one per tile (SwiGLU
+//   epilogue per step, O -> bf16 -> global).
 #include <stdio.h>
 
 #include "tc_common.cuh"
@@ -27,8 +31,8 @@ constexpr int HD = 128;        // head dimension
 constexpr int TM = 128;        // tokens per tile (MMA M)
 constexpr int HSTEP = 64;      // hidden units per step
 constexpr int NST = 3;         // weight ring stages
-constexpr int EPI_WARPS = 16;
-constexpr int THREADS = (4 + EPI_WARPS) * 32;
+constexpr int GRP_WARPS = 8;   // epilogue warps per tile
+constexpr int THREADS = (4 + 2 * GRP_WARPS) * 32;
 constexpr int QSUB_BYTES = TM * 128;            // [128 tokens x 64] bf16 sub-tile (half of hd)
 constexpr int QTILE_BYTES = 2 * QSUB_BYTES;
 constexpr int BOX_BYTES = HSTEP * 128;          // one TMA box of weights: [64 rows x 64]
@@ -61,9 +65,9 @@ bf16_apply_wide_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_co
       mbar_init(&q_full[t], 1);
       mbar_init(&q_free[t], 1);
       mbar_init(&f_full[t], 1);
-      mbar_init(&hq_ready[t], EPI_WARPS);
+      mbar_init(&hq_ready[t], GRP_WARPS);
       mbar_init(&o_full[t], 1);
-      mbar_init(&o_free[t], EPI_WARPS);
+      mbar_init(&o_free[t], GRP_WARPS);
     }
     fence_mbar_init();
     tma_prefetch_desc(&mapW);
@@ -85,7 +89,7 @@ bf16_apply_wide_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_co
       for (int u = 0, unit = blockIdx.x; unit < nunits; unit += gridDim.x, ++u) {
         const int h = unit / npairs, p = unit % npairs;
         for (int t = 0; t < 2; ++t) {
-          if (u > 0) mbar_wait(&q_free[t], (u - 1) & 1);
+          if (u > 0) mbar_wait(&q_free[t], (u - 1) & 1);     // the forward MMAs of the tile's previous unit are done
           mbar_arrive_expect_tx(&q_full[t], QTILE_BYTES);
           for (int c = 0; c < 2; ++c)
             tma_load_2d(smem + t * QTILE_BYTES + c * QSUB_BYTES, &mapQ, &q_full[t], h * HD + c * 64,
@@ -109,9 +113,9 @@ bf16_apply_wide_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_co
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (elect_one()) {
-      constexpr uint32_t idesc_f = umma_idesc_bf16(TM, 128, 0, 0);    // A = Q (smem), B = [W1^T | W3^T] rows
-      constexpr uint32_t idesc_d = umma_idesc_bf16(TM, HD, 0, 1);     // A = Hq (TMEM), B = W2 rows, MN-major
+      constexpr uint32_t idesc_f = umma_idesc_bf16(TM, 2 * HSTEP, 0, 0);   // A = Q (smem), B = [W1^T | W3^T] rows
       const uint64_t dq = umma_smem_desc_sw128(sbase, 16, 1024);
+      constexpr uint32_t idesc_d = umma_idesc_bf16(TM, HD, 0, 1);          // A = Hq (TMEM), B = W2 rows, MN-major
       const uint64_t dwf = umma_smem_desc_sw128(sbase + 2 * QTILE_BYTES, 16, 1024);
       const uint64_t dw2 = umma_smem_desc_sw128(sbase + 2 * QTILE_BYTES + W2_OFF, BOX_BYTES, 1024);
       auto issueF = [&](int t, int s) {      // x | b of tile t <- Q(t) [W1^T | W3^T]^T of ring stage s
@@ -157,55 +161,56 @@ bf16_apply_wide_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_co
       }
     }
   } else if (warp >= 4) {
-    // ===================== epilogue warps =====================
-    const int ew = warp - 4, q = warp & 3, cg = ew >> 2;   // lane quadrant, 16-hidden / 32-output column group
+    // ===================== epilogue warps: group t = one token tile =====================
+    const int ew = warp - 4, t = ew >> 3, q = warp & 3, cg = (ew >> 2) & 1;   // tile, lane quadrant, column half
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
+    const int row = q * 32 + lane;                         // token row of the tile = TMEM lane
     const uint64_t HALF2 = pack2(0.5f, 0.5f);
+    const uint32_t buf = lane_base + C_F + t * 128;
     for (int u = 0, unit = blockIdx.x; unit < nunits; unit += gridDim.x, ++u) {
       const int h = unit / npairs, p = unit % npairs;
       for (int n = 0; n < nstep; ++n) {
-#pragma unroll
-        for (int t = 0; t < 2; ++t) {
-          mbar_wait(&f_full[t], (u * nstep + n) & 1);
-          tc_fence_after();
-          const uint32_t buf = lane_base + C_F + t * 128;
-          uint32_t rx[16], rb[16];
-          tmem_ld_x16(buf + 16 * cg, rx);
-          tmem_ld_x16(buf + 64 + 16 * cg, rb);
-          tc_wait_ld();
-          tc_fence_before();
-          asm volatile("bar.sync 1, 512;" ::: "memory");   // every warp holds its x | b: x may be overwritten
-          uint32_t ph[8];
-#pragma unroll
-          for (int c = 0; c < 16; c += 2) {
-            const uint64_t x = fmul2(pack2u(rx[c], rx[c + 1]), HALF2);   // a / 2
-            float x0, x1;
-            unpack2(x, x0, x1);
-            const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
-            const uint64_t S = ffma2(x, th, x);                          // SiLU(a) = a/2 (1 + tanh(a/2))
-            ph[c >> 1] = pack_bf16x2_from2(fmul2(S, pack2u(rb[c], rb[c + 1])));
-          }
-          tmem_st_x8(buf + 8 * cg, ph);
-          tc_wait_st();
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(&hq_ready[t]);
-        }
-      }
-      // ---- O(t) -> bf16 -> global: this thread owns token row q*32+lane, columns 32 cg .. 32 cg + 31 ----
-#pragma unroll
-      for (int t = 0; t < 2; ++t) {
-        mbar_wait(&o_full[t], u & 1);
+        mbar_wait(&f_full[t], (u * nstep + n) & 1);
         tc_fence_after();
-        uint32_t ro[32];
-        tmem_ld_x32(lane_base + C_O + t * 128 + 32 * cg, ro);
+        uint32_t rx[32], rb[32];
+        tmem_ld_x32(buf + 32 * cg, rx);
+        tmem_ld_x32(buf + 64 + 32 * cg, rb);
         tc_wait_ld();
         tc_fence_before();
+        // every warp of the tile holds its x | b: x may be overwritten (named barrier 1 + t, 8 warps)
+        asm volatile("bar.sync %0, 256;" ::"r"(1 + t) : "memory");
+        uint32_t ph[16];
+#pragma unroll
+        for (int c = 0; c < 32; c += 2) {
+          const uint64_t x = fmul2(pack2u(rx[c], rx[c + 1]), HALF2);   // a / 2
+          float x0, x1;
+          unpack2(x, x0, x1);
+          const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
+          const uint64_t S = ffma2(x, th, x);                          // SiLU(a) = a/2 (1 + tanh(a/2))
+          ph[c >> 1] = pack_bf16x2_from2(fmul2(S, pack2u(rb[c], rb[c + 1])));
+        }
+        tmem_st_x16(buf + 16 * cg, ph);
+        tc_wait_st();
+        tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(&o_free[t]);
-        const int64_t tok = (int64_t)(2 * p + t) * TM + q * 32 + lane;
+        if (lane == 0) mbar_arrive(&hq_ready[t]);
+      }
+      // ---- O(t) -> bf16 -> global: this thread owns token row `row`, columns 64 cg .. 64 cg + 63 ----
+      mbar_wait(&o_full[t], u & 1);
+      tc_fence_after();
+      const int64_t tok = (int64_t)(2 * p + t) * TM + row;
+#pragma unroll
+      for (int half = 0; half < 2; ++half) {
+        uint32_t ro[32];
+        tmem_ld_x32(lane_base + C_O + t * 128 + 64 * cg + 32 * half, ro);
+        tc_wait_ld();
+        if (half == 1) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&o_free[t]);
+        }
         if (tok < M) {
-          uint4* dst = reinterpret_cast<uint4*>(O + tok * ld + h * HD + 32 * cg);
+          uint4* dst = reinterpret_cast<uint4*>(O + tok * ld + h * HD + 64 * cg + 32 * half);
 #pragma unroll
           for (int v = 0; v < 4; ++v) {
             uint4 w;
