@@ -150,13 +150,21 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
 #pragma unroll
     for (int k = 0; k < 8; ++k)
       g[k] = use_G ? reinterpret_cast<const float4*>(G + blk)[tid + THREADS * k] : make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int s = 0; s < n_sets; ++s) {
-      const float4* ps = reinterpret_cast<const float4*>(P + (size_t)s * set_elems + blk);
-      float4 p[8];
+    for (int s = 0; s < n_sets; s += 2) {              // two sets in flight, summed in set order
+      const float4* p0 = reinterpret_cast<const float4*>(P + (size_t)s * set_elems + blk);
+      const float4* p1 = reinterpret_cast<const float4*>(P + (size_t)(s + 1) * set_elems + blk);
+      const bool two = s + 1 < n_sets;
+      float4 a[8], b[8];
 #pragma unroll
-      for (int k = 0; k < 8; ++k) p[k] = __ldcg(ps + tid + THREADS * k);
+      for (int k = 0; k < 8; ++k) {
+        a[k] = __ldcg(p0 + tid + THREADS * k);
+        b[k] = two ? __ldcg(p1 + tid + THREADS * k) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
 #pragma unroll
-      for (int k = 0; k < 8; ++k) { g[k].x += p[k].x; g[k].y += p[k].y; g[k].z += p[k].z; g[k].w += p[k].w; }
+      for (int k = 0; k < 8; ++k) {
+        g[k].x = (g[k].x + a[k].x) + b[k].x; g[k].y = (g[k].y + a[k].y) + b[k].y;
+        g[k].z = (g[k].z + a[k].z) + b[k].z; g[k].w = (g[k].w + a[k].w) + b[k].w;
+      }
     }
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
@@ -264,23 +272,30 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
       float4* dst = reinterpret_cast<float4*>(sc_mat + ((size_t)rank * 2 + (it & 1)) * RB * HD);
 #pragma unroll
       for (int k = 0; k < 8; ++k) dst[tid + THREADS * k] = *reinterpret_cast<const float4*>(ex_co(k));
-      __threadfence();
     }
     NSW_TR(3 + it * 8);
-    cluster_arrive();                  // release: this rank's partial is in global memory
+    cluster_arrive();                  // release at cluster scope: orders this rank's global writes for its peers
     cluster_wait();
     NSW_TR(4 + it * 8);
     if (!issuer) {
       float4 a[8];
 #pragma unroll
       for (int k = 0; k < 8; ++k) a[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-      for (uint32_t r = 0; r < nc; ++r) {                  // rank order: identical A on every rank
-        const float4* src = reinterpret_cast<const float4*>(sc_mat + ((size_t)r * 2 + (it & 1)) * RB * HD);
-        float4 p[8];
+      for (uint32_t r = 0; r < nc; r += 2) {               // rank order: identical A on every rank
+        const float4* s0 = reinterpret_cast<const float4*>(sc_mat + ((size_t)r * 2 + (it & 1)) * RB * HD);
+        const float4* s1 = reinterpret_cast<const float4*>(sc_mat + ((size_t)(r + 1) * 2 + (it & 1)) * RB * HD);
+        const bool two = r + 1 < nc;
+        float4 p[8], p2[8];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) p[k] = __ldcg(src + tid + THREADS * k);
+        for (int k = 0; k < 8; ++k) {
+          p[k] = __ldcg(s0 + tid + THREADS * k);
+          p2[k] = two ? __ldcg(s1 + tid + THREADS * k) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
 #pragma unroll
-        for (int k = 0; k < 8; ++k) { a[k].x += p[k].x; a[k].y += p[k].y; a[k].z += p[k].z; a[k].w += p[k].w; }
+        for (int k = 0; k < 8; ++k) {
+          a[k].x = (a[k].x + p[k].x) + p2[k].x; a[k].y = (a[k].y + p[k].y) + p2[k].y;
+          a[k].z = (a[k].z + p[k].z) + p2[k].z; a[k].w = (a[k].w + p[k].w) + p2[k].w;
+        }
       }
 #pragma unroll
       for (int k = 0; k < 8; ++k) *reinterpret_cast<float4*>(ex_co(k)) = a[k];
