@@ -132,6 +132,10 @@ def _bf16_workload(base, **kw):
     ("cfg3", dict(nh=2, tokens_per_frame=257, frames_per_chunk=2, n_frames=6)),
     # re-normalised plain update, L2-normalised K, 4 chunks with a short last chunk
     ("cfg4", dict(nh=3, tokens_per_frame=190, frames_per_chunk=2, n_frames=7)),
+    # hd = 128 kernels: Newton-Schulz + re-normalisation (NS result left in G, generic commit), 3 chunks
+    ("cfg5", dict(nh=2, hidden=256, renorm=1, tokens_per_frame=150, frames_per_chunk=3, n_frames=9)),
+    # hd = 128, plain re-normalised update, L2-normalised keys
+    ("cfg4", dict(nh=2, hd=128, hidden=256, tokens_per_frame=210, frames_per_chunk=2, n_frames=6)),
 ])
 def test_bf16_stream_parity(base, kw):
     w = _bf16_workload(base, **kw)
@@ -242,9 +246,10 @@ def test_bf16_apply_only_and_head_independence():
     gpu.close(); g1.close()
 
 
-def test_bf16_bitwise_determinism_and_chunk_step_composition():
+@pytest.mark.parametrize("hd", [64, 128])
+def test_bf16_bitwise_determinism_and_chunk_step_composition(hd):
     dev = torch.device("cuda", 0)
-    w = _bf16_workload("cfg3", nh=2, tokens_per_frame=300, frames_per_chunk=2, n_frames=4)
+    w = _bf16_workload("cfg3", nh=2, hd=hd, tokens_per_frame=300, frames_per_chunk=2, n_frames=4)
     W1, W2, W3 = (x.to(dev) for x in ti.fast_weights(w))
     chunks = [tuple(x.to(dev) for x in c) for c in ti.TokenStream(w)]
     outs = []
@@ -262,11 +267,12 @@ def test_bf16_bitwise_determinism_and_chunk_step_composition():
         assert torch.equal(x, y) and torch.equal(x, z)
 
 
-def test_accumulate_commit_equals_update_on_concatenation():
+@pytest.mark.parametrize("hd", [64, 128])
+def test_accumulate_commit_equals_update_on_concatenation(hd):
     """Eq. 10: accumulate over two chunks at the same W, one commit == update on the concatenation
     (up to the fp32 summation order of the partials)."""
     dev = torch.device("cuda", 0)
-    w = _bf16_workload("cfg2", nh=2, tokens_per_frame=256, frames_per_chunk=2, n_frames=4)
+    w = _bf16_workload("cfg2", nh=2, hd=hd, tokens_per_frame=256, frames_per_chunk=2, n_frames=4)
     W1, W2, W3 = (x.to(dev) for x in ti.fast_weights(w))
     (Q0, K0, V0, l0), (Q1, K1, V1, l1) = [tuple(x.to(dev) for x in c) for c in ti.TokenStream(w)]
     a = _mk(w, max_tokens=2 * w.chunk_tokens); a.ttt_init(W1, W2, W3)
@@ -356,13 +362,22 @@ def test_cfg4_full_size_first_chunks_sampled_head():
     assert max(errs) <= TOL_BF16 and max(errs_w) <= TOL_BF16, (errs, errs_w)
 
 
+def test_cfg5_full_size_first_chunks_sampled_head():
+    """BASELINE.json:configs[4] exactly (8 heads x 128, H 512, 43 856-token chunks, Newton-Schulz), in
+    the launch configuration bench.py times; first 2 of the 32 chunks, one head through the oracle."""
+    errs, errs_w = _full_size_stream("cfg5", 2, [5])
+    assert max(errs) <= TOL_BF16 and max(errs_w) <= TOL_BF16, (errs, errs_w)
+
+
+@pytest.mark.parametrize("hd,H", [(64, 128), (128, 256)])
 @pytest.mark.parametrize("M", [1, 5, 33, 130])
-def test_bf16_tiny_chunks_strided_rows_and_nonuniform_lr(M):
-    """Edge cases of the tensor path: chunks smaller than one update tile (32) / apply tile (128),
-    token rows with padding (ld > nh*hd), per-token learning rates of both signs and zero."""
+def test_bf16_tiny_chunks_strided_rows_and_nonuniform_lr(M, hd, H):
+    """Edge cases of the tensor paths (hd 64 and hd 128 kernels): chunks smaller than one update tile
+    (32) / apply tile (128), token rows with padding (ld > nh*hd), per-token learning rates of both
+    signs and zero."""
     from paper_2604_08542_b200 import TTT, TTT_BF16
     dev = torch.device("cuda", 0)
-    nh, hd, H, ld = 2, 64, 128, 2 * 64 + 24
+    nh, ld = 2, 2 * hd + 24
     g = torch.Generator().manual_seed(100 + M)
     W1 = torch.randn(nh, hd, H, generator=g) / 8
     W2 = torch.randn(nh, H, hd, generator=g) / 8
