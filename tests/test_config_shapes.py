@@ -1,6 +1,8 @@
 """Shape facts the paper states (Eq. 13, Table 3) and the workload table of BASELINE.json."""
 import os
 
+import torch
+
 import ttt_inputs as ti
 
 GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
@@ -51,6 +53,28 @@ def test_streams_are_seeded_and_shaped():
     n = k.float().reshape(32, w.nh, w.hd).norm(dim=-1)
     assert float((n - 1).abs().max()) < 2 ** -7
     assert lr.shape == (w.nh, 32) and abs(float(lr[0, 0]) - w.lr) < 1e-9
+
+
+def test_structured_stream_is_three_projections_of_common_tokens():
+    """Secondary workload: Q, K, V = X P_q, X P_k, X P_v of common AR(1)
+    tokens X: unit marginals, the same frame-to-frame correlation, and K a linear map of Q's
+    source (rank check: [Q K V] of d+8 tokens has rank d, iid streams would have rank d+8)."""
+    w = ti.scaled(ti.CONFIGS["cfg3"], nh=2, hd=16, hidden=32, act_dtype="f32", tokens_per_frame=40,
+                  frames_per_chunk=1, n_frames=3, structured=True)
+    ch = list(ti.TokenStream(w))
+    q, k, v, lr = ch[0]
+    assert q.shape == (40, 32) and lr.shape == (2, 40)
+    stacked = torch.cat([q, k, v], dim=1).double()              # [40, 96] = X [40, 32] @ [P_q P_k P_v]
+    assert torch.linalg.matrix_rank(stacked, tol=1e-4) == 32
+    iid = ti.scaled(w, structured=False)
+    q2, k2, v2, _ = ti.TokenStream(iid).next_chunk()
+    assert torch.linalg.matrix_rank(torch.cat([q2, k2, v2], dim=1).double(), tol=1e-4) == 40
+    big = ti.scaled(w, tokens_per_frame=600, frames_per_chunk=2, n_frames=2)
+    qq, kk, vv, _ = ti.TokenStream(big).next_chunk()
+    for x in (qq, kk, vv):
+        assert abs(float(x.std()) - 1.0) < 0.05
+        f = x.reshape(2, 600, -1)
+        assert abs(float((f[0] * f[1]).mean() / (f[0].std() * f[1].std())) - 0.9) < 0.05
 
 
 def test_sharding_helpers_cover_everything_once():

@@ -136,6 +136,10 @@ def _bf16_workload(base, **kw):
     ("cfg5", dict(nh=2, hidden=256, renorm=1, tokens_per_frame=150, frames_per_chunk=3, n_frames=9)),
     # hd = 128, plain re-normalised update, L2-normalised keys
     ("cfg4", dict(nh=2, hd=128, hidden=256, tokens_per_frame=210, frames_per_chunk=2, n_frames=6)),
+    # secondary "structured" workload: Q, K, V are projections of common AR(1) tokens
+    ("cfg3", dict(nh=2, tokens_per_frame=257, frames_per_chunk=2, n_frames=6, structured=True)),
+    ("cfg5", dict(nh=2, hidden=256, rho=0.9, l2_k=True, tokens_per_frame=150, frames_per_chunk=3,
+                  n_frames=9, structured=True)),
 ])
 def test_bf16_stream_parity(base, kw):
     w = _bf16_workload(base, **kw)

@@ -11,6 +11,11 @@ Streams: base seed s -> independent torch CPU generators seeded s*16 + {0:W1, 1:
 AR(1) over frames with coefficient rho per (position, channel), state carried across
 chunk boundaries; optional per-head L2 normalisation of K rows done in fp32 BEFORE the
 rounding to the activation dtype. lr: the config's constant, as a [nh, M] fp32 array.
+
+Secondary "structured" workload (parity only): Q, K, V are three fixed seeded
+projections X P_q, X P_k, X P_v (P ~ N(0, 1/d), streams 6, 7, 8) of COMMON tokens X (the Q stream's
+AR(1) process) - the relation the paper's module has between its q, k, v (PAPER.md:132, 141);
+marginals stay N(0,1).
 """
 from __future__ import annotations
 
@@ -20,7 +25,7 @@ from typing import Iterator, Optional, Tuple
 
 import torch
 
-_STREAM = {"W1": 0, "W2": 1, "W3": 2, "Q": 3, "K": 4, "V": 5}
+_STREAM = {"W1": 0, "W2": 1, "W3": 2, "Q": 3, "K": 4, "V": 5, "PQ": 6, "PK": 7, "PV": 8}
 
 
 @dataclasses.dataclass(frozen=True)
@@ -41,6 +46,7 @@ class TTTWorkload:
     ns_iters: int = 0         # Newton-Schulz iterations (0 = plain Eq. 8)
     renorm: int = 0           # restore per-unit fan-in norms after the update
     seed: int = 0
+    structured: bool = False  # Q, K, V = projections of common tokens (secondary workload)
 
     @property
     def d(self) -> int:
@@ -108,6 +114,11 @@ class TokenStream:
         self._g = {s: _gen(w.seed, s) for s in ("Q", "K", "V")}
         self._prev = {s: None for s in ("Q", "K", "V")}
         self._chunk = 0
+        self._proj = None
+        if w.structured:
+            std = 1.0 / math.sqrt(w.d)
+            self._proj = {s: torch.randn(w.d, w.d, generator=_gen(w.seed, "P" + s), dtype=torch.float32) * std
+                          for s in ("Q", "K", "V")}
 
     def _frames(self, s: str, nf: int) -> torch.Tensor:
         w = self.w
@@ -131,8 +142,9 @@ class TokenStream:
         self._chunk += 1
         M = nf * w.tokens_per_frame
         out = []
+        common = self._frames("Q", nf).reshape(M, w.d) if w.structured else None
         for s in ("Q", "K", "V"):
-            X = self._frames(s, nf).reshape(M, w.nh, w.hd)
+            X = (common @ self._proj[s] if w.structured else self._frames(s, nf)).reshape(M, w.nh, w.hd)
             if s == "K" and w.l2_k:
                 X = X / X.norm(dim=-1, keepdim=True)
             out.append(X.reshape(M, w.d).to(w.torch_dtype).contiguous())
