@@ -187,6 +187,25 @@ def test_bf16_wide_head_gradient_and_apply(M):
     gpu.close()
 
 
+def test_bf16_wide_head_more_pairs_than_sms():
+    """hd = 128 gradient kernel when (head, slice) pairs outnumber the SMs: 40 heads x 4 slices = 160
+    pairs, so a CTA's unit range crosses several pair boundaries (one segment per pair)."""
+    dev = torch.device("cuda", 0)
+    w = _bf16_workload("cfg5", nh=40, tokens_per_frame=100, frames_per_chunk=1, n_frames=1, ns_iters=0)
+    W1, W2, W3 = ti.fast_weights(w)
+    Q, K, V, lr = ti.TokenStream(w).next_chunk()
+    gpu = _mk(w)
+    gpu.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    loss = torch.zeros(w.nh, dtype=torch.float32, device=dev)
+    O = gpu.ttt_chunk_step(Q.to(dev), K.to(dev), V.to(dev), lr.to(dev), loss=loss)
+    ora = OracleTTT(W1, W2, W3)
+    O_ref, loss_ref = ora.chunk_step(Q, K, V, lr)
+    assert rel_err(O.float().cpu(), O_ref) <= TOL_BF16
+    assert max(rel_err(a.cpu(), b) for a, b in zip(gpu.ttt_get_weights(), ora.weights())) <= TOL_BF16
+    assert rel_err(loss.cpu(), loss_ref) <= TOL_LOSS_BF16
+    gpu.close()
+
+
 def test_bf16_gradient_against_oracle():
     """The raw gradient (before the commit) is the most sensitive quantity: compare G1, G2, G3."""
     dev = torch.device("cuda", 0)
@@ -206,7 +225,7 @@ def test_bf16_gradient_against_oracle():
     gpu.close()
 
 
-@pytest.mark.parametrize("hd,H", [(64, 128), (64, 256), (128, 128), (128, 256), (128, 512)])
+@pytest.mark.parametrize("hd,H", [(64, 128), (64, 256), (128, 128), (128, 256), (128, 512), (128, 1024)])
 def test_bf16_newton_schulz_kernel_against_oracle(hd, H):
     """The tensor-core Newton-Schulz kernels in isolation (hd = 64: one CTA per matrix; hd = 128: a
     cluster of H / 128 CTAs per matrix): W0 - W' after a commit must equal the oracle's NS of the
