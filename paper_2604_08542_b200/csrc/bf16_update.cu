@@ -45,6 +45,10 @@ __device__ unsigned long long g_ttt_time[4];      // globaltimer ns + clock64 at
 extern "C" int ttt_debug_time(unsigned long long* host) {
   return (int)cudaMemcpyFromSymbol(host, g_ttt_time, sizeof(g_ttt_time));
 }
+__device__ unsigned long long g_ttt_cta_time[2 * 256];   // globaltimer at start / end of every CTA
+extern "C" int ttt_debug_cta_time(unsigned long long* host) {
+  return (int)cudaMemcpyFromSymbol(host, g_ttt_cta_time, sizeof(g_ttt_cta_time));
+}
 __device__ unsigned g_ttt_trace2[32 * 16 * 4];   // [tile][epilogue warp][got, loaded, math, done]
 #define TTT_TR2(i, w, k) do { if ((i) < 32 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && lane == 0) g_ttt_trace2[((i) * 16 + (w)) * 4 + (k)] = (unsigned)clock(); } while (0)
 extern "C" int ttt_debug_trace2(unsigned* host) {
@@ -113,6 +117,11 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   for (int e = threadIdx.x; e < 64 * 16; e += blockDim.x) tr_s[e] = 0;
   __syncthreads();
   if (threadIdx.x == 0) tr_s[15] = (unsigned)clock();
+  if (threadIdx.x == 0) {
+    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    const int lin = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    if (lin < 256) g_ttt_cta_time[2 * lin] = t;
+  }
   if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) {
     unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     g_ttt_time[0] = t; g_ttt_time[1] = clock64();
@@ -415,6 +424,13 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     if (ew == 0 && lane == 0) TTT_TR(3, 13);
     float* Pset = P + (size_t)split * 3 * me;
     const uint32_t gcol[3] = {C_G1, C_G2, C_G3};
+    // TMEM gives a thread 16 columns of ONE row: written to global memory directly, a warp store would
+    // touch 32 lines for 512 bytes (measured: 6.3 K clk for the flush). The idle K/V ring stages each
+    // matrix as [128][68] fp32 (two buffers, alternating), then the slice's 32 KB leave as full lines.
+    constexpr int SLD = HD + 4;
+    float* stg = reinterpret_cast<float*>(smem);
+    const int et = ew * 32 + lane;                         // 0 .. 511
+    const size_t slice_base = ((size_t)h * H + (size_t)slice * HS) * HD;
 #pragma unroll
     for (int mat = 0; mat < 3; ++mat) {                    // this warp: columns 16 tc .. 16 tc + 15
       uint32_t r[16];
@@ -426,11 +442,19 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         for (int u = 0; u < 16; ++u) r[u] = 0u;
       }
       const float sc = mat == 0 ? 0.5f : 1.0f;             // G1 was accumulated from 2 dA
-      float4* dst = reinterpret_cast<float4*>(Pset + mat * me + row + 16 * tc);
+      float* sb = stg + (mat & 1) * HS * SLD;
+      float4* d = reinterpret_cast<float4*>(sb + j * SLD + 16 * tc);
 #pragma unroll
       for (int v = 0; v < 4; ++v)
-        dst[v] = make_float4(sc * __uint_as_float(r[4 * v]), sc * __uint_as_float(r[4 * v + 1]),
-                             sc * __uint_as_float(r[4 * v + 2]), sc * __uint_as_float(r[4 * v + 3]));
+        d[v] = make_float4(sc * __uint_as_float(r[4 * v]), sc * __uint_as_float(r[4 * v + 1]),
+                           sc * __uint_as_float(r[4 * v + 2]), sc * __uint_as_float(r[4 * v + 3]));
+      asm volatile("bar.sync 9, 512;" ::: "memory");
+      float4* dst = reinterpret_cast<float4*>(Pset + mat * me + slice_base);
+#pragma unroll
+      for (int k = 0; k < HS * HD / 4 / 512; ++k) {
+        const int e = et + 512 * k;                        // float4 index: row e / 16, columns 4 (e % 16)
+        dst[e] = *reinterpret_cast<const float4*>(sb + (e >> 4) * SLD + 4 * (e & 15));
+      }
     }
     if (ew == 0 && lane == 0) TTT_TR(4, 13);
     if (LOSS) {
@@ -527,6 +551,11 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   }
 #ifdef TTT_TRACE
   if (threadIdx.x == 0) tr_s[16 + 15] = (unsigned)clock();
+  if (threadIdx.x == 0) {
+    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    const int lin = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    if (lin < 256) g_ttt_cta_time[2 * lin + 1] = t;
+  }
   if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) {
     unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     g_ttt_time[2] = t; g_ttt_time[3] = clock64();
