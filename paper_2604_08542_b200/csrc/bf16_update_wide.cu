@@ -40,7 +40,7 @@ namespace updw {
 constexpr int HS = 128;        // hidden units per CTA (MMA M)
 constexpr int HD = 128;        // head dimension (forward MMA K, gradient MMA N)
 constexpr int T = 32;          // tokens per tile (forward MMA N, gradient MMA K)
-constexpr int STAGES = 6;      // K/V shared-memory ring
+constexpr int STAGES = 5;      // K/V shared-memory ring
 constexpr int EPI_WARPS = 8;
 constexpr int THREADS = (4 + EPI_WARPS) * 32;
 constexpr int SUB_BYTES = T * 128;          // one [T x 64] bf16 sub-tile (half of hd), 128-B swizzled
@@ -49,7 +49,9 @@ constexpr int STAGE_BYTES = 2 * TILE_BYTES;
 constexpr int WSUB_BYTES = HS * 128;        // one [128 x 64] bf16 weight sub-tile
 constexpr int WMAT_BYTES = 2 * WSUB_BYTES;
 constexpr int W_BYTES = 3 * WMAT_BYTES;
-constexpr size_t SMEM_BYTES = (size_t)W_BYTES + (size_t)STAGES * STAGE_BYTES + 1024;
+constexpr int SLD = 64 + 4;                 // flush staging row stride (floats)
+constexpr int STG_BYTES = HS * SLD * 4;     // [128][68] fp32 staging of one 64-column half
+constexpr size_t SMEM_BYTES = (size_t)W_BYTES + (size_t)STAGES * STAGE_BYTES + STG_BYTES + 1024;
 
 // TMEM column plan (512 columns x 128 lanes x 32 bit)
 constexpr uint32_t C_G1 = 0, C_G3 = 128, C_G2 = 256;   // fp32 gradient accumulators [hidden][hd]
@@ -74,6 +76,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
   uint8_t* ring = smem + W_BYTES;
+  float* stg = reinterpret_cast<float*>(ring + STAGES * STAGE_BYTES);
   __shared__ uint64_t full[STAGES], empty[STAGES], w_full, fwd_full, xbg_free, opnd_ready, opnd_free, grad_done;
   __shared__ uint32_t tmem_base_s;
   __shared__ float loss_red[EPI_WARPS];
@@ -343,28 +346,43 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
         ord = (int)(blockIdx.x - c1);
       }
       const bool pair_done = t0 + n == tiles_total;          // zero-fill the sets no segment writes
-      const size_t row = ((size_t)h * H + (size_t)slice * HS + j) * HD;
+      // TMEM gives a thread columns of ONE row; stored directly, a warp store would touch 32 lines for
+      // 512 bytes. Each 64-column half of a matrix is staged as [128][68] fp32 in shared memory and
+      // leaves as full lines (the slice's rows are contiguous in the partial set).
+      const size_t slice_base = ((size_t)h * H + (size_t)slice * HS) * HD;
       const uint32_t gcol[3] = {C_G1, C_G2, C_G3};
+      const int et = ew * 32 + lane;                         // 0 .. 255
 #pragma unroll
-      for (int mat = 0; mat < 3; ++mat) {                    // this warp: columns 64 kh .. 64 kh + 63
+      for (int mat = 0; mat < 3; ++mat) {
         const float sc = mat == 0 ? 0.5f : 1.0f;             // G1 was accumulated from 2 dA
 #pragma unroll
-        for (int cc = 0; cc < 4; ++cc) {
-          uint32_t r[16];
-          tmem_ld_x16(lane_base + gcol[mat] + 64 * kh + 16 * cc, r);
-          tc_wait_ld();
-          const size_t e = mat * me + row + 64 * kh + 16 * cc;
-          float4* dst = reinterpret_cast<float4*>(P + (size_t)ord * 3 * me + e);
+        for (int p = 0; p < 2; ++p) {                        // column half; its four warps fill the stage
+          if (kh == p) {
 #pragma unroll
-          for (int v = 0; v < 4; ++v)
-            dst[v] = make_float4(sc * __uint_as_float(r[4 * v]), sc * __uint_as_float(r[4 * v + 1]),
-                                 sc * __uint_as_float(r[4 * v + 2]), sc * __uint_as_float(r[4 * v + 3]));
-          if (pair_done)
-            for (int z = ord + 1; z < nsets; ++z) {
-              float4* zd = reinterpret_cast<float4*>(P + (size_t)z * 3 * me + e);
+            for (int cc = 0; cc < 4; ++cc) {
+              uint32_t r[16];
+              tmem_ld_x16(lane_base + gcol[mat] + 64 * p + 16 * cc, r);
+              tc_wait_ld();
+              float4* d = reinterpret_cast<float4*>(stg + j * SLD + 16 * cc);
 #pragma unroll
-              for (int v = 0; v < 4; ++v) zd[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+              for (int v = 0; v < 4; ++v)
+                d[v] = make_float4(sc * __uint_as_float(r[4 * v]), sc * __uint_as_float(r[4 * v + 1]),
+                                   sc * __uint_as_float(r[4 * v + 2]), sc * __uint_as_float(r[4 * v + 3]));
             }
+          }
+          asm volatile("bar.sync 1, 256;" ::: "memory");
+          const size_t e0 = mat * me + slice_base + 64 * p;
+#pragma unroll
+          for (int k = 0; k < HS * 64 / 4 / 256; ++k) {
+            const int e = et + 256 * k, rr = e >> 4, c4 = e & 15;   // row, float4 within the 64-column half
+            const size_t g = e0 + (size_t)rr * HD + 4 * c4;
+            *reinterpret_cast<float4*>(P + (size_t)ord * 3 * me + g) =
+                *reinterpret_cast<const float4*>(stg + rr * SLD + 4 * c4);
+            if (pair_done)
+              for (int z = ord + 1; z < nsets; ++z)
+                *reinterpret_cast<float4*>(P + (size_t)z * 3 * me + g) = make_float4(0.f, 0.f, 0.f, 0.f);
+          }
+          asm volatile("bar.sync 1, 256;" ::: "memory");
         }
       }
       tc_fence_before();

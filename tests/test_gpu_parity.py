@@ -130,6 +130,8 @@ def _bf16_workload(base, **kw):
     ("cfg2", dict(nh=2, tokens_per_frame=333, frames_per_chunk=3, n_frames=3)),
     # hidden 256 (two hidden slices), Newton-Schulz, 3 chunks, AR(1) tokens
     ("cfg3", dict(nh=2, tokens_per_frame=257, frames_per_chunk=2, n_frames=6)),
+    # Newton-Schulz + re-normalisation (cfg3's secondary flag set)
+    ("cfg3", dict(nh=2, renorm=1, tokens_per_frame=200, frames_per_chunk=2, n_frames=6)),
     # re-normalised plain update, L2-normalised K, 4 chunks with a short last chunk
     ("cfg4", dict(nh=3, tokens_per_frame=190, frames_per_chunk=2, n_frames=7)),
     # hd = 128 kernels: Newton-Schulz + re-normalisation (NS result left in G, generic commit), 3 chunks
