@@ -1,6 +1,6 @@
 """Per-chunk parity curve of a full-size config (not a pytest module; run by hand on a GPU box):
 
-    python tests/parity_curve.py cfg5 2,5 [max_chunks]
+    python tests/parity_curve.py cfg5 2,5 [max_chunks] [field=value ...]     (e.g. l2_k=1 renorm=1)
 
 streams the whole config through the CUDA path (all heads) and through the float64 oracle (the listed
 heads: heads are independent, so this is exact per head) and prints, per chunk, the errors of O and of
@@ -16,8 +16,16 @@ from oracle.ttt_oracle import OracleTTT, rel_err
 from paper_2604_08542_b200 import TTT, TTT_BF16
 
 name = sys.argv[1]; heads = [int(x) for x in sys.argv[2].split(",")]
-nmax = int(sys.argv[3]) if len(sys.argv) > 3 else 10**9
+nmax = int(sys.argv[3]) if len(sys.argv) > 3 and "=" not in sys.argv[3] else 10**9
 w = ti.CONFIGS[name]; dev = torch.device("cuda", 0)
+over = {}
+for a in sys.argv[3:]:
+    if "=" in a:
+        k, v = a.split("=")
+        over[k] = type(getattr(w, k))(int(v)) if not isinstance(getattr(w, k), float) else float(v)
+if over:
+    w = ti.scaled(w, **over)
+    print("# overrides:", over)
 W1, W2, W3 = ti.fast_weights(w)
 cols = torch.cat([torch.arange(h * w.hd, (h + 1) * w.hd) for h in heads])
 r = lambda x: x.to(torch.bfloat16).to(torch.float32)
