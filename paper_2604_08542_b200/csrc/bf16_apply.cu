@@ -49,7 +49,7 @@ constexpr int NF = 3;            // forward buffers: two in the epilogue (one pe
 
 __global__ void __launch_bounds__(app::THREADS, 1)
 bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ CUtensorMap mapQ,
-                  const __grid_constant__ CUtensorMap mapO, int nh, int H, int tiles_total) {
+                  const __grid_constant__ CUtensorMap mapO, int nh, int H, int tiles_total, int q_early) {
   using namespace app;
   constexpr int HD = 64;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -71,16 +71,33 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   uint8_t* q_ring = smem + w_bytes;                          // QST x 16 KB
   uint8_t* o_stage = q_ring + QST * TILE_BYTES;              // 2 x 16 KB
 
+  // Prologue spread over three threads (barriers of the Q ring + first Q requests | other barriers |
+  // TMEM allocation). With `q_early` (set by ttt_chunk_step, where the preceding kernels in the
+  // stream are this library's own and Q was complete before the first of them started) the first Q
+  // tiles are requested BEFORE griddepcontrol.wait, so the first TMA round trip (~2 us with the
+  // descriptor fetch) overlaps the tail of the kernel that produces the weights.
+  const int npre = min(my_tiles, QST);
   if (tid == 0) {
+    tma_prefetch_desc(&mapQ);
+    tma_prefetch_desc(&mapW);
+    for (int s = 0; s < QST; ++s) mbar_init(&qr_full[s], 1);
+    fence_mbar_init();
+    if (q_early)
+      for (int tl = 0; tl < npre; ++tl) {
+        mbar_arrive_expect_tx(&qr_full[tl], TILE_BYTES);
+        tma_load_2d_hint(q_ring + tl * TILE_BYTES, &mapQ, &qr_full[tl], h * HD,
+                         ((int)blockIdx.x + tl * (int)gridDim.x) * TM, kEvictFirst);
+      }
+  } else if (tid == 32) {
     for (int n = 0; n < 8; ++n) mbar_init(&w_full[n], 1);
     for (int b = 0; b < NF; ++b) { mbar_init(&fwd_full[b], 1); mbar_init(&epi_done[b], 8); }
     for (int b = 0; b < 2; ++b) { mbar_init(&q_full[b], 128); mbar_init(&q_empty[b], 1); }
     mbar_init(&o_full, 1);
     mbar_init(&o_empty, 128);
-    for (int s = 0; s < QST; ++s) { mbar_init(&qr_full[s], 1); mbar_init(&qr_empty[s], 128); }
+    for (int s = 0; s < QST; ++s) mbar_init(&qr_empty[s], 128);
     fence_mbar_init();
   }
-  if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  if (warp == 2) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -95,17 +112,14 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   if (warp == 0) {
     // ===================== TMA producer: weights once, then the Q tiles =====================
     if (elect_one() && my_tiles > 0) {
-      tma_prefetch_desc(&mapW);
-      tma_prefetch_desc(&mapQ);
-      // first Q tiles first (they feed the I/O warpgroup's shared -> TMEM copy), then the weights step
+      // first Q tile first (it feeds the Q-load warpgroup's shared -> TMEM copy), then the weights step
       // by step, each step on its own barrier so the MMAs start when step 0 has landed
-      const int npre = min(my_tiles, QST);
       auto q_load = [&](int tl) {
         mbar_arrive_expect_tx(&qr_full[tl], TILE_BYTES);
         tma_load_2d_hint(q_ring + tl * TILE_BYTES, &mapQ, &qr_full[tl], h * HD,
                          ((int)blockIdx.x + tl * (int)gridDim.x) * TM, kEvictFirst);
       };
-      q_load(0);               // what the first MMAs need goes first: Q tile 0, then the weights in step order
+      if (!q_early) q_load(0);
       // smem, boxes of 64 rows (8 KB): per 64-hidden step n [W1^T rows | W3^T rows] back to back
       // (one 128-row K-major B operand), then the W2 row blocks
       for (int n = 0; n < nsl; ++n) {
@@ -115,7 +129,8 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
         tma_load_2d_hint(smem + (size_t)nsl * 16384 + (size_t)n * 8192, &mapW, &w_full[n], 0,
                          (1 * nh + h) * H + 64 * n, kEvictLast);
       }
-      for (int tl = 1; tl < npre; ++tl) q_load(tl);
+      if (!q_early)
+        for (int tl = 1; tl < npre; ++tl) q_load(tl);
       for (int tl = npre; tl < my_tiles; ++tl) {
         const int rs = tl % QST, it = tl / QST;
         mbar_wait(&qr_empty[rs], (it & 1) ^ 1);
@@ -283,7 +298,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 0) tmem_dealloc(tb, 512);
+  if (warp == 2) tmem_dealloc(tb, 512);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -321,8 +336,8 @@ int bf16_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  int nh = c.nh, H = c.hidden, ntl = tiles;
-  cudaError_t e = cudaLaunchKernelEx(&cfg, bf16_apply_kernel, mapW, mapQ, mapO, nh, H, ntl);
+  int nh = c.nh, H = c.hidden, ntl = tiles, q_early = ctx->apply_q_early;
+  cudaError_t e = cudaLaunchKernelEx(&cfg, bf16_apply_kernel, mapW, mapQ, mapO, nh, H, ntl, q_early);
   if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, "bf16_apply_kernel launch", e);
   TTT_LAUNCH_CHECK(ctx, "bf16_apply_kernel");
   return TTT_OK;

@@ -134,8 +134,32 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   const int tile_lo = split * tiles_per_split;
   const int ntiles = min(tiles_per_split, tiles_total - tile_lo);
 
+  // Prologue, spread over three threads so that nothing queues behind anything else: the first
+  // TMA round trip (descriptor fetch + HBM, ~2 us = 3.5 K clk) is the critical path of the start-up,
+  // so thread 0 initialises only the ring's `full` barriers and requests the first ring of K/V tiles;
+  // warp 1 initialises the other barriers; warp 3 allocates TMEM (trace, r01e: requests left at
+  // 2.3-3.6 K clk when all of this was serial in thread 0, first forward MMA at 7-9 K clk).
   if (tid == 0) {
-    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 2); mbar_init(&empty[s], 1); }
+    TTT_TR(8, 14);
+    tma_prefetch_desc(&mapK);
+    tma_prefetch_desc(&mapV);
+    TTT_TR(9, 14);
+#pragma unroll
+    for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 2);
+    TTT_TR(10, 14);
+    fence_mbar_init();
+    TTT_TR(1, 14);
+    const int npre = min(ntiles, STAGES);
+    for (int i = 0; i < npre; ++i) {
+      mbar_arrive_expect_tx(&full[i], STAGE_BYTES);
+      uint8_t* dst = smem + i * STAGE_BYTES;
+      tma_load_2d(dst, &mapK, &full[i], h * HD, (tile_lo + i) * T);
+      tma_load_2d(dst + TILE_BYTES, &mapV, &full[i], h * HD, (tile_lo + i) * T);
+    }
+    TTT_TR(2, 14);
+  } else if (tid == 32) {
+#pragma unroll
+    for (int s = 0; s < STAGES; ++s) mbar_init(&empty[s], 1);
     mbar_init(&fwd_full[0], 1);
     mbar_init(&fwd_full[1], 1);
     mbar_init(&g_free, EPI_WARPS / 2);
@@ -144,17 +168,6 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     mbar_init(&w_ready, EPI_WARPS);
     mbar_init(&grad_done, 1);
     fence_mbar_init();
-    // the first ring of K/V tiles is requested before anything else: the first TMA round trip
-    // (descriptor fetch + HBM) is ~2 us and would otherwise start after the TMEM allocation
-    tma_prefetch_desc(&mapK);
-    tma_prefetch_desc(&mapV);
-    const int npre = min(ntiles, STAGES);
-    for (int i = 0; i < npre; ++i) {
-      mbar_arrive_expect_tx(&full[i], STAGE_BYTES);
-      uint8_t* dst = smem + i * STAGE_BYTES;
-      tma_load_2d(dst, &mapK, &full[i], h * HD, (tile_lo + i) * T);
-      tma_load_2d(dst + TILE_BYTES, &mapV, &full[i], h * HD, (tile_lo + i) * T);
-    }
   }
   __syncwarp();
   // epilogue warps request their share of the bf16 weights now (row j of W1^T, W2, W3^T; 16-byte
@@ -178,10 +191,15 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
 #pragma unroll
     for (int u = 0; u < LRPF; ++u) {
       const int t = (tile_lo + u) * T + lane;
-      lr_pre[u] = (u < ntiles && t < M) ? -__ldg(lr + (size_t)h * M + t) : 0.f;
+      lr_pre[u] = (u < ntiles && t < M) ? __ldg(lr + (size_t)h * M + t) : 0.f;   // negated after the barrier
     }
   }
-  if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  if (warp == 3) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  if (tid == 96) TTT_TR(3, 14);
+  if (tid == 255) TTT_TR(4, 14);
+  if (tid == 64) TTT_TR(11, 14);
+  if (tid == 31) TTT_TR(12, 14);
+  if (tid == 33) TTT_TR(13, 14);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -288,7 +306,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     };
     float cur[LRPF], nxt[LRPF];
 #pragma unroll
-    for (int u = 0; u < LRPF; ++u) cur[u] = lr_pre[u];       // requested before the allocation barrier
+    for (int u = 0; u < LRPF; ++u) cur[u] = -lr_pre[u];      // requested before the allocation barrier
     for (int i0 = 0; i0 < ntiles; i0 += LRPF) {
       ld_batch(i0 + LRPF, nxt);
 #pragma unroll
@@ -335,6 +353,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&w_ready);
+      if (ew == 0 && lane == 0) TTT_TR(5, 14);
     }
     uint64_t loss2 = 0ull;
     const uint64_t ONE2 = pack2(1.0f, 1.0f), NONE2 = pack2(-1.0f, -1.0f);
@@ -474,7 +493,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 0) tmem_dealloc(tb, 512);
+  if (warp == 3) tmem_dealloc(tb, 512);
   if (Wm != nullptr) {
     // ---- fused commit (Eq. 8): W <- W - sum_s P[s], summed in split order [+ re-normalisation] ----
     // The `gridDim.x` CTAs that share this (head, slice) meet at a counter in global memory (the
@@ -490,6 +509,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(sync_ctr + h * nslices + slice) : "memory");
         if (clock64() - t0 > TTT_MBAR_TIMEOUT_CYCLES) __trap();
       } while ((int)(v - sync_target) < 0);
+      TTT_TR(6, 14);
     }
     __syncthreads();
     const size_t me = (size_t)nh * H * HD, set = 3 * me;
@@ -499,41 +519,68 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     const int chunk = ((N4 + nsplit - 1) / nsplit + RQ - 1) / RQ * RQ;   // whole rows per CTA
     const int e_lo = min(N4, split * chunk), e_hi = min(N4, e_lo + chunk);
     float4 colacc = make_float4(0.f, 0.f, 0.f, 0.f);        // renorm: W2 column sums of squares
-    for (int base = e_lo; base < e_hi; base += THREADS) {   // THREADS % 16 == 0: a lane keeps its columns
-      const int e = base + tid;
-      const bool ok = e < e_hi;
-      const int mat = ok ? e / (HS * HD / 4) : 0, r4 = ok ? e % (HS * HD / 4) : 0;
-      const size_t off = mat * me + row0 + (size_t)r4 * 4;
-      float4 w = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (ok) {
-        float4 g = __ldcg(reinterpret_cast<const float4*>(P + off));
-#pragma unroll 4
-        for (int sp = 1; sp < nsplit; ++sp) {
-          const float4 p = __ldcg(reinterpret_cast<const float4*>(P + (size_t)sp * set + off));
-          g.x += p.x; g.y += p.y; g.z += p.z; g.w += p.w;
-        }
-        w = *reinterpret_cast<const float4*>(Wm + off);
-        w.x -= g.x; w.y -= g.y; w.z -= g.z; w.w -= g.w;
-      }
-      if (renorm_n0 != nullptr) {
-        if (mat != 1) {       // W1^T / W3^T: a row is a unit's fan-in vector -> back to its initial norm
-          float sq = w.x * w.x + w.y * w.y + w.z * w.z + w.w * w.w;
+    // The loop is bound by L2 round trips (~700 clk each under load), so a pass covers CE elements
+    // per thread and requests CU partial sets of each at once: nsplit = 9 (cfg2: 688 float4 per CTA)
+    // takes 2 round trips, nsplit = 4 (cfg3/cfg4: 1536) 2 passes of one (trace, r01e: 5.7 K clk for
+    // the one-element, four-sets-at-a-time loop at cfg2). The sum keeps the split order.
+    constexpr int CE = 2, CU = 5;
+    for (int base = e_lo; base < e_hi; base += CE * THREADS) {   // THREADS % 16 == 0: a lane keeps its columns
+      bool ok[CE];
+      int mat[CE], r4[CE];
+      size_t off[CE];
+      float4 w[CE], g[CE];
 #pragma unroll
-          for (int o = RQ / 2; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
-          const int j = slice * HS + r4 / RQ;
-          const float* n0m = renorm_n0 + (mat == 0 ? (size_t)h * H : (size_t)nh * H + (size_t)nh * HD + (size_t)h * H);
-          const float f = ok ? n0m[j] / (sqrtf(sq) + 1e-5f) : 0.f;
-          w.x *= f; w.y *= f; w.z *= f; w.w *= f;
-        } else if (ok) {      // W2: fan-in = column; finished by renorm_w2_kernel from per-CTA partials
-          colacc.x = fmaf(w.x, w.x, colacc.x); colacc.y = fmaf(w.y, w.y, colacc.y);
-          colacc.z = fmaf(w.z, w.z, colacc.z); colacc.w = fmaf(w.w, w.w, colacc.w);
-        }
+      for (int k = 0; k < CE; ++k) {
+        const int e = base + k * THREADS + tid;
+        ok[k] = e < e_hi;
+        mat[k] = ok[k] ? e / (HS * HD / 4) : 0;
+        r4[k] = ok[k] ? e % (HS * HD / 4) : 0;
+        off[k] = mat[k] * me + row0 + (size_t)r4[k] * 4;
+        w[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        g[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (ok[k]) w[k] = *reinterpret_cast<const float4*>(Wm + off[k]);
       }
-      if (ok) {
-        *reinterpret_cast<float4*>(Wm + off) = w;
-        *reinterpret_cast<uint2*>(Wbw + off) = make_uint2(pack_bf16x2(w.x, w.y), pack_bf16x2(w.z, w.w));
+      for (int sp0 = 0; sp0 < nsplit; sp0 += CU) {
+        float4 p[CE][CU];
+#pragma unroll
+        for (int k = 0; k < CE; ++k)
+#pragma unroll
+          for (int u = 0; u < CU; ++u)
+            if (ok[k] && sp0 + u < nsplit)
+              p[k][u] = __ldcg(reinterpret_cast<const float4*>(P + (size_t)(sp0 + u) * set + off[k]));
+#pragma unroll
+        for (int k = 0; k < CE; ++k)
+#pragma unroll
+          for (int u = 0; u < CU; ++u)
+            if (ok[k] && sp0 + u < nsplit) {
+              if (sp0 + u == 0) g[k] = p[k][u];
+              else { g[k].x += p[k][u].x; g[k].y += p[k][u].y; g[k].z += p[k][u].z; g[k].w += p[k][u].w; }
+            }
+      }
+#pragma unroll
+      for (int k = 0; k < CE; ++k) {
+        if (ok[k]) { w[k].x -= g[k].x; w[k].y -= g[k].y; w[k].z -= g[k].z; w[k].w -= g[k].w; }
+        if (renorm_n0 != nullptr) {
+          if (mat[k] != 1) {    // W1^T / W3^T: a row is a unit's fan-in vector -> back to its initial norm
+            float sq = w[k].x * w[k].x + w[k].y * w[k].y + w[k].z * w[k].z + w[k].w * w[k].w;
+#pragma unroll
+            for (int o = RQ / 2; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+            const int j = slice * HS + r4[k] / RQ;
+            const float* n0m = renorm_n0 + (mat[k] == 0 ? (size_t)h * H : (size_t)nh * H + (size_t)nh * HD + (size_t)h * H);
+            const float f = ok[k] ? n0m[j] / (sqrtf(sq) + 1e-5f) : 0.f;
+            w[k].x *= f; w[k].y *= f; w[k].z *= f; w[k].w *= f;
+          } else if (ok[k]) {   // W2: fan-in = column; finished by renorm_w2_kernel from per-CTA partials
+            colacc.x = fmaf(w[k].x, w[k].x, colacc.x); colacc.y = fmaf(w[k].y, w[k].y, colacc.y);
+            colacc.z = fmaf(w[k].z, w[k].z, colacc.z); colacc.w = fmaf(w[k].w, w[k].w, colacc.w);
+          }
+        }
+        if (ok[k]) {
+          *reinterpret_cast<float4*>(Wm + off[k]) = w[k];
+          *reinterpret_cast<uint2*>(Wbw + off[k]) = make_uint2(pack_bf16x2(w[k].x, w[k].y), pack_bf16x2(w[k].z, w[k].w));
+        }
       }
     }
+    if (tid == 0) TTT_TR(7, 14);
     if (renorm_n0 != nullptr) {
       float4* cs = reinterpret_cast<float4*>(smem);         // the K/V ring is idle by now
       cs[tid] = colacc;

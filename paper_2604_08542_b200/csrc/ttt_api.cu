@@ -283,7 +283,12 @@ int ttt_chunk_step(ttt_ctx* ctx, const void* Q, const void* K, const void* V, co
     rc = launch_commit(ctx, s);
     if (rc != TTT_OK) return rc;
   }
-  return do_apply(ctx, Q, O, M, ld, s);
+  // the kernels between here and the caller's last write of Q are this library's own: the apply
+  // kernel may request its first Q tiles before its programmatic-dependency wait
+  ctx->apply_q_early = 1;
+  rc = do_apply(ctx, Q, O, M, ld, s);
+  ctx->apply_q_early = 0;
+  return rc;
 }
 
 int ttt_get_weights(ttt_ctx* ctx, float* W1, float* W2, float* W3, void* stream) {

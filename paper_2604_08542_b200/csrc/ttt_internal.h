@@ -50,6 +50,8 @@ struct ttt_ctx {
   float* ns_scratch;
   unsigned* sync_ctr;
   unsigned sync_target;
+  // set by ttt_chunk_step around its apply launch: Q may be requested before the PDL wait
+  int apply_q_early;
 
   // bf16 path: driver entry point for cuTensorMapEncodeTiled
   void* encode_tiled;
