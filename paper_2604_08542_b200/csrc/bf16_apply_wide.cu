@@ -17,6 +17,7 @@
 //   Warps: TMA producer, MMA issuer, two epilogue groups of 8 warps, one per tile (SwiGLU
 //   epilogue per step, O -> bf16 -> global).
 #include <stdio.h>
+#include <stdlib.h>
 
 #include "tc_common.cuh"
 #include "ttt_internal.h"
@@ -239,6 +240,10 @@ int bf16_apply_wide_supported(const ttt_config* cfg) {
 int bf16_apply_wide(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
                     cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
+  // CTA-pair kernel by default (bf16_apply_wide_pair.cu); TTT_APPLY_WIDE_PAIR=0 selects this file's
+  // single-CTA kernel (kept for A/B measurements)
+  static const int use_pair = [] { const char* e = getenv("TTT_APPLY_WIDE_PAIR"); return e ? atoi(e) : 1; }();
+  if (use_pair) return bf16_apply_wide_pair(ctx, Q, O, M, ld, s);
   const int tiles = (int)((M + appw::TM - 1) / appw::TM);
   const int npairs = (tiles + 1) / 2;
   CUtensorMap mapW, mapQ;

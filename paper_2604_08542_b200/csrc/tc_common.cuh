@@ -85,6 +85,17 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   }
 }
 
+// polling wait: test_wait never suspends the thread (a suspended try_wait is woken promptly by
+// arrivals from its own SM; for multicast commits and remote arrivals from the pair's other SM a
+// polling loop is used instead)
+__device__ __forceinline__ void mbar_wait_spin(uint64_t* bar, uint32_t parity) {
+  if (mbar_test_wait(bar, parity)) return;
+  long long t0 = clock64();
+  while (!mbar_test_wait(bar, parity)) {
+    if (clock64() - t0 > TTT_MBAR_TIMEOUT_CYCLES) __trap();
+  }
+}
+
 // ----------------------------------------------------------------------------------------------
 // TMA: 2-D tiled load global -> shared, completion on an mbarrier (complete_tx::bytes)
 // ----------------------------------------------------------------------------------------------
@@ -205,12 +216,14 @@ __device__ __forceinline__ void tc_commit2(uint64_t* bar) {
       "h"(static_cast<uint16_t>(3))
       : "memory");
 }
-// arrive on the barrier at this shared-memory offset in CTA `rank` of the cluster
+// arrive on the barrier at this shared-memory offset in CTA `rank` of the cluster. Default (CTA-scope
+// release) semantics: what the pair hands over lives in TMEM and is ordered by the tcgen05 fences; an
+// explicit .release.cluster costs the arriving thread ~1 200 clk (measured, r01e).
 __device__ __forceinline__ void mbar_arrive_remote(uint64_t* bar, uint32_t rank) {
   asm volatile(
       "{\n\t.reg .b32 ra;\n\t"
       "mapa.shared::cluster.u32 ra, %0, %1;\n\t"
-      "mbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n\t}\n" ::"r"(smem_u32(bar)),
+      "mbarrier.arrive.shared::cluster.b64 _, [ra];\n\t}\n" ::"r"(smem_u32(bar)),
       "r"(rank)
       : "memory");
 }
@@ -229,6 +242,35 @@ __device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity
     if (ok) return;
     if (clock64() - t0 > TTT_MBAR_TIMEOUT_CYCLES) __trap();
   }
+}
+// D[tmem] (+)= A[smem] . B[smem], M = 256 over the CTA pair (issued by rank 0 only): the descriptors
+// are CTA-relative — each CTA reads its 128 rows of A and its N/2 rows of B at the same offsets
+__device__ __forceinline__ void umma_ss2(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc,
+                                         uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}\n"
+      ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// address of this shared-memory object in CTA `rank` of the cluster (shared::cluster window)
+__device__ __forceinline__ uint32_t mapa_u32(const void* p, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_u32(p)), "r"(rank));
+  return r;
+}
+// 2-D tiled load into THIS CTA's shared memory whose completion bytes go to a barrier that may live
+// in the pair's other CTA (`bar_cluster_addr` from mapa_u32): both CTAs of a pair feed the barrier
+// the MMA-issuing CTA waits on.
+__device__ __forceinline__ void tma_load_2d_pair(void* smem_dst, const CUtensorMap* map,
+                                                 uint32_t bar_cluster_addr, int32_t c0, int32_t c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes"
+      " [%0], [%1, {%3, %4}], [%2];"
+      ::"r"(smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(bar_cluster_addr),
+        "r"(c0), "r"(c1)
+      : "memory");
 }
 // D[tmem] (+)= A[tmem] . B[smem], M = 256 over the CTA pair (issued by rank 0 only)
 __device__ __forceinline__ void umma_ts2(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc,

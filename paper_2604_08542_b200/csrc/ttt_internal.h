@@ -104,6 +104,9 @@ int bf16_update_tensor_path(const ttt_config* cfg);
 int bf16_apply_tensor_path(const ttt_config* cfg);
 // hd = 128 apply kernel (bf16_apply_wide.cu)
 int bf16_apply_wide_supported(const ttt_config* cfg);
+// the same on CTA pairs (bf16_apply_wide_pair.cu)
+int bf16_apply_wide_pair(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
+                         cudaStream_t s);
 int bf16_apply_wide(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
                     cudaStream_t s);
 // hd = 128 update kernel (bf16_update_wide.cu)

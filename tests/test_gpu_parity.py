@@ -189,6 +189,25 @@ def test_bf16_wide_head_gradient_and_apply(M):
     gpu.close()
 
 
+def test_bf16_wide_head_apply_single_cta_variant():
+    """The hd = 128 apply runs on CTA pairs by default (bf16_apply_wide_pair.cu). The single-CTA
+    kernel (bf16_apply_wide.cu, selected with TTT_APPLY_WIDE_PAIR=0 when the library is first used,
+    hence a fresh process) is kept for A/B measurements: the hd-128 parity cases — many units per
+    CTA, ragged tails, chunks smaller than a tile, the cfg5-shaped stream, bitwise determinism — pass
+    with it too."""
+    import os
+    import subprocess
+    import sys
+    env = dict(os.environ, TTT_APPLY_WIDE_PAIR="0")
+    r = subprocess.run([sys.executable, "-m", "pytest", os.path.abspath(__file__), "-q", "-x", "-m", "gpu", "-k",
+                        "wide_head_gradient_and_apply or wide_head_more_pairs or cfg5_shape or tiny_chunks "
+                        "or determinism"],
+                       env=env, capture_output=True, text=True, timeout=900,
+                       cwd=os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    assert r.returncode == 0, r.stdout[-3000:] + r.stderr[-2000:]
+    assert " passed" in r.stdout and "failed" not in r.stdout
+
+
 def test_bf16_wide_head_more_pairs_than_sms():
     """hd = 128 gradient kernel when (head, slice) pairs outnumber the SMs: 40 heads x 4 slices = 160
     pairs, so a CTA's unit range crosses several pair boundaries (one segment per pair)."""
