@@ -243,8 +243,9 @@ def run_ours(args, w, rank, local_rank, world):
     app_tflops = flops_per_chunk(w, M, "apply") / (k_ms[2] * 1e-3) / 1e12
     step_tflops = flops_per_chunk(w, M, "step") / (ms_per_step * 1e-3) / 1e12
     # dram__bytes_read.sum + dram__bytes_write.sum of bf16_update_kernel, one launch, from the
-    # `ncu --set full` captures summarised in profiles/r01d_cfg2_cfg4_update.md and r01c_cfg5.md (None = not captured)
-    traffic = {"cfg2": 48131328 + 421888, "cfg4": 187718912 + 4704512,
+    # `ncu --set full` captures summarised in profiles/r01e_cfg2_startup_commit.md (cfg2), r01d_cfg2_cfg4_update.md
+    # (cfg4) and r01c_cfg5.md (None = not captured)
+    traffic = {"cfg2": 48135424 + 533760, "cfg4": 187718912 + 4704512,
                "cfg5": 186227456 + 9412352}.get(w.name)
     # (the per-kernel pass calls ttt_accumulate / ttt_commit / ttt_apply separately; inside
     #  ttt_chunk_step the plain commit is fused into the update kernel's tail)
