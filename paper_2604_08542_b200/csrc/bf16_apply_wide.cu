@@ -243,7 +243,10 @@ int bf16_apply_wide(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int6
   // CTA-pair kernel by default (bf16_apply_wide_pair.cu); TTT_APPLY_WIDE_PAIR=0 selects this file's
   // single-CTA kernel (kept for A/B measurements)
   static const int use_pair = [] { const char* e = getenv("TTT_APPLY_WIDE_PAIR"); return e ? atoi(e) : 1; }();
-  if (use_pair) return bf16_apply_wide_pair(ctx, Q, O, M, ld, s);
+  if (use_pair) {
+    const int rc = bf16_apply_wide_pair(ctx, Q, O, M, ld, s);
+    if (rc != 1) return rc;          // 1 = the device cannot host a CTA pair: single-CTA kernel below
+  }
   const int tiles = (int)((M + appw::TM - 1) / appw::TM);
   const int npairs = (tiles + 1) / 2;
   CUtensorMap mapW, mapQ;

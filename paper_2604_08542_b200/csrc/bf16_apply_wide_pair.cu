@@ -320,11 +320,8 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
 }
 
 // ------------------------------------------------------------------------------------------------
-static int fail_pairs(ttt_ctx* ctx) {
-  snprintf(ctx->err, sizeof(ctx->err), "bf16_apply_wide_pair_kernel: the device cannot host a CTA pair of this kernel");
-  return TTT_ERR_UNSUPPORTED;
-}
-
+// Returns 1 (nothing launched) when the device cannot host a CTA pair of this kernel: the caller then
+// runs the single-CTA kernel.
 int bf16_apply_wide_pair(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
                          cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
@@ -363,10 +360,10 @@ int bf16_apply_wide_pair(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O,
     int n = 0;
     TTT_CUDA_TRY(ctx, cudaOccupancyMaxActiveClusters(&n, bf16_apply_wide_pair_kernel, &cfg),
                  "bf16_apply_wide_pair_kernel occupancy");
-    if (n < 1) return fail_pairs(ctx);
-    max_pairs = n;
+    max_pairs = n > 0 ? n : -1;
     if (getenv("TTT_DEBUG_PAIRS")) fprintf(stderr, "bf16_apply_wide_pair: %d co-resident CTA pairs\n", n);
   }
+  if (max_pairs < 0) return 1;
   cfg.numAttrs = 2;
   int ncl = c.nh * npairs;
   if (ncl > max_pairs) ncl = max_pairs;
