@@ -183,6 +183,8 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
       long long pp_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
       long long pp_t = clock64();
       const long long pp_start = pp_t;
+      unsigned long long pp_gt0;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(pp_gt0));
 #endif
       // O(unit) (+)= Hq(step g) W2[step rows]; the step's W2 rows landed with its forward rows
       // (w_full was waited on by the forward issuer before F(g), which precedes Hq(g))
@@ -210,6 +212,9 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
         for (int k = 0; k < 8; ++k) g_appp_trace[k] = pp_acc[k];
         g_appp_trace[8] = clock64() - pp_start;
         g_appp_trace[9] = G;
+        unsigned long long pp_gt1;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(pp_gt1));
+        g_appp_trace[13] = (long long)(pp_gt1 - pp_gt0);      // ns: SM clock = [8] / [13] GHz
       }
 #endif
     }
