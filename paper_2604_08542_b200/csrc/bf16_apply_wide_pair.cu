@@ -16,10 +16,9 @@
 // limits a step (first pair version, two tiles per CTA with single forward buffers as in the
 // single-CTA kernel: 177 us at cfg5 — both tiles' epilogues ran in lock-step, 2 000 of 3 650 clk per
 // step the issuer waited for Hq). So a unit is (head, ONE 128-token tile per CTA = 256 tokens per pair),
-// the forward accumulators x | b are double-buffered (F(g + 2) is issued right behind D(g)), all
-// 16 epilogue warps work on the one tile (a step's epilogue halves), the O accumulator is
-// double-buffered too and drained to global memory by four warps of their own while the next unit's
-// steps run. TMEM (512 columns): O[2] at 0 / 128, x | b [2] at 256 / 384 (64 + 64 columns); the bf16
+// the forward accumulators x | b are triple-buffered (F(g + 3) follows the completion of D(g)), all
+// 16 epilogue warps work on the one tile, and four warps of their own drain the O accumulator to
+// global memory. TMEM (512 columns): O at 0, x | b [3] at 128 / 256 / 384 (64 + 64 columns); the bf16
 // Hq (A operand of the down MMAs) overwrites the first 32 columns of its own x once all epilogue
 // warps hold their x | b in registers.
 #include <stdio.h>
@@ -32,8 +31,16 @@
 __device__ long long g_appp_trace[32];
 extern "C" int ttt_debug_appp_trace(long long* host) { return (int)cudaMemcpyFromSymbol(host, g_appp_trace, sizeof(g_appp_trace)); }
 #define PP_ACC(k) do { pp_acc[k] += clock64() - pp_t; pp_t = clock64(); } while (0)
+// timeline of one steady-state step (g == PP_G) of CTA pair 0, rank 0: clock64 marks of every role
+__device__ long long g_appp_tl[16];
+__device__ unsigned long long g_appp_span[2 * 80];   // globaltimer at start / end of rank 0 of every pair
+extern "C" int ttt_debug_appp_span(unsigned long long* host) { return (int)cudaMemcpyFromSymbol(host, g_appp_span, sizeof(g_appp_span)); }
+extern "C" int ttt_debug_appp_timeline(long long* host) { return (int)cudaMemcpyFromSymbol(host, g_appp_tl, sizeof(g_appp_tl)); }
+#define PP_G 44
+#define PP_TL(cond, k) do { if ((cond) && cid == 0 && rank == 0) g_appp_tl[k] = clock64(); } while (0)
 #else
 #define PP_ACC(k) do { } while (0)
+#define PP_TL(cond, k) do { } while (0)
 #endif
 
 namespace ttt {
@@ -47,7 +54,7 @@ constexpr int TM = 128;        // tokens per tile and CTA (MMA M = 256 over the 
 constexpr int HSTEP = 64;      // hidden units per step
 constexpr int NST = 4;         // weight ring stages (24 KB per CTA and stage)
 constexpr int EPI_WARPS = 16;  // SwiGLU epilogue warps (4 per TMEM lane quadrant, 16 hidden columns each)
-constexpr int DRAIN_WARPS = 4; // O -> bf16 -> global
+constexpr int DRAIN_WARPS = 8; // O -> bf16 -> global (2 per TMEM lane quadrant, 64 columns each)
 constexpr int DRAIN_WARP0 = 4 + EPI_WARPS;
 constexpr int THREADS = (4 + EPI_WARPS + DRAIN_WARPS) * 32;
 constexpr int QSUB_BYTES = TM * 128;            // [128 tokens x 64] bf16 sub-tile (half of hd)
@@ -84,10 +91,13 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
   const int my_units = cid < nunits ? (nunits - cid + ncl - 1) / ncl : 0;
   const int G = my_units * nstep;                // steps of this pair, all units
 
+#ifdef TTT_TRACE
+  if (tid == 0 && rank == 0 && cid < 80) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); g_appp_span[2 * cid] = t; }
+#endif
   if (tid == 0) {
     for (int s = 0; s < NST; ++s) { mbar_init(&w_full[s], 1); mbar_init(&w_empty[s], 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(&q_full[b], 1); mbar_init(&q_free[b], 1); }
-    for (int b = 0; b < NF; ++b) { mbar_init(&f_full[b], 1); mbar_init(&hq_ready[b], EPI_WARPS); }   // 8 warps of a group in each CTA
+    for (int b = 0; b < NF; ++b) { mbar_init(&f_full[b], 1); mbar_init(&hq_ready[b], 2 * EPI_WARPS); }
     mbar_init(&o_full, 1);
     mbar_init(&o_free, 2 * DRAIN_WARPS);
     fence_mbar_init();
@@ -157,13 +167,21 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
       int n = 0, qb = 0, st = 0, fb = 0, sw = 0;
       uint32_t qph = 0, sph = 0, swph = 0;
       for (int g = 0; g < G; ++g) {
-        if (g >= NF) {
-          mbar_wait(&w_empty[sw], swph);
-          if (++sw == NST) { sw = 0; swph ^= 1; }
-        }
+        // operands first (they landed long ago), the buffer's release by D(g - NF) last: that wait is
+        // on the critical cycle F -> epilogue -> D -> F, the others are not. Polling waits: a
+        // suspended try_wait wakes ~230 clk after the phase completes.
         if (n == 0) mbar_wait(&q_full[qb], qph);
         mbar_wait(&w_full[st], sph);
+        PP_TL(g == PP_G, 0);
+        PP_TL(g == PP_G + NF, 10);
+        if (g >= NF) {
+          mbar_wait_spin(&w_empty[sw], swph);
+          if (++sw == NST) { sw = 0; swph ^= 1; }
+        }
         tc_fence_after();
+        PP_TL(g == PP_G, 1);
+        PP_TL(g == PP_G + NF, 11);
+        PP_TL(g == PP_G, 2);
         const uint64_t a0 = dq + (uint64_t)(qb * (QTILE_BYTES >> 4));
         const uint64_t b0 = dwf + (uint64_t)(st * (WSTAGE_BYTES >> 4));
         const uint32_t acc = C_F + fb * 128;
@@ -172,6 +190,7 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
           umma_ss2(acc, a0 + (uint64_t)((k >> 2) * (QSUB_BYTES >> 4) + (k & 3) * 2),
                    b0 + (uint64_t)((k >> 2) * (BOX_BYTES >> 4) + (k & 3) * 2), idesc_f, k > 0);
         tc_commit2(&f_full[fb]);
+        PP_TL(g == PP_G, 3);
         if (++n == nstep) { tc_commit2(&q_free[qb]); n = 0; if (qb) qph ^= 1; qb ^= 1; }
         if (++st == NST) { st = 0; sph ^= 1; }
         if (++fb == NF) fb = 0;
@@ -194,10 +213,12 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
       int n = 0, u = 0, st = 0, fb = 0;
       uint32_t fph = 0;
       for (int g = 0; g < G; ++g) {
-        if (n == 0 && u > 0) mbar_wait(&o_free, (u - 1) & 1);   // O of the previous unit has been read
+        if (n == 0 && u > 0) mbar_wait_spin(&o_free, (u - 1) & 1);   // O of the previous unit has been read
         PP_ACC(3);
-        mbar_wait(&hq_ready[fb], fph);
+        PP_TL(g == PP_G, 8);
+        mbar_wait_spin(&hq_ready[fb], fph);
         tc_fence_after();
+        PP_TL(g == PP_G, 9);
         PP_ACC(4);
         const uint64_t b0 = dw2 + (uint64_t)(st * (WSTAGE_BYTES >> 4));
         const uint32_t hq = C_F + fb * 128;
@@ -205,6 +226,7 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
         for (int k = 0; k < HSTEP / 16; ++k)             // +2048 B per 16 hidden rows
           umma_ts2(C_O, hq + 8 * k, b0 + 128 * k, idesc_d, (n > 0) | k);
         tc_commit2(&w_empty[st]);
+        PP_TL(g == PP_G, 12);
         if (++n == nstep) { tc_commit2(&o_full); n = 0; ++u; }
         if (++st == NST) st = 0;
         if (++fb == NF) { fb = 0; fph ^= 1; }
@@ -223,34 +245,38 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
     }
   } else if (warp >= 4 && warp < DRAIN_WARP0) {
     // ===================== SwiGLU epilogue warps =====================
-    // Two groups of 8 warps alternate steps (three forward buffers: two in the epilogue, one being
-    // filled), so one group's TMEM load / store round trips overlap the other's MUFU burst.
-    const int ew = warp - 4, grp = ew >> 3, q = warp & 3, cg = (ew >> 2) & 1;   // lane quadrant, column half
+    // All 16 warps work on every step (4 per TMEM lane quadrant, 16 hidden columns each): the
+    // epilogue is on the critical cycle F -> epilogue -> D -> F, so its latency counts, not its
+    // throughput (two groups of 8 warps alternating steps share the MUFU pipe and take 1 350 clk per
+    // step each against 900 for the step handled by all warps).
+    const int ew = warp - 4, q = warp & 3, cg = ew >> 2;   // lane quadrant, 16-column group of the step's 64
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
     const uint64_t HALF2 = pack2(0.5f, 0.5f);
-    int fb = grp;                  // g % NF
-    uint32_t fph = 0;              // (g / NF) & 1
+    int fb = 0;
+    uint32_t fph = 0;
 #ifdef TTT_TRACE
     long long pp_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     long long pp_t = clock64();
 #endif
-    for (int g = grp; g < G; g += 2) {
+    for (int g = 0; g < G; ++g) {
       const uint32_t buf = lane_base + C_F + fb * 128;
+      PP_TL(g == PP_G && warp == 4 && lane == 0, 4);
       mbar_wait(&f_full[fb], fph);
       tc_fence_after();
+      PP_TL(g == PP_G && warp == 4 && lane == 0, 5);
       PP_ACC(0);
-      uint32_t rx[32], rb[32];
-      tmem_ld_x32(buf + 32 * cg, rx);
-      tmem_ld_x32(buf + 64 + 32 * cg, rb);
+      uint32_t rx[16], rb[16];
+      tmem_ld_x16(buf + 16 * cg, rx);
+      tmem_ld_x16(buf + 64 + 16 * cg, rb);
       tc_wait_ld();
       tc_fence_before();
       PP_ACC(1);
-      // every warp of the group holds its x | b: x may be overwritten by Hq (named barrier 1 + grp)
-      asm volatile("bar.sync %0, 256;" ::"r"(1 + grp) : "memory");
+      // every epilogue warp holds its x | b: x may be overwritten by Hq (named barrier 1, 16 warps)
+      asm volatile("bar.sync 1, 512;" ::: "memory");
       PP_ACC(2);
-      uint32_t ph[16];
+      uint32_t ph[8];
 #pragma unroll
-      for (int c = 0; c < 32; c += 2) {
+      for (int c = 0; c < 16; c += 2) {
         const uint64_t x = fmul2(pack2u(rx[c], rx[c + 1]), HALF2);   // a / 2
         float x0, x1;
         unpack2(x, x0, x1);
@@ -262,16 +288,17 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
         const uint64_t S = ffma2(x, th, x);                          // SiLU(a) = a/2 (1 + tanh(a/2))
         ph[c >> 1] = pack_bf16x2_from2(fmul2(S, pack2u(rb[c], rb[c + 1])));
       }
+      PP_TL(g == PP_G && warp == 4 && lane == 0, 6);
       PP_ACC(3);
-      tmem_st_x16(buf + 16 * cg, ph);
+      tmem_st_x8(buf + 8 * cg, ph);
       tc_wait_st();
       tc_fence_before();
       __syncwarp();
       if (lane == 0) {
         if (rank == 0) mbar_arrive(&hq_ready[fb]); else mbar_arrive_remote(&hq_ready[fb], 0);
       }
-      fb += 2;
-      if (fb >= NF) { fb -= NF; fph ^= 1; }
+      PP_TL(g == PP_G && warp == 4 && lane == 0, 7);
+      if (++fb == NF) { fb = 0; fph ^= 1; }
       PP_ACC(4);
     }
 #ifdef TTT_TRACE
@@ -280,7 +307,7 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
 #endif
   } else if (warp >= DRAIN_WARP0) {
     // ===================== O drain warps: O(unit) -> bf16 -> global =====================
-    const int q = warp & 3;
+    const int q = warp & 3, half = (warp - DRAIN_WARP0) >> 2;
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
     const int row = q * 32 + lane;                         // token row of the tile = TMEM lane
 #ifdef TTT_TRACE
@@ -289,17 +316,18 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
 #endif
     for (int u = 0; u < my_units; ++u) {
       const int unit = cid + u * ncl, h = unit / npairs, p = unit % npairs;
-      mbar_wait(&o_full, u & 1);
+      mbar_wait_spin(&o_full, u & 1);
       tc_fence_after();
       PP_ACC(0);
       const int64_t tok = (int64_t)(2 * p + (int)rank) * TM + row;
-      // the whole row is pulled into registers (packed to bf16 on the fly: 64 registers) before the
-      // first store, so the single O accumulator is released after ~8 TMEM round trips
-      uint32_t pk[64];
+      // this thread's 64 columns are pulled into registers (packed to bf16 on the fly) before the
+      // first store: the single O accumulator is released after four TMEM round trips — the drain
+      // sits between the last D of a unit and the first D of the next
+      uint32_t pk[32];
 #pragma unroll
-      for (int part = 0; part < 8; ++part) {               // 16 columns at a time
+      for (int part = 0; part < 4; ++part) {               // 16 columns at a time
         uint32_t ro[16];
-        tmem_ld_x16(lane_base + C_O + 16 * part, ro);
+        tmem_ld_x16(lane_base + C_O + 64 * half + 16 * part, ro);
         tc_wait_ld();
 #pragma unroll
         for (int v = 0; v < 8; ++v)
@@ -312,9 +340,9 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
         if (rank == 0) mbar_arrive(&o_free); else mbar_arrive_remote(&o_free, 0);
       }
       if (tok < M) {
-        uint4* dst = reinterpret_cast<uint4*>(O + tok * ld + h * HD);
+        uint4* dst = reinterpret_cast<uint4*>(O + tok * ld + h * HD + 64 * half);
 #pragma unroll
-        for (int v = 0; v < 16; ++v) dst[v] = make_uint4(pk[4 * v], pk[4 * v + 1], pk[4 * v + 2], pk[4 * v + 3]);
+        for (int v = 0; v < 8; ++v) dst[v] = make_uint4(pk[4 * v], pk[4 * v + 1], pk[4 * v + 2], pk[4 * v + 3]);
       }
       PP_ACC(2);
     }
@@ -329,6 +357,9 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
   __syncthreads();
   cluster_sync_all();
   if (warp == 0) tmem_dealloc2(tb, 512);
+#ifdef TTT_TRACE
+  if (tid == 0 && rank == 0 && cid < 80) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); g_appp_span[2 * cid + 1] = t; }
+#endif
 }
 
 // ------------------------------------------------------------------------------------------------
