@@ -316,22 +316,22 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
 #endif
     for (int u = 0; u < my_units; ++u) {
       const int unit = cid + u * ncl, h = unit / npairs, p = unit % npairs;
-      mbar_wait_spin(&o_full, u & 1);
+      mbar_wait(&o_full, u & 1);
       tc_fence_after();
       PP_ACC(0);
       const int64_t tok = (int64_t)(2 * p + (int)rank) * TM + row;
       // this thread's 64 columns are pulled into registers (packed to bf16 on the fly) before the
-      // first store: the single O accumulator is released after four TMEM round trips — the drain
+      // first store: the single O accumulator is released after two TMEM round trips — the drain
       // sits between the last D of a unit and the first D of the next
       uint32_t pk[32];
 #pragma unroll
-      for (int part = 0; part < 4; ++part) {               // 16 columns at a time
-        uint32_t ro[16];
-        tmem_ld_x16(lane_base + C_O + 64 * half + 16 * part, ro);
+      for (int part = 0; part < 2; ++part) {               // 32 columns per TMEM round trip
+        uint32_t ro[32];
+        tmem_ld_x32(lane_base + C_O + 64 * half + 32 * part, ro);
         tc_wait_ld();
 #pragma unroll
-        for (int v = 0; v < 8; ++v)
-          pk[8 * part + v] = pack_bf16x2(__uint_as_float(ro[2 * v]), __uint_as_float(ro[2 * v + 1]));
+        for (int v = 0; v < 16; ++v)
+          pk[16 * part + v] = pack_bf16x2(__uint_as_float(ro[2 * v]), __uint_as_float(ro[2 * v + 1]));
       }
       PP_ACC(1);
       tc_fence_before();
