@@ -17,7 +17,7 @@
 // single-CTA kernel: 177 us at cfg5 — both tiles' epilogues ran in lock-step, 2 000 of 3 650 clk per
 // step the issuer waited for Hq). So a unit is (head, ONE 128-token tile per CTA = 256 tokens per pair),
 // the forward accumulators x | b are triple-buffered (F(g + 3) follows the completion of D(g)), all
-// 16 epilogue warps work on the one tile, and four warps of their own drain the O accumulator to
+// 16 epilogue warps work on the one tile, and eight warps of their own drain the O accumulator to
 // global memory. TMEM (512 columns): O at 0, x | b [3] at 128 / 256 / 384 (64 + 64 columns); the bf16
 // Hq (A operand of the down MMAs) overwrites the first 32 columns of its own x once all epilogue
 // warps hold their x | b in registers.
