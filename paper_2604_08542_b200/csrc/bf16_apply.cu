@@ -145,8 +145,8 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       // The issuing thread is bound by its own serial instruction stream: absolute TMEM columns,
       // descriptors that advance by fixed steps, and one 128-wide forward MMA per K step
       // (Aq | Bq in one accumulator: W1^T and W3^T rows of a step are adjacent in shared memory).
-      constexpr uint32_t idesc_f = umma_idesc_bf16(TM, 2 * NS, 0, 0);  // B = [W1^T ; W3^T] rows, K-major
-      constexpr uint32_t idesc_d = umma_idesc_bf16(TM, HD, 0, 1);      // B = W2 rows, MN-major
+      constexpr uint32_t idesc_f = umma_idesc(TM, 2 * NS, 0, 0, TTT_FMT_F16, TTT_FMT_F16);  // A = Q (fp16 in TMEM), B = [W1^T ; W3^T] rows, K-major
+      constexpr uint32_t idesc_d = umma_idesc(TM, HD, 0, 1, TTT_FMT_F16, TTT_FMT_F16);      // A = Hq (fp16), B = W2 rows, MN-major
       const uint64_t d13 = umma_smem_desc_sw128(sbase, 16, 1024);
       const uint64_t d2 = umma_smem_desc_sw128(sbase + nsl * 16384, 8192, 1024);
       APP_TR(3);
@@ -223,7 +223,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
           float x0, x1;
           unpack2(hf, x0, x1);
           const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
-          ph[c >> 1] = pack_bf16x2_from2(fmul2(ffma2(hf, th, hf), bb));  // Hq = SiLU(a) b, SiLU(a) = h + h tanh(h)
+          ph[c >> 1] = pack_f16x2_from2(fmul2(ffma2(hf, th, hf), bb));  // Hq = SiLU(a) b, SiLU(a) = h + h tanh(h)
         }
         tmem_st_x8(buf + 8 * part, ph);          // Hq (bf16) over Aq columns this thread has already read
       }
@@ -246,7 +246,9 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
 #pragma unroll
       for (int c = 0; c < 8; ++c) {
         const uint4 x = *reinterpret_cast<const uint4*>(rowp + ((c ^ swz) << 4));
-        w[4 * c] = x.x; w[4 * c + 1] = x.y; w[4 * c + 2] = x.z; w[4 * c + 3] = x.w;
+        // bf16 -> fp16 on the way to TMEM: every MMA operand is fp16 (ttt_internal.h)
+        w[4 * c] = bf16x2_to_f16x2(x.x); w[4 * c + 1] = bf16x2_to_f16x2(x.y);
+        w[4 * c + 2] = bf16x2_to_f16x2(x.z); w[4 * c + 3] = bf16x2_to_f16x2(x.w);
       }
       mbar_arrive(&qr_empty[rs]);
       mbar_wait(&q_empty[qb], ((tl >> 1) & 1) ^ 1);

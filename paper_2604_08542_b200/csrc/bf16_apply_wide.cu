@@ -114,9 +114,9 @@ bf16_apply_wide_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_co
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (elect_one()) {
-      constexpr uint32_t idesc_f = umma_idesc_bf16(TM, 2 * HSTEP, 0, 0);   // A = Q (smem), B = [W1^T | W3^T] rows
+      constexpr uint32_t idesc_f = umma_idesc(TM, 2 * HSTEP, 0, 0, TTT_FMT_BF16, TTT_FMT_BF16);   // A = Q (smem), B = [W1^T | W3^T] rows
       const uint64_t dq = umma_smem_desc_sw128(sbase, 16, 1024);
-      constexpr uint32_t idesc_d = umma_idesc_bf16(TM, HD, 0, 1);          // A = Hq (TMEM), B = W2 rows, MN-major
+      constexpr uint32_t idesc_d = umma_idesc(TM, HD, 0, 1, TTT_FMT_BF16, TTT_FMT_BF16);          // A = Hq (TMEM), B = W2 rows, MN-major
       const uint64_t dwf = umma_smem_desc_sw128(sbase + 2 * QTILE_BYTES, 16, 1024);
       const uint64_t dw2 = umma_smem_desc_sw128(sbase + 2 * QTILE_BYTES + W2_OFF, BOX_BYTES, 1024);
       auto issueF = [&](int t, int s) {      // x | b of tile t <- Q(t) [W1^T | W3^T]^T of ring stage s
@@ -250,7 +250,7 @@ int bf16_apply_wide(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int6
   const int tiles = (int)((M + appw::TM - 1) / appw::TM);
   const int npairs = (tiles + 1) / 2;
   CUtensorMap mapW, mapQ;
-  int rc = make_token_map(ctx, &mapW, ctx->Wb, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, appw::HSTEP);
+  int rc = make_token_map(ctx, &mapW, ctx->Wq, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, appw::HSTEP);
   if (rc != TTT_OK) return rc;
   rc = make_token_map(ctx, &mapQ, Q, M, (int64_t)c.nh * c.hd, ld, appw::TM);
   if (rc != TTT_OK) return rc;

@@ -159,7 +159,7 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
     // commit ~200, a barrier probe ~90 — one thread issuing a step's 12 MMAs and 2-3 commits needs
     // ~1 000 clk against 768 clk of tensor work.
     if (rank == 0 && elect_one() && G > 0) {
-      constexpr uint32_t idesc_f = umma_idesc_bf16(2 * TM, 2 * HSTEP, 0, 0);   // A = Q (smem), B = forward rows, K-major
+      constexpr uint32_t idesc_f = umma_idesc(2 * TM, 2 * HSTEP, 0, 0, TTT_FMT_BF16, TTT_FMT_BF16);   // A = Q (smem), B = forward rows, K-major
       const uint64_t dq = umma_smem_desc_sw128(sbase, 16, 1024);
       const uint64_t dwf = umma_smem_desc_sw128(sbase + 2 * QTILE_BYTES, 16, 1024);
       // x | b of step g <- Q(unit) [W1^T | W3^T]^T of the step's ring stage. F(g) overwrites the
@@ -199,7 +199,7 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
   } else if (warp == 2) {
     // ===================== down-MMA issuer (rank 0 only) =====================
     if (rank == 0 && elect_one() && G > 0) {
-      constexpr uint32_t idesc_d = umma_idesc_bf16(2 * TM, HD, 0, 1);          // A = Hq (TMEM), B = W2 rows, MN-major
+      constexpr uint32_t idesc_d = umma_idesc(2 * TM, HD, 0, 1, TTT_FMT_BF16, TTT_FMT_BF16);          // A = Hq (TMEM), B = W2 rows, MN-major
       const uint64_t dw2 = umma_smem_desc_sw128(sbase + 2 * QTILE_BYTES + W2_OFF, BOX_BYTES, 1024);
 #ifdef TTT_TRACE
       long long pp_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -371,7 +371,7 @@ int bf16_apply_wide_pair(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O,
   const int tiles = (int)((M + appp::TM - 1) / appp::TM);
   const int npairs = (tiles + 1) / 2;
   CUtensorMap mapW, mapQ;
-  int rc = make_token_map(ctx, &mapW, ctx->Wb, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, appp::HSTEP);
+  int rc = make_token_map(ctx, &mapW, ctx->Wq, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, appp::HSTEP);
   if (rc != TTT_OK) return rc;
   rc = make_token_map(ctx, &mapQ, Q, M, (int64_t)c.nh * c.hd, ld, appp::TM);
   if (rc != TTT_OK) return rc;

@@ -95,10 +95,10 @@ constexpr uint32_t C_H = 448;                             // bf16 operands dA2 |
 template <bool LOSS>
 __global__ void __launch_bounds__(upd::THREADS, 1)
 bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
-                   const __nv_bfloat16* __restrict__ Wb, const float* __restrict__ lr,
+                   const ttt_wop_t* __restrict__ Wb, const float* __restrict__ lr,
                    float* __restrict__ P, float* __restrict__ loss_part, int M, int nh, int H,
                    int tiles_total, int tiles_per_split, float* __restrict__ Wm,
-                   __nv_bfloat16* __restrict__ Wbw, unsigned* __restrict__ sync_ctr,
+                   ttt_wop_t* __restrict__ Wbw, unsigned* __restrict__ sync_ctr,
                    unsigned sync_target, const float* __restrict__ renorm_n0,
                    float* __restrict__ renorm_colsq) {
   using namespace upd;
@@ -107,11 +107,12 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   // 1024-B aligned base, computed on the 32-bit shared-space address (a uniform value)
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
-  __shared__ uint64_t full[STAGES], empty[STAGES], fwd_full[2], xb_free[2], g_free,
-      epi_done[2], opnd_free, w_ready, grad_done;
+  __shared__ uint64_t tma_full[STAGES], full[STAGES], empty[STAGES], fwd_full[2], xb_free[2], g_free,
+      epi_done[2], opnd_free[2], w_ready, grad_done;
   __shared__ uint32_t tmem_base_s;
   __shared__ float loss_red[EPI_WARPS];
-  __shared__ __align__(16) float ne_s[STAGES][T];   // -eta of the stage's tokens (0 beyond M)
+  __shared__ float lrmax_s[THREADS / 32];
+  __shared__ __align__(16) float ne_s[STAGES][T];   // -eta of the stage's tokens, scaled (0 beyond M)
 #ifdef TTT_TRACE
   __shared__ unsigned tr_s[64 * 16];
   for (int e = threadIdx.x; e < 64 * 16; e += blockDim.x) tr_s[e] = 0;
@@ -145,25 +146,26 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     tma_prefetch_desc(&mapV);
     TTT_TR(9, 14);
 #pragma unroll
-    for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 2);
+    for (int s = 0; s < STAGES; ++s) mbar_init(&tma_full[s], 1);
     TTT_TR(10, 14);
     fence_mbar_init();
     TTT_TR(1, 14);
     const int npre = min(ntiles, STAGES);
     for (int i = 0; i < npre; ++i) {
-      mbar_arrive_expect_tx(&full[i], STAGE_BYTES);
+      mbar_arrive_expect_tx(&tma_full[i], STAGE_BYTES);
       uint8_t* dst = smem + i * STAGE_BYTES;
-      tma_load_2d(dst, &mapK, &full[i], h * HD, (tile_lo + i) * T);
-      tma_load_2d(dst + TILE_BYTES, &mapV, &full[i], h * HD, (tile_lo + i) * T);
+      tma_load_2d(dst, &mapK, &tma_full[i], h * HD, (tile_lo + i) * T);
+      tma_load_2d(dst + TILE_BYTES, &mapV, &tma_full[i], h * HD, (tile_lo + i) * T);
     }
     TTT_TR(2, 14);
   } else if (tid == 32) {
 #pragma unroll
-    for (int s = 0; s < STAGES; ++s) mbar_init(&empty[s], 1);
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&empty[s], 1); mbar_init(&full[s], 1); }
     mbar_init(&fwd_full[0], 1);
     mbar_init(&fwd_full[1], 1);
     mbar_init(&g_free, EPI_WARPS / 2);
-    mbar_init(&opnd_free, 1);
+    mbar_init(&opnd_free[0], 1);
+    mbar_init(&opnd_free[1], 1);
     for (int b = 0; b < 2; ++b) { mbar_init(&epi_done[b], EPI_WARPS / 2); mbar_init(&xb_free[b], EPI_WARPS / 2); }
     mbar_init(&w_ready, EPI_WARPS);
     mbar_init(&grad_done, 1);
@@ -194,6 +196,17 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       lr_pre[u] = (u < ntiles && t < M) ? __ldg(lr + (size_t)h * M + t) : 0.f;   // negated after the barrier
     }
   }
+  // max |eta| over the CTA's token range (all threads; the loads overlap the first TMA round trip)
+  {
+    const float* lrh = lr + (size_t)h * M;
+    const int t_hi = min(M, (tile_lo + ntiles) * T);
+    float mx = 0.f;
+#pragma unroll 4
+    for (int t = tile_lo * T + tid; t < t_hi; t += THREADS) mx = fmaxf(mx, fabsf(__ldg(lrh + t)));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if (lane == 0) lrmax_s[warp] = mx;
+  }
   if (warp == 3) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
   if (tid == 96) TTT_TR(3, 14);
   if (tid == 255) TTT_TR(4, 14);
@@ -206,6 +219,13 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   const uint32_t tb = tmem_base_s;
   if (tb != 0) __trap();      // all 512 columns belong to this CTA: the issuers use absolute columns
   if (tid == 0) TTT_TR(0, 14);
+  float eta_sc, eta_isc;      // the gradient operands carry eta * eta_sc; undone at the flush
+  {
+    float mx = 0.f;
+#pragma unroll
+    for (int w = 0; w < THREADS / 32; ++w) mx = fmaxf(mx, lrmax_s[w]);
+    eta_scale(mx, eta_sc, eta_isc);
+  }
 
   if (warp == 0) {
     // ===================== TMA producer =====================
@@ -214,10 +234,10 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         const int s = i % STAGES, it = i / STAGES;
         mbar_wait(&empty[s], (it & 1) ^ 1);
         TTT_TR(i, 12);
-        mbar_arrive_expect_tx(&full[s], STAGE_BYTES);
+        mbar_arrive_expect_tx(&tma_full[s], STAGE_BYTES);
         uint8_t* dst = smem + s * STAGE_BYTES;
-        tma_load_2d(dst, &mapK, &full[s], h * HD, (tile_lo + i) * T);
-        tma_load_2d(dst + TILE_BYTES, &mapV, &full[s], h * HD, (tile_lo + i) * T);
+        tma_load_2d(dst, &mapK, &tma_full[s], h * HD, (tile_lo + i) * T);
+        tma_load_2d(dst + TILE_BYTES, &mapV, &tma_full[s], h * HD, (tile_lo + i) * T);
       }
     }
   } else if (warp == 1) {
@@ -226,7 +246,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     // everything it needs per tile is a constant or an increment: the CTA owns all 512 TMEM columns
     // (base 0, checked above), stage descriptors advance by a fixed step, phases are flipped bits.
     if (elect_one()) {
-      constexpr uint32_t idesc_f = umma_idesc_bf16(HS, T, 0, 0);    // B = token tile, K-major
+      constexpr uint32_t idesc_f = umma_idesc(HS, T, 0, 0, TTT_FMT_F16, TTT_FMT_F16);   // A = weights, B = token tile (fp16), K-major
       constexpr uint32_t V_OFF = TILE_BYTES >> 4, ST_OFF = STAGE_BYTES >> 4;   // descriptor steps (16-B units)
       const uint64_t d0 = umma_smem_desc_sw128(sbase, 16, 1024);
       mbar_wait(&w_ready, 0);
@@ -263,7 +283,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   } else if (warp == 3) {
     // ===================== gradient-MMA issuer =====================
     if (elect_one()) {
-      constexpr uint32_t idesc_g = umma_idesc_bf16(HS, HD, 0, 1);   // B = token tile, MN-major
+      constexpr uint32_t idesc_g = umma_idesc(HS, HD, 0, 1, TTT_FMT_F16, TTT_FMT_F16);   // A = fp16 operands, B = token tile (fp16), MN-major
       constexpr uint32_t V_OFF = TILE_BYTES >> 4, ST_OFF = STAGE_BYTES >> 4;
       const uint64_t d0 = umma_smem_desc_sw128(sbase, TILE_BYTES, 1024);
       int s = 0;
@@ -286,27 +306,29 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
           umma_ts(C_G2, C_H + 32 + 8 * k, dk + V_OFF + 128 * k, idesc_g, acc_flag | k);
 #endif
         tc_commit(&empty[s]);          // the tile's forward MMAs completed long ago (epilogue read them)
-        tc_commit(&opnd_free);
+        tc_commit(&opnd_free[b]);     // one barrier per tile parity (see the epilogue's wait)
         TTT_TR(i, 4);
         if (++s == STAGES) { s = 0; dk = d0; } else { dk += ST_OFF; }
       }
       tc_commit(&grad_done);
     }
   } else if (warp == 2) {
-    // ===================== learning-rate loader =====================
-    // -eta of tile i (32 tokens = one 128-B line of lr) goes to the stage's shared-memory slot. The
-    // global loads run LRPF tiles ahead of the ring (register double buffer).
+    // ===================== stage finisher: fp16 conversion + learning rates =====================
+    // When the TMA has landed a stage, this warp converts its K and V tiles from bf16 to fp16 in place
+    // (all MMA operands are fp16, ttt_internal.h) and puts -eta of the tile's 32 tokens (one 128-B line
+    // of lr, scaled by the CTA's power of two) into the stage's slot; then the stage is `full`. The
+    // global loads of lr run LRPF tiles ahead of the ring (register double buffer).
     const float* lrh = lr + (size_t)h * M;
     auto ld_batch = [&](int i0, float (&v)[LRPF]) {
 #pragma unroll
       for (int u = 0; u < LRPF; ++u) {
         const int t = (tile_lo + i0 + u) * T + lane;
-        v[u] = (i0 + u < ntiles && t < M) ? -__ldg(lrh + t) : 0.f;
+        v[u] = (i0 + u < ntiles && t < M) ? -eta_sc * __ldg(lrh + t) : 0.f;
       }
     };
     float cur[LRPF], nxt[LRPF];
 #pragma unroll
-    for (int u = 0; u < LRPF; ++u) cur[u] = -lr_pre[u];      // requested before the allocation barrier
+    for (int u = 0; u < LRPF; ++u) cur[u] = -eta_sc * lr_pre[u];   // requested before the allocation barrier
     for (int i0 = 0; i0 < ntiles; i0 += LRPF) {
       ld_batch(i0 + LRPF, nxt);
 #pragma unroll
@@ -314,8 +336,10 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         const int i = i0 + u;
         if (i < ntiles) {
           const int s = i % STAGES, it = i / STAGES;
-          if (it > 0) mbar_wait(&empty[s], (it & 1) ^ 1);
+          mbar_wait(&tma_full[s], it & 1);       // (the TMA was issued after the stage's `empty`)
+          tile_bf16_to_f16<STAGE_BYTES / 512>(smem + s * STAGE_BYTES, lane);
           ne_s[s][lane] = cur[u];
+          fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) mbar_arrive(&full[s]);
 
@@ -344,8 +368,10 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
                          x[mat][1].x, x[mat][1].y, x[mat][1].z, x[mat][1].w};
         if (mat == 0) {
 #pragma unroll
-          for (int e = 0; e < 8; ++e)      // W1 / 2: the accumulator becomes the tanh argument a / 2
-            r[e] = pack_bf16x2(0.5f * __uint_as_float(r[e] << 16), 0.5f * __uint_as_float(r[e] & 0xffff0000u));
+          for (int e = 0; e < 8; ++e) {    // W1 / 2: the accumulator becomes the tanh argument a / 2
+            const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&r[e]));
+            r[e] = pack_f16x2(0.5f * f.x, 0.5f * f.y);
+          }
         }
         tmem_st_x8(tb + lane_base + cols[mat] + 8 * tc, r);
       }
@@ -409,15 +435,19 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         const uint64_t m = ffma2(th, NONE2, ONE2);           // 2 (1 - sigmoid(a))
         const uint64_t t2 = ffma2(S, m, p);                  // 2 SiLU'(a)
         const uint64_t hdv = fmul2(S, bb);                   // hidden activation Hd
-        pa[c >> 1] = pack_bf16x2_from2(fmul2(fmul2(g, bb), t2));   // 2 dA
-        pb[c >> 1] = pack_bf16x2_from2(fmul2(g, S));               // dB
-        ph[c >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));            // Hd' = -eta Hd
+        pa[c >> 1] = pack_f16x2_from2(fmul2(fmul2(g, bb), t2));   // 2 dA
+        pb[c >> 1] = pack_f16x2_from2(fmul2(g, S));               // dB
+        ph[c >> 1] = pack_f16x2_from2(fmul2(ne, hdv));            // Hd' = -eta Hd
         if (LOSS) loss2 = ffma2(hdv, g, loss2);
       }
       if (ew == 0 && lane == 0) TTT_TR(i, 8);
       TTT_TR2(i, ew, 2);
       // the operand buffer was last read by the gradient MMAs of tile i - 1
-      if (i > 0) { mbar_wait(&opnd_free, (i - 1) & 1); tc_fence_after(); }
+      // (an epilogue group sees every OTHER tile: on one barrier shared by both tile parities its
+      // parity wait could not tell "tile i - 1 done" from "tile i - 3 done" when the gradient issuer
+      // lags by two tiles, and a fast warp would overwrite operands not yet read; with one barrier per
+      // tile parity the phase it waits for is always the barrier's current or latest completed one)
+      if (i > 0) { mbar_wait(&opnd_free[grp ^ 1], ((i - 1) >> 1) & 1); tc_fence_after(); }
       if (ew == 0 && lane == 0) TTT_TR(i, 10);
 #ifdef TTT_EXP_NOTMEM
       if (pa[0] + pb[1] + ph[2] == 0x12345u) tmem_st_x8(hbuf, pa);
@@ -460,7 +490,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
 #pragma unroll
         for (int u = 0; u < 16; ++u) r[u] = 0u;
       }
-      const float sc = mat == 0 ? 0.5f : 1.0f;             // G1 was accumulated from 2 dA
+      const float sc = (mat == 0 ? 0.5f : 1.0f) * eta_isc; // G1 was accumulated from 2 dA; eta scale undone
       float* sb = stg + (mat & 1) * HS * SLD;
       float4* d = reinterpret_cast<float4*>(sb + j * SLD + 16 * tc);
 #pragma unroll
@@ -487,7 +517,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       if (ew == 0 && lane == 0) {
         float t = 0.f;
         for (int w = 0; w < EPI_WARPS; ++w) t += loss_red[w];
-        loss_part[((size_t)split * nslices + slice) * nh + h] = t;
+        loss_part[((size_t)split * nslices + slice) * nh + h] = t * eta_isc;
       }
     }
   }
@@ -576,7 +606,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         }
         if (ok[k]) {
           *reinterpret_cast<float4*>(Wm + off[k]) = w[k];
-          *reinterpret_cast<uint2*>(Wbw + off[k]) = make_uint2(pack_bf16x2(w[k].x, w[k].y), pack_bf16x2(w[k].z, w[k].w));
+          *reinterpret_cast<uint2*>(Wbw + off[k]) = make_uint2(ttt_pack_wop2(w[k].x, w[k].y), ttt_pack_wop2(w[k].z, w[k].w));
         }
       }
     }
@@ -709,11 +739,11 @@ int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V
   // fused commit: the CTAs of a (head, slice) group wait on one another, so they must all be
   // resident -> cooperative launch (fails instead of deadlocking if the device cannot hold them)
   fuse_commit = fuse_commit && (int)(grid.x * grid.y * grid.z) <= ctx->sm_count;
-  const __nv_bfloat16* Wb = ctx->Wb;
+  const ttt_wop_t* Wb = ctx->Wb;
   float* loss_part = ctx->loss_part;
   int Mi = (int)M, nh = c.nh, H = c.hidden;
   float* Wm = fuse_commit ? ctx->Wm : nullptr;
-  __nv_bfloat16* Wbw = fuse_commit ? ctx->Wb : nullptr;
+  ttt_wop_t* Wbw = fuse_commit ? ctx->Wb : nullptr;
   unsigned* ctr = ctx->sync_ctr;
   if (fuse_commit) ctx->sync_target += (unsigned)splits;
   unsigned target = ctx->sync_target;

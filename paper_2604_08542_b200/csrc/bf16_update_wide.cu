@@ -79,10 +79,11 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
   uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
   uint8_t* ring = smem + W_BYTES;
   float* stg = reinterpret_cast<float*>(ring + STAGES * STAGE_BYTES);
-  __shared__ uint64_t full[STAGES], empty[STAGES], w_full, fwd_full, xbg_free, opnd_ready, opnd_free, grad_done;
+  __shared__ uint64_t tma_full[STAGES], full[STAGES], empty[STAGES], w_full, fwd_full, xbg_free, opnd_ready, opnd_free, grad_done;
   __shared__ uint32_t tmem_base_s;
   __shared__ float loss_red[EPI_WARPS];
-  __shared__ __align__(16) float ne_s[STAGES][T];   // -eta of the stage's tokens (0 beyond M)
+  __shared__ float lrmax_s[THREADS / 32];
+  __shared__ __align__(16) float ne_s[STAGES][T];   // -eta of the stage's tokens, scaled (0 beyond M)
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int nslices = H / HS;
@@ -101,12 +102,12 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
     int pair, tile;
     locate(gi, pair, tile);
     const int s = gi % STAGES, h = pair % nh, row = tile * T;
-    mbar_arrive_expect_tx(&full[s], STAGE_BYTES);
+    mbar_arrive_expect_tx(&tma_full[s], STAGE_BYTES);
     uint8_t* dst = ring + s * STAGE_BYTES;
-    tma_load_2d(dst, &mapK, &full[s], h * HD, row);
-    tma_load_2d(dst + SUB_BYTES, &mapK, &full[s], h * HD + 64, row);
-    tma_load_2d(dst + TILE_BYTES, &mapV, &full[s], h * HD, row);
-    tma_load_2d(dst + TILE_BYTES + SUB_BYTES, &mapV, &full[s], h * HD + 64, row);
+    tma_load_2d(dst, &mapK, &tma_full[s], h * HD, row);
+    tma_load_2d(dst + SUB_BYTES, &mapK, &tma_full[s], h * HD + 64, row);
+    tma_load_2d(dst + TILE_BYTES, &mapV, &tma_full[s], h * HD, row);
+    tma_load_2d(dst + TILE_BYTES + SUB_BYTES, &mapV, &tma_full[s], h * HD + 64, row);
   };
   // weights of a pair: mat m (0 = W1^T, 1 = W2, 2 = W3^T), hd half c -> [128 rows x 64] sub-tile
   auto load_weights = [&](int pair) {
@@ -119,7 +120,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
   };
 
   if (tid == 0) {
-    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 2); mbar_init(&empty[s], 1); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&tma_full[s], 1); mbar_init(&full[s], 2); mbar_init(&empty[s], 1); }
     mbar_init(&w_full, 1);
     mbar_init(&fwd_full, 1);
     mbar_init(&xbg_free, 1);
@@ -135,12 +136,35 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
     for (int gi = 0; gi < npre; ++gi) load_stage(gi);
   }
   __syncwarp();
+  // max |eta| over the tokens of all of this CTA's segments (all threads; overlaps the first TMA round trip)
+  {
+    float mx = 0.f;
+    for (long long u = lo; u < hi;) {
+      const int pair = (int)(u / tiles_total), t0 = (int)(u - (long long)pair * tiles_total);
+      const int n = (int)min(hi - u, (long long)(tiles_total - t0));
+      const float* lrh = lr + (size_t)(pair % nh) * M;
+      const int t_hi = min(M, (t0 + n) * T);
+#pragma unroll 4
+      for (int t = t0 * T + tid; t < t_hi; t += THREADS) mx = fmaxf(mx, fabsf(__ldg(lrh + t)));
+      u += n;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if (lane == 0) lrmax_s[warp] = mx;
+  }
   if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tb = tmem_base_s;
   if (tb != 0) __trap();      // all 512 columns belong to this CTA: the issuer uses absolute columns
+  float eta_sc, eta_isc;      // the gradient operands carry eta * eta_sc; undone at the flush
+  {
+    float mx = 0.f;
+#pragma unroll
+    for (int w = 0; w < THREADS / 32; ++w) mx = fmaxf(mx, lrmax_s[w]);
+    eta_scale(mx, eta_sc, eta_isc);
+  }
 
   if (warp == 0) {
     // ===================== TMA producer =====================
@@ -153,8 +177,8 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
   } else if (warp == 1) {
     // ===================== MMA issuer (forward and gradients) =====================
     if (elect_one()) {
-      constexpr uint32_t idesc_f = umma_idesc_bf16(HS, T, 0, 0);    // A = weights, B = token tile, K-major
-      constexpr uint32_t idesc_g = umma_idesc_bf16(HS, HD, 0, 1);   // A = TMEM operand, B = token tile, MN-major
+      constexpr uint32_t idesc_f = umma_idesc(HS, T, 0, 0, TTT_FMT_F16, TTT_FMT_F16);    // A = weights, B = token tile (fp16), K-major
+      constexpr uint32_t idesc_g = umma_idesc(HS, HD, 0, 1, TTT_FMT_F16, TTT_FMT_F16);   // A = fp16 TMEM operand, B = token tile (fp16), MN-major
       const uint64_t dw = umma_smem_desc_sw128(sbase, 16, 1024);
       const uint64_t dr_k = umma_smem_desc_sw128(sbase + W_BYTES, 16, 1024);
       const uint64_t dr_mn = umma_smem_desc_sw128(sbase + W_BYTES, SUB_BYTES, 1024);   // 2nd hd atom: +SUB_BYTES
@@ -237,9 +261,11 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
 #endif
     }
   } else if (warp == 2) {
-    // ===================== learning-rate loader =====================
-    // -eta of a tile (32 tokens = one 128-B line of lr) goes to the stage's shared-memory slot; the
-    // global loads run LRPF tiles ahead of the ring (register double buffer)
+    // ===================== stage finisher 1: K tile -> fp16, learning rates =====================
+    // When the TMA has landed a stage, this warp converts its K tile from bf16 to fp16 in place (all MMA
+    // operands are fp16, ttt_internal.h; warp 3 does the V tile) and puts -eta of the tile's 32 tokens
+    // (one 128-B line of lr, scaled by the CTA's power of two) into the stage's slot; the global loads
+    // of lr run LRPF tiles ahead of the ring (register double buffer)
     constexpr int LRPF = 4;
     auto ld_batch = [&](int g0, float (&v)[LRPF]) {
 #pragma unroll
@@ -249,7 +275,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
           int pair, tile;
           locate(g0 + u, pair, tile);
           const int t = tile * T + lane;
-          if (t < M) x = -__ldg(lr + (size_t)(pair % nh) * M + t);
+          if (t < M) x = -eta_sc * __ldg(lr + (size_t)(pair % nh) * M + t);
         }
         v[u] = x;
       }
@@ -263,14 +289,26 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
         const int gi = g0 + u;
         if (gi < total) {
           const int s = gi % STAGES, it = gi / STAGES;
-          if (it > 0) mbar_wait(&empty[s], (it & 1) ^ 1);
+          mbar_wait(&tma_full[s], it & 1);       // (the TMA was issued after the stage's `empty`)
+          tile_bf16_to_f16<TILE_BYTES / 512>(ring + s * STAGE_BYTES, lane);
           ne_s[s][lane] = cur[u];
+          fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) mbar_arrive(&full[s]);
         }
       }
 #pragma unroll
       for (int u = 0; u < LRPF; ++u) cur[u] = nxt[u];
+    }
+  } else if (warp == 3) {
+    // ===================== stage finisher 2: V tile -> fp16 =====================
+    for (int gi = 0; gi < total; ++gi) {
+      const int s = gi % STAGES;
+      mbar_wait(&tma_full[s], (gi / STAGES) & 1);
+      tile_bf16_to_f16<TILE_BYTES / 512>(ring + s * STAGE_BYTES + TILE_BYTES, lane);
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&full[s]);
     }
   } else if (warp >= 4) {
     // ===================== epilogue warps =====================
@@ -315,9 +353,9 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
           const uint64_t m = ffma2(th, NONE2, ONE2);           // 2 (1 - sigmoid(a))
           const uint64_t t2 = ffma2(S, m, p);                  // 2 SiLU'(a)
           const uint64_t hdv = fmul2(S, bb);                   // hidden activation Hd
-          pa[c >> 1] = pack_bf16x2_from2(fmul2(fmul2(g, bb), t2));   // 2 dA
-          pb[c >> 1] = pack_bf16x2_from2(fmul2(g, S));               // dB
-          ph[c >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));            // Hd' = -eta Hd
+          pa[c >> 1] = pack_f16x2_from2(fmul2(fmul2(g, bb), t2));   // 2 dA
+          pb[c >> 1] = pack_f16x2_from2(fmul2(g, S));               // dB
+          ph[c >> 1] = pack_f16x2_from2(fmul2(ne, hdv));            // Hd' = -eta Hd
           if (LOSS) loss2 = ffma2(hdv, g, loss2);
         }
         // Hd' columns: their last readers (W2-gradient MMAs of the previous tile) were issued before the x
@@ -356,7 +394,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
       const int et = ew * 32 + lane;                         // 0 .. 255
 #pragma unroll
       for (int mat = 0; mat < 3; ++mat) {
-        const float sc = mat == 0 ? 0.5f : 1.0f;             // G1 was accumulated from 2 dA
+        const float sc = (mat == 0 ? 0.5f : 1.0f) * eta_isc; // G1 was accumulated from 2 dA; eta scale undone
 #pragma unroll
         for (int p = 0; p < 2; ++p) {                        // column half; its four warps fill the stage
           if (kh == p) {
@@ -399,7 +437,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
         if (ew == 0 && lane == 0) {
           float t = 0.f;
           for (int w = 0; w < EPI_WARPS; ++w) t += loss_red[w];
-          loss_part[((size_t)ord * nslices + slice) * nh + h] = t;
+          loss_part[((size_t)ord * nslices + slice) * nh + h] = t * eta_isc;
           if (pair_done)
             for (int z = ord + 1; z < nsets; ++z) loss_part[((size_t)z * nslices + slice) * nh + h] = 0.f;
         }

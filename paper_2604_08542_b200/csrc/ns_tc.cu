@@ -75,7 +75,7 @@ __device__ __forceinline__ uint32_t sw128_off(int row, int chunk) {
 __global__ void __launch_bounds__(nstc::LAUNCH_THREADS, 1)
 ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, size_t set_elems,
              int use_G, int H, int iters, uint32_t tmem_cols, float* __restrict__ Wm,
-             __nv_bfloat16* __restrict__ Wb) {
+             ttt_wop_t* __restrict__ Wb) {
   using namespace nstc;
   constexpr int HD = 64;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -355,7 +355,7 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
           w[u].x -= x.x; w[u].y -= x.y; w[u].z -= x.z; w[u].w -= x.w;
           reinterpret_cast<float4*>(Wm + mat_off)[e] = w[u];
           reinterpret_cast<uint2*>(Wb + mat_off)[e] =
-              make_uint2(pack_bf16x2(w[u].x, w[u].y), pack_bf16x2(w[u].z, w[u].w));
+              make_uint2(ttt_pack_wop2(w[u].x, w[u].y), ttt_pack_wop2(w[u].z, w[u].w));
         } else {
           reinterpret_cast<float4*>(X)[e] = x;
         }
@@ -404,7 +404,7 @@ int launch_ns_tc(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s) {
   int n_sets = ctx->n_partials, use_G = ctx->G_valid ? 1 : 0, H = c.hidden, iters = c.ns_iters;
   size_t set_elems = 3 * ctx->mat_elems;
   float* Wm = fuse_commit ? ctx->Wm : nullptr;
-  __nv_bfloat16* Wb = fuse_commit ? ctx->Wb : nullptr;
+  ttt_wop_t* Wb = fuse_commit ? ctx->Wb : nullptr;
   cudaError_t e = cudaLaunchKernelEx(&cfg, ns_tc_kernel, G, P, n_sets, set_elems, use_G, H, iters, alloc, Wm, Wb);
   if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, "ns_tc_kernel launch", e);
   TTT_LAUNCH_CHECK(ctx, "ns_tc_kernel");

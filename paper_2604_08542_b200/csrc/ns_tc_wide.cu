@@ -97,7 +97,7 @@ __device__ __forceinline__ void split_row32(const float (&v)[32], uint8_t* hi_ti
 
 __global__ void __launch_bounds__(nsw::LAUNCH_THREADS, 1)
 ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, size_t set_elems,
-                  int use_G, int H, int iters, float* __restrict__ Wm, __nv_bfloat16* __restrict__ Wb,
+                  int use_G, int H, int iters, float* __restrict__ Wm, ttt_wop_t* __restrict__ Wb, __nv_bfloat16* __restrict__ Wq,
                   float* __restrict__ scratch) {
   using namespace nsw;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -347,6 +347,7 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
         if (Wm != nullptr) {
           float4* wm = reinterpret_cast<float4*>(Wm + blk);
           uint2* wb = reinterpret_cast<uint2*>(Wb + blk);
+          uint2* wq = reinterpret_cast<uint2*>(Wq + blk);      // bf16 copy for the apply kernel
           float4 w[8];
 #pragma unroll
           for (int k = 0; k < 8; ++k) w[k] = wm[tid + THREADS * k];
@@ -355,7 +356,8 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
             const float4 d = *reinterpret_cast<const float4*>(ex_co(k));
             w[k].x -= d.x; w[k].y -= d.y; w[k].z -= d.z; w[k].w -= d.w;
             wm[tid + THREADS * k] = w[k];
-            wb[tid + THREADS * k] = make_uint2(pack_bf16x2(w[k].x, w[k].y), pack_bf16x2(w[k].z, w[k].w));
+            wb[tid + THREADS * k] = make_uint2(ttt_pack_wop2(w[k].x, w[k].y), ttt_pack_wop2(w[k].z, w[k].w));
+            wq[tid + THREADS * k] = make_uint2(pack_bf16x2(w[k].x, w[k].y), pack_bf16x2(w[k].z, w[k].w));
           }
         } else {
           float4* gd = reinterpret_cast<float4*>(G + blk);
@@ -406,8 +408,8 @@ int launch_ns_tc_wide(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s) {
   int n_sets = ctx->n_partials, use_G = ctx->G_valid ? 1 : 0, H = c.hidden, iters = c.ns_iters;
   size_t set_elems = 3 * ctx->mat_elems;
   float* Wm = fuse_commit ? ctx->Wm : nullptr;
-  __nv_bfloat16* Wb = fuse_commit ? ctx->Wb : nullptr;
-  cudaError_t e = cudaLaunchKernelEx(&cfg, ns_tc_wide_kernel, G, P, n_sets, set_elems, use_G, H, iters, Wm, Wb, ctx->ns_scratch);
+  ttt_wop_t* Wb = fuse_commit ? ctx->Wb : nullptr;
+  cudaError_t e = cudaLaunchKernelEx(&cfg, ns_tc_wide_kernel, G, P, n_sets, set_elems, use_G, H, iters, Wm, Wb, ctx->Wq, ctx->ns_scratch);
   if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, "ns_tc_wide_kernel launch", e);
   TTT_LAUNCH_CHECK(ctx, "ns_tc_wide_kernel");
   ctx->G_valid = !fuse_commit;

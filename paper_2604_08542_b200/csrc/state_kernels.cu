@@ -36,15 +36,16 @@ __device__ __forceinline__ float warp_sum(float v) {
 // ------------------------------------------------------------------------------------------------
 __global__ void init_load_kernel(const float* __restrict__ W1, const float* __restrict__ W2,
                                  const float* __restrict__ W3, float* __restrict__ Wm,
-                                 __nv_bfloat16* __restrict__ Wb, float* __restrict__ n0,
-                                 float* __restrict__ colsq, int nh, int hd, int H) {
+                                 ttt_wop_t* __restrict__ Wb, __nv_bfloat16* __restrict__ Wq,
+                                 float* __restrict__ n0, float* __restrict__ colsq, int nh, int hd, int H) {
   __shared__ float tile[32][33];
   __shared__ float cs[8][128];
   const int mat = blockIdx.z, h = blockIdx.y, j0 = blockIdx.x * 32;
   const int tx = threadIdx.x, ty = threadIdx.y;
   const size_t me = (size_t)nh * H * hd;
   float* dst = Wm + mat * me + (size_t)h * H * hd;
-  __nv_bfloat16* dstb = Wb + mat * me + (size_t)h * H * hd;
+  ttt_wop_t* dstb = Wb + mat * me + (size_t)h * H * hd;
+  __nv_bfloat16* dstq = Wq ? Wq + mat * me + (size_t)h * H * hd : nullptr;
   if (mat == 1) {  // W2 [H][hd]: straight copy + column sums of squares over this CTA's rows
     const float* src = W2 + (size_t)h * H * hd;
     float colacc[4] = {0.f, 0.f, 0.f, 0.f};
@@ -57,7 +58,8 @@ __global__ void init_load_kernel(const float* __restrict__ W1, const float* __re
         if (i < hd) {
           const float v = src[(size_t)j * hd + i];
           dst[(size_t)j * hd + i] = v;
-          dstb[(size_t)j * hd + i] = __float2bfloat16_rn(v);
+          dstb[(size_t)j * hd + i] = ttt_to_wop(v);
+          if (dstq) dstq[(size_t)j * hd + i] = __float2bfloat16_rn(v);
           colacc[c] = fmaf(v, v, colacc[c]);
         }
       }
@@ -86,7 +88,8 @@ __global__ void init_load_kernel(const float* __restrict__ W1, const float* __re
       if (j < H && i < hd) {
         const float v = tile[tx][r];
         dst[(size_t)j * hd + i] = v;
-        dstb[(size_t)j * hd + i] = __float2bfloat16_rn(v);
+        dstb[(size_t)j * hd + i] = ttt_to_wop(v);
+        if (dstq) dstq[(size_t)j * hd + i] = __float2bfloat16_rn(v);
         rowacc[k] = fmaf(v, v, rowacc[k]);
       }
     }
@@ -265,7 +268,8 @@ constexpr int CM_ROWS = 16;
 
 // float4 per thread, `tpr` (power of two >= hd/4, <= 32) threads per row, 256/tpr rows per pass.
 __global__ void __launch_bounds__(256)
-commit_kernel(float* __restrict__ Wm, __nv_bfloat16* __restrict__ Wb, const float* __restrict__ G,
+commit_kernel(float* __restrict__ Wm, ttt_wop_t* __restrict__ Wb, __nv_bfloat16* __restrict__ Wq,
+              const float* __restrict__ G,
               const float* __restrict__ P, int n_sets, int use_G, const float* __restrict__ n0,
               float* __restrict__ colsq, int renorm, int nh, int hd, int H, int tpr) {
   __shared__ float4 cs[256];
@@ -312,11 +316,12 @@ commit_kernel(float* __restrict__ Wm, __nv_bfloat16* __restrict__ Wb, const floa
     }
     if (ok) {
       *reinterpret_cast<float4*>(Wm + e) = w;
-      __nv_bfloat162 lo = __floats2bfloat162_rn(w.x, w.y), hi = __floats2bfloat162_rn(w.z, w.w);
-      uint2 packed;
-      packed.x = *reinterpret_cast<uint32_t*>(&lo);
-      packed.y = *reinterpret_cast<uint32_t*>(&hi);
-      *reinterpret_cast<uint2*>(Wb + e) = packed;
+      *reinterpret_cast<uint2*>(Wb + e) = make_uint2(ttt_pack_wop2(w.x, w.y), ttt_pack_wop2(w.z, w.w));
+      if (Wq) {
+        const __nv_bfloat162 lo = __floats2bfloat162_rn(w.x, w.y), hi = __floats2bfloat162_rn(w.z, w.w);
+        *reinterpret_cast<uint2*>(Wq + e) = make_uint2(*reinterpret_cast<const uint32_t*>(&lo),
+                                                        *reinterpret_cast<const uint32_t*>(&hi));
+      }
       colacc.x = fmaf(w.x, w.x, colacc.x); colacc.y = fmaf(w.y, w.y, colacc.y);
       colacc.z = fmaf(w.z, w.z, colacc.z); colacc.w = fmaf(w.w, w.w, colacc.w);
     }
@@ -338,7 +343,7 @@ commit_kernel(float* __restrict__ Wm, __nv_bfloat16* __restrict__ Wb, const floa
 // W2[:, o] *= n0[o] / (||W2[:, o]|| + 1e-5), norms from the per-block partial sums (fixed order).
 // grid (ceil(H/CM_ROWS), nh), block 256.
 __global__ void __launch_bounds__(256)
-renorm_w2_kernel(float* __restrict__ Wm, __nv_bfloat16* __restrict__ Wb,
+renorm_w2_kernel(float* __restrict__ Wm, ttt_wop_t* __restrict__ Wb, __nv_bfloat16* __restrict__ Wq,
                  const float* __restrict__ colsq, const float* __restrict__ n0, int nblk, int nh,
                  int hd, int H) {
   __shared__ float f[128];
@@ -356,7 +361,8 @@ renorm_w2_kernel(float* __restrict__ Wm, __nv_bfloat16* __restrict__ Wb,
     if (j < H) {
       const float w = Wm[base + (size_t)j * hd + i] * f[i];
       Wm[base + (size_t)j * hd + i] = w;
-      Wb[base + (size_t)j * hd + i] = __float2bfloat16_rn(w);
+      Wb[base + (size_t)j * hd + i] = ttt_to_wop(w);
+      if (Wq) Wq[base + (size_t)j * hd + i] = __float2bfloat16_rn(w);
     }
   }
 }
@@ -367,7 +373,7 @@ renorm_w2_kernel(float* __restrict__ Wm, __nv_bfloat16* __restrict__ Wb,
 int launch_init(ttt_ctx* ctx, const float* W1, const float* W2, const float* W3, cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
   dim3 grid((c.hidden + 31) / 32, c.nh, 3), block(32, 8);
-  init_load_kernel<<<grid, block, 0, s>>>(W1, W2, W3, ctx->Wm, ctx->Wb, ctx->n0, ctx->colsq, c.nh,
+  init_load_kernel<<<grid, block, 0, s>>>(W1, W2, W3, ctx->Wm, ctx->Wb, ctx->Wq, ctx->n0, ctx->colsq, c.nh,
                                           c.hd, c.hidden);
   TTT_LAUNCH_CHECK(ctx, "init_load_kernel");
   init_colnorm_kernel<<<c.nh, 128, 0, s>>>(ctx->colsq, ctx->n0, (int)grid.x, c.nh, c.hd, c.hidden);
@@ -406,7 +412,7 @@ int launch_loss_reduce(ttt_ctx* ctx, int n, float* loss, cudaStream_t s) {
 int launch_renorm_w2(ttt_ctx* ctx, int nblk, cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
   const int nrow = (c.hidden + CM_ROWS - 1) / CM_ROWS;
-  renorm_w2_kernel<<<dim3(nrow, c.nh), 256, 0, s>>>(ctx->Wm, ctx->Wb, ctx->colsq, ctx->n0, nblk, c.nh,
+  renorm_w2_kernel<<<dim3(nrow, c.nh), 256, 0, s>>>(ctx->Wm, ctx->Wb, ctx->Wq, ctx->colsq, ctx->n0, nblk, c.nh,
                                                     c.hd, c.hidden);
   TTT_LAUNCH_CHECK(ctx, "renorm_w2_kernel");
   return TTT_OK;
@@ -438,7 +444,7 @@ int launch_commit(ttt_ctx* ctx, cudaStream_t s) {
   const int nblk = (c.hidden + CM_ROWS - 1) / CM_ROWS;
   int tpr = 1;
   while (tpr * 4 < c.hd) tpr <<= 1;
-  commit_kernel<<<dim3(nblk, c.nh, 3), 256, 0, s>>>(ctx->Wm, ctx->Wb, ctx->G, ctx->partials,
+  commit_kernel<<<dim3(nblk, c.nh, 3), 256, 0, s>>>(ctx->Wm, ctx->Wb, ctx->Wq, ctx->G, ctx->partials,
                                                     ctx->n_partials, ctx->G_valid ? 1 : 0, ctx->n0,
                                                     ctx->colsq, c.renorm, c.nh, c.hd, c.hidden,
                                                     tpr);

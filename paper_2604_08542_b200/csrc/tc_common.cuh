@@ -306,17 +306,22 @@ __device__ __forceinline__ uint64_t umma_smem_desc_sw128(uint32_t smem_addr, uin
   return d;
 }
 
-// Instruction descriptor for kind::f16 with bf16 A and B, fp32 accumulation.
+// Instruction descriptor for kind::f16, fp32 accumulation. a_fmt / b_fmt: 0 = fp16, 1 = bf16, chosen
+// independently (a bf16 token tile against an fp16 weight or gradient operand).
 // a_mn_major / b_mn_major: 0 = K-major, 1 = MN-major. A from TMEM must be K-major.
-__host__ __device__ constexpr uint32_t umma_idesc_bf16(int M, int N, int a_mn_major,
-                                                       int b_mn_major) {
+__host__ __device__ constexpr uint32_t umma_idesc(int M, int N, int a_mn_major, int b_mn_major,
+                                                  int a_fmt, int b_fmt) {
   return (1u << 4)                                   // [4,6)   D format: f32
-         | (1u << 7)                                 // [7,10)  A format: bf16
-         | (1u << 10)                                // [10,13) B format: bf16
+         | (static_cast<uint32_t>(a_fmt) << 7)       // [7,10)  A format
+         | (static_cast<uint32_t>(b_fmt) << 10)      // [10,13) B format
          | (static_cast<uint32_t>(a_mn_major) << 15) // [15]    A major
          | (static_cast<uint32_t>(b_mn_major) << 16) // [16]    B major
          | (static_cast<uint32_t>(N >> 3) << 17)     // [17,23) N >> 3
          | (static_cast<uint32_t>(M >> 4) << 24);    // [24,29) M >> 4
+}
+__host__ __device__ constexpr uint32_t umma_idesc_bf16(int M, int N, int a_mn_major,
+                                                       int b_mn_major) {
+  return umma_idesc(M, N, a_mn_major, b_mn_major, 1, 1);
 }
 
 // D[tmem] (+)= A[tmem] . B[smem]   (cta_group::1, kind::f16). One thread issues.
@@ -420,6 +425,13 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   return r;
 }
 
+// two fp32 -> one fp16x2 word, `lo` in bits [0,16) (RN-even, saturating to +-65504)
+__device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+
 // packed fp32x2 arithmetic (FFMA2 / FMUL2 / FADD2): one issue slot for two lanes of math
 __device__ __forceinline__ uint64_t pack2(float lo, float hi) {
   uint64_t r;
@@ -459,6 +471,45 @@ __device__ __forceinline__ uint32_t pack_bf16x2_from2(uint64_t v) {
   float lo, hi;
   unpack2(v, lo, hi);
   return pack_bf16x2(lo, hi);
+}
+
+__device__ __forceinline__ uint32_t pack_f16x2_from2(uint64_t v) {
+  float lo, hi;
+  unpack2(v, lo, hi);
+  return pack_f16x2(lo, hi);
+}
+
+// one bf16x2 word -> fp16x2 (exact in fp16's normal range)
+__device__ __forceinline__ uint32_t bf16x2_to_f16x2(uint32_t w) {
+  return pack_f16x2(__uint_as_float(w << 16), __uint_as_float(w & 0xffff0000u));
+}
+// In-place bf16 -> fp16 conversion of a shared-memory token tile by one warp: 32 * CPL chunks of
+// 16 bytes (element-wise, so the 128-B swizzle is untouched). The caller orders the writes before the
+// MMAs that read the tile: fence.proxy.async, then the arrive on the stage's barrier.
+template <int CPL>
+__device__ __forceinline__ void tile_bf16_to_f16(uint8_t* tile, int lane) {
+  uint4* p = reinterpret_cast<uint4*>(tile) + lane;
+#pragma unroll
+  for (int k0 = 0; k0 < CPL; k0 += 4) {
+    uint4 v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) v[u] = p[32 * (k0 + u)];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      v[u].x = bf16x2_to_f16x2(v[u].x); v[u].y = bf16x2_to_f16x2(v[u].y);
+      v[u].z = bf16x2_to_f16x2(v[u].z); v[u].w = bf16x2_to_f16x2(v[u].w);
+      p[32 * (k0 + u)] = v[u];
+    }
+  }
+}
+// power-of-two scale that brings max|eta| of a CTA's tokens into [1, 2): the fp16 gradient operands
+// carry the factor eta, so without it a small learning rate would push them into fp16's subnormals.
+// Exact (a power of two) and undone at the flush. 1 when the maximum is 0, subnormal, inf or NaN.
+__device__ __forceinline__ void eta_scale(float max_abs, float& scale, float& inv_scale) {
+  const uint32_t e = (__float_as_uint(max_abs) >> 23) & 0xffu;
+  const bool ok = e >= 1u && e <= 253u;
+  scale = ok ? __uint_as_float((254u - e) << 23) : 1.0f;
+  inv_scale = ok ? __uint_as_float(e << 23) : 1.0f;
 }
 
 // L2 cache-policy words for TMA cache hints (createpolicy encodings used by CUTLASS' CacheHintSm90)

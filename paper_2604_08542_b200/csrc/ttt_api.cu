@@ -162,7 +162,8 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
     if (ok && cudaMalloc(p, bytes) != cudaSuccess) ok = false;
   };
   alloc((void**)&ctx->Wm, set * sizeof(float));
-  alloc((void**)&ctx->Wb, set * sizeof(__nv_bfloat16));
+  alloc((void**)&ctx->Wb, set * sizeof(ttt_wop_t));
+  if (is_bf16 && bf16_apply_wide_supported(cfg)) alloc((void**)&ctx->Wq, set * sizeof(__nv_bfloat16));
   alloc((void**)&ctx->n0, ((size_t)2 * cfg->nh * cfg->hidden + (size_t)cfg->nh * cfg->hd) * sizeof(float));
   alloc((void**)&ctx->colsq, (size_t)cfg->nh * nblk * cfg->hd * sizeof(float));
   alloc((void**)&ctx->G, set * sizeof(float));
@@ -206,7 +207,7 @@ void ttt_destroy(ttt_ctx* ctx) {
   if (!ctx) return;
   cudaSetDevice(ctx->cfg.device);
   cudaDeviceSynchronize();
-  cudaFree(ctx->Wm); cudaFree(ctx->Wb); cudaFree(ctx->n0); cudaFree(ctx->colsq);
+  cudaFree(ctx->Wm); cudaFree(ctx->Wb); cudaFree(ctx->Wq); cudaFree(ctx->n0); cudaFree(ctx->colsq);
   cudaFree(ctx->G); cudaFree(ctx->partials); cudaFree(ctx->loss_part); cudaFree(ctx->loss_blk); cudaFree(ctx->sync_ctr); cudaFree(ctx->ns_scratch); cudaFree(ctx->stage[0]); cudaFree(ctx->stage[1]);
   for (int i = 0; i < 3; ++i) cudaFree(ctx->act[i]);
   delete ctx;

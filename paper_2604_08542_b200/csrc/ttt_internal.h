@@ -4,10 +4,33 @@
 
 #include <cuda.h>
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 #include "../../include/ttt.h"
+
+// Operand precision. Everything the library itself rounds to 16 bits
+// for an MMA — the operand copy of the fp32 fast weights and the epilogue's gradient operands — is
+// rounded to IEEE fp16 (11-bit significand, 8x finer than bf16). A kind::f16 MMA needs A and B in the
+// SAME format (fp16 x bf16 raises an illegal-instruction fault on sm_100a — measured), so the bf16
+// token tiles are converted to fp16 on chip before they serve as operands: exact for magnitudes in
+// [2^-14, 65504], absolute error <= 2^-25 below. Saturating conversions: a value beyond +-65504
+// clamps instead of turning into inf.
+typedef __half ttt_wop_t;
+constexpr int TTT_FMT_F16 = 0, TTT_FMT_BF16 = 1;     // instruction-descriptor format codes, kind::f16
+constexpr int TTT_FMT_WOP = TTT_FMT_F16;
+#ifdef __CUDACC__
+__device__ __forceinline__ uint32_t ttt_pack_wop2(float lo, float hi) {   // `lo` in bits [0,16)
+  uint32_t r;
+  asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+__device__ __forceinline__ ttt_wop_t ttt_to_wop(float v) {
+  const uint32_t r = ttt_pack_wop2(v, 0.f);
+  return __ushort_as_half(static_cast<unsigned short>(r & 0xffffu));
+}
+#endif
 
 // Internal weight layout ("hidden-major"): three matrices per head, each [H][hd], hd contiguous:
 //   mat 0 = W1^T   (row j = fan-in vector of hidden unit j of the gate branch, Eq. 12)
@@ -24,7 +47,9 @@ struct ttt_ctx {
 
   size_t mat_elems;      // nh*H*hd
   float* Wm;             // [3][nh][H][hd] fp32 master weights
-  __nv_bfloat16* Wb;     // [3][nh][H][hd] bf16 operand copy (refreshed by init/commit)
+  ttt_wop_t* Wb;         // [3][nh][H][hd] 16-bit operand copy (fp16; refreshed by init/commit)
+  __nv_bfloat16* Wq;     // hd = 128 only: bf16 copy for the apply kernel, whose Q tiles are SS-mode A
+                         // operands straight from the TMA (bf16 x bf16 products); NULL otherwise
   float* n0;             // initial fan-in norms: [nh][H] (mat 0), [nh][hd] (mat 1), [nh][H] (mat 2)
   float* colsq;          // [nh][rowblocks][hd] partial column sums of squares of W2 (renorm)
 
