@@ -15,12 +15,14 @@
  * fan-in re-normalisation) are defined in DESIGN.md, readings R-NS and R-RENORM.
  *
  * Conventions for every function below
- *   - returns TTT_OK (0) or a negative ttt_status; never throws, aborts or prints;
+ *   - returns TTT_OK (0) or a negative ttt_status; never throws, aborts, prints or reads the
+ *     environment;
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream); all work is
  *     enqueued asynchronously on it; calls on one context must be stream-ordered by the caller;
  *   - every data pointer is a DEVICE pointer on cfg.device unless it says "host"; pointers are
- *     BORROWED for the call and must stay valid until the enqueued work has completed;
- *   - the context OWNS the fp32 master weights, their bf16 operand copies, the partial-gradient
+ *     BORROWED for the call and must stay valid until the enqueued work has completed; every call
+ *     makes cfg.device current for its own duration and restores the caller's device;
+ *   - the context OWNS the fp32 master weights, their 16-bit operand copies, the partial-gradient
  *     and Newton-Schulz workspaces and the initial fan-in norms;
  *   - a context is not thread-safe; distinct contexts are independent.
  * Token tensors Q, K, V, O: [M][nh][hd] token-major, heads interleaved in the last dimension
@@ -51,10 +53,13 @@ typedef enum {
 
 typedef enum {
   TTT_F32 = 0,  /* Q,K,V,O fp32; every contraction in fp32 FFMA (parity config 1, tol 1e-4)   */
-  TTT_BF16 = 1  /* Q,K,V,O bf16, fp32 master weights. hd = 64 with hidden 128|256 and hd = 128 with
-                   hidden a multiple of 128: tcgen05 bf16 MMAs with fp32 accumulation; other shapes
-                   (hd % 8 == 0): the fp32 CUDA-core kernels behind a bf16 <-> fp32 conversion
-                   (same semantics)                                                             */
+  TTT_BF16 = 1  /* Q,K,V,O bf16, fp32 master weights, tcgen05 MMAs with fp32 accumulation. Shapes the
+                   tensor kernels take: hd = 64 with hidden 128|256, hd = 128 with hidden a multiple
+                   of 128 (<= 1024 with Newton-Schulz). Any other shape: ttt_create returns
+                   TTT_ERR_UNSUPPORTED, unless cfg.cuda_core_fallback = 1 asks for the fp32 CUDA-core
+                   kernels behind a bf16 <-> fp32 conversion (hd % 8 == 0; same semantics, ~40x slower).
+                   Token values are MMA operands as fp16 (converted on chip, exact for magnitudes in
+                   [2^-14, 65504]; smaller ones keep an absolute error <= 2^-25, larger ones clamp) */
 } ttt_dtype;
 
 typedef struct {
@@ -68,17 +73,27 @@ typedef struct {
                                  (needs hidden == hd; f32 path only)                           */
   int32_t device;             /* CUDA device ordinal                                           */
   int64_t max_tokens;         /* largest M of any later call (workspace sizing)                */
+  int32_t cuda_core_fallback; /* TTT_BF16 only. 0: shapes without a tcgen05 kernel are rejected;
+                                 1: they run on the fp32 CUDA-core kernels (explicit opt-in)      */
+  int32_t reserved;           /* must be 0                                                     */
 } ttt_config;
 
-/* Create a context on cfg->device. `*out` is written only on success. */
+/* Create a context on cfg->device. `*out` is written only on success; on failure
+ * ttt_create_error() describes why (thread-local static text, valid until the thread's next
+ * ttt_create). */
 int ttt_create(ttt_ctx** out, const ttt_config* cfg);
+const char* ttt_create_error(void);
+
+/* Which kernels the context's two call families run on: 1 = tcgen05 tensor-core kernels,
+ * 0 = fp32 CUDA-core kernels (TTT_F32 contexts, or cfg.cuda_core_fallback). Either pointer may be NULL. */
+int ttt_kernel_path(const ttt_ctx* ctx, int* update_on_tensor_cores, int* apply_on_tensor_cores);
 
 /* Free everything the context owns. NULL is allowed. Synchronises the device. */
 void ttt_destroy(ttt_ctx* ctx);
 
 /* Load the initial fast weights (DEVICE, fp32, row-major): W1, W3 [nh][hd][H], W2 [nh][H][hd].
  * Records each unit's initial fan-in 2-norm (columns of W1/W3, length hd; columns of W2,
- * length H) for cfg.renorm, refreshes the bf16 operand copies and resets the chunk counter.
+ * length H) for cfg.renorm, refreshes the 16-bit operand copies and drops any pending gradient.
  * May be called again at any time = reset of the memory (new sequence). */
 int ttt_init(ttt_ctx* ctx, const float* W1, const float* W2, const float* W3, void* stream);
 

@@ -16,12 +16,13 @@ import torch
 
 TTT_F32, TTT_BF16 = 0, 1
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.environ.get("TTT_B200_LIB") or os.path.join(_HERE, "libttt_b200.so")  # debug-build override
+_LIB_PATH = os.path.join(_HERE, "libttt_b200.so")
 _lib = None
 
 EXPORTS = ("ttt_create", "ttt_destroy", "ttt_init", "ttt_update", "ttt_apply", "ttt_chunk_step",
            "ttt_accumulate", "ttt_commit", "ttt_pending_gradient", "ttt_get_weights",
-           "ttt_launch_count", "ttt_strerror", "ttt_last_error", "ttt_version")
+           "ttt_launch_count", "ttt_strerror", "ttt_last_error", "ttt_version", "ttt_create_error",
+           "ttt_kernel_path")
 
 
 class TTTError(RuntimeError):
@@ -34,7 +35,8 @@ class _Config(ctypes.Structure):
     _fields_ = [("nh", ctypes.c_int32), ("hd", ctypes.c_int32), ("hidden", ctypes.c_int32),
                 ("act_dtype", ctypes.c_int32), ("ns_iters", ctypes.c_int32),
                 ("renorm", ctypes.c_int32), ("linear_fast_weight", ctypes.c_int32),
-                ("device", ctypes.c_int32), ("max_tokens", ctypes.c_int64)]
+                ("device", ctypes.c_int32), ("max_tokens", ctypes.c_int64),
+                ("cuda_core_fallback", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
 
 def lib_path() -> str:
@@ -70,6 +72,8 @@ def load_library() -> ctypes.CDLL:
     lib.ttt_last_error.argtypes = [vp]
     lib.ttt_last_error.restype = ctypes.c_char_p
     lib.ttt_version.restype = ctypes.c_char_p
+    lib.ttt_create_error.restype = ctypes.c_char_p
+    lib.ttt_kernel_path.argtypes = [vp, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int)]
     _lib = lib
     return lib
 
@@ -87,17 +91,18 @@ class TTT:
 
     def __init__(self, nh: int, hd: int, hidden: int, act_dtype: int = TTT_BF16, ns_iters: int = 0,
                  renorm: int = 0, linear_fast_weight: int = 0, max_tokens: int = 65536,
-                 device: int = 0):
+                 device: int = 0, cuda_core_fallback: int = 0):
         self._lib = load_library()
         self._ctx = ctypes.c_void_p()
         self.cfg = _Config(nh, hd, hidden, act_dtype, ns_iters, renorm, linear_fast_weight, device,
-                           max_tokens)
+                           max_tokens, cuda_core_fallback, 0)
         self.device = torch.device("cuda", device)
         self.dtype = torch.bfloat16 if act_dtype == TTT_BF16 else torch.float32
         st = self._lib.ttt_create(ctypes.byref(self._ctx), ctypes.byref(self.cfg))
         if st != 0:
             self._ctx = ctypes.c_void_p()
-            raise TTTError(st, "ttt_create", self._lib.ttt_strerror(st).decode())
+            raise TTTError(st, "ttt_create", self._lib.ttt_strerror(st).decode() + "; " +
+                           self._lib.ttt_create_error().decode())
 
     # -- plumbing --------------------------------------------------------------------------
     def _check(self, st: int, what: str):
@@ -111,6 +116,12 @@ class TTT:
     def _tok(self, X: torch.Tensor, name: str) -> Tuple[int, int]:
         assert X.is_cuda and X.dtype == self.dtype and X.dim() == 2 and X.stride(1) == 1, name
         return X.shape[0], X.stride(0) if X.shape[0] > 1 else max(X.stride(0), X.shape[1])
+
+    def kernel_path(self) -> Tuple[bool, bool]:
+        """(update on tensor cores, apply on tensor cores) — include/ttt.h: ttt_kernel_path."""
+        u, a = ctypes.c_int(), ctypes.c_int()
+        self._check(self._lib.ttt_kernel_path(self._ctx, ctypes.byref(u), ctypes.byref(a)), "ttt_kernel_path")
+        return bool(u.value), bool(a.value)
 
     def close(self):
         if getattr(self, "_ctx", None) is not None and self._ctx.value:

@@ -307,7 +307,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
 int bf16_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
                cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
-  if (c.hd == 128) return bf16_apply_wide(ctx, Q, O, M, ld, s);   // streamed weights
+  if (c.hd == 128) return bf16_apply_wide_pair(ctx, Q, O, M, ld, s);   // streamed weights, CTA pairs
   const int tiles = (int)((M + app::TM - 1) / app::TM);
   int per_head = ctx->sm_count / c.nh;
   if (per_head < 1) per_head = 1;
@@ -320,12 +320,11 @@ int bf16_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M
   rc = make_token_map(ctx, &mapO, O, M, (int64_t)c.nh * c.hd, ld, app::TM);
   if (rc != TTT_OK) return rc;
   const size_t smem = (size_t)3 * c.hidden * 128 + (app::QST + 2) * app::TILE_BYTES + 1024;
-  static size_t attr_smem = 0;
-  if (smem > attr_smem) {
+  if (smem > ctx->attr_smem_apply) {
     TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_apply_kernel,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
                  "bf16_apply_kernel smem attr");
-    attr_smem = smem;
+    ctx->attr_smem_apply = smem;
   }
   dim3 grid(per_head, c.nh);
   cudaLaunchConfig_t cfg = {};

@@ -3,7 +3,7 @@
 //
 // Why pairs: with M = 128 the B-operand reads of an N = 128 MMA alone need the full 128 B/clk of the
 // shared-memory port at the nominal tensor rate, and the streamed weights add their TMA writes on
-// top (single-CTA kernel, bf16_apply_wide.cu: ~112 clk per M128 N128 K16 MMA against a floor of 64).
+// top (a single-CTA version of this kernel measured ~112 clk per M128 N128 K16 MMA against a floor of 64).
 // A CTA pair shares every B operand: each CTA streams and reads HALF of a step's weights —
 //   forward   x | b [256 x 128] = Q [256 x 128] . [W1^T rows ; W3^T rows]^T : rank 0 holds the 64 W1^T
 //             rows (N 0-63 = x), rank 1 the 64 W3^T rows (N 64-127 = b) of the 64-hidden step;
@@ -22,7 +22,6 @@
 // Hq (A operand of the down MMAs) overwrites the first 32 columns of its own x once all epilogue
 // warps hold their x | b in registers.
 #include <stdio.h>
-#include <stdlib.h>
 
 #include "tc_common.cuh"
 #include "ttt_internal.h"
@@ -363,8 +362,10 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
 }
 
 // ------------------------------------------------------------------------------------------------
-// Returns 1 (nothing launched) when the device cannot host a CTA pair of this kernel: the caller then
-// runs the single-CTA kernel.
+int bf16_apply_wide_supported(const ttt_config* cfg) {
+  return cfg->hd == appp::HD && cfg->hidden % appp::HSTEP == 0 && !cfg->linear_fast_weight;
+}
+
 int bf16_apply_wide_pair(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
                          cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
@@ -375,12 +376,11 @@ int bf16_apply_wide_pair(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O,
   if (rc != TTT_OK) return rc;
   rc = make_token_map(ctx, &mapQ, Q, M, (int64_t)c.nh * c.hd, ld, appp::TM);
   if (rc != TTT_OK) return rc;
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (!(ctx->attr_done & ATTR_APPW)) {
     TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_apply_wide_pair_kernel,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            (int)appp::SMEM_BYTES), "bf16_apply_wide_pair_kernel smem attr");
-    attr_set = true;
+    ctx->attr_done |= ATTR_APPW;
   }
   cudaLaunchConfig_t cfg = {};
   cfg.blockDim = dim3(appp::THREADS);
@@ -397,19 +397,19 @@ int bf16_apply_wide_pair(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O,
   cfg.numAttrs = 1;
   // persistent CTA pairs, units round-robin: one wave only — a pair that had to wait for a free
   // TPC would start when the others are done (not every SM of the device can host a pair)
-  static int max_pairs = 0;
-  if (max_pairs == 0) {
+  if (ctx->max_pairs == 0) {
     cfg.gridDim = dim3(2 * (ctx->sm_count / 2));
     int n = 0;
     TTT_CUDA_TRY(ctx, cudaOccupancyMaxActiveClusters(&n, bf16_apply_wide_pair_kernel, &cfg),
                  "bf16_apply_wide_pair_kernel occupancy");
-    max_pairs = n > 0 ? n : -1;
-    if (getenv("TTT_DEBUG_PAIRS")) fprintf(stderr, "bf16_apply_wide_pair: %d co-resident CTA pairs\n", n);
+    ctx->max_pairs = n > 0 ? n : -1;
   }
-  if (max_pairs < 0) return 1;
+  if (ctx->max_pairs < 0)
+    return set_error(ctx, TTT_ERR_UNSUPPORTED, "hd = 128 apply: this device cannot host a CTA pair "
+                     "(cta_group::2) of bf16_apply_wide_pair_kernel", cudaSuccess);
   cfg.numAttrs = 2;
   int ncl = c.nh * npairs;
-  if (ncl > max_pairs) ncl = max_pairs;
+  if (ncl > ctx->max_pairs) ncl = ctx->max_pairs;
   cfg.gridDim = dim3(2 * ncl);
   int Mi = (int)M, nh = c.nh, H = c.hidden, q_early = ctx->apply_q_early;
   cudaError_t e = cudaLaunchKernelEx(&cfg, bf16_apply_wide_pair_kernel, mapW, mapQ, O, Mi, ld, nh, H, npairs, q_early);

@@ -80,6 +80,9 @@ constexpr int HS = 128;        // hidden units per CTA (MMA M)
 constexpr int T = 32;          // tokens per tile (forward MMA N, gradient MMA K)
 constexpr int STAGES = 10;     // K/V shared-memory ring (ring latency = TMA + F -> E -> G hand-offs)
 constexpr int EPI_WARPS = 16;
+constexpr int CVT_WARPS = 2;   // stage finishers: warps 0 and 2
+// 20 warps: 5 per scheduler keep 96 registers per thread (a 21st warp caps everybody at 80 and the
+// epilogue spills)
 constexpr int THREADS = (4 + EPI_WARPS) * 32;
 constexpr int TILE_BYTES = T * 128;  // one [T x 64] bf16 tile
 constexpr int STAGE_BYTES = 2 * TILE_BYTES;
@@ -112,6 +115,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   __shared__ uint32_t tmem_base_s;
   __shared__ float loss_red[EPI_WARPS];
   __shared__ float lrmax_s[THREADS / 32];
+  static_assert(THREADS % 16 == 0, "the fused commit gives 16 lanes one weight row");
   __shared__ __align__(16) float ne_s[STAGES][T];   // -eta of the stage's tokens, scaled (0 beyond M)
 #ifdef TTT_TRACE
   __shared__ unsigned tr_s[64 * 16];
@@ -160,7 +164,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     TTT_TR(2, 14);
   } else if (tid == 32) {
 #pragma unroll
-    for (int s = 0; s < STAGES; ++s) { mbar_init(&empty[s], 1); mbar_init(&full[s], 1); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&empty[s], 1); mbar_init(&full[s], CVT_WARPS); }
     mbar_init(&fwd_full[0], 1);
     mbar_init(&fwd_full[1], 1);
     mbar_init(&g_free, EPI_WARPS / 2);
@@ -228,17 +232,15 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   }
 
   if (warp == 0) {
-    // ===================== TMA producer =====================
-    if (elect_one()) {
-      for (int i = STAGES; i < ntiles; ++i) {        // tiles 0 .. STAGES-1 were requested in the prologue
-        const int s = i % STAGES, it = i / STAGES;
-        mbar_wait(&empty[s], (it & 1) ^ 1);
-        TTT_TR(i, 12);
-        mbar_arrive_expect_tx(&tma_full[s], STAGE_BYTES);
-        uint8_t* dst = smem + s * STAGE_BYTES;
-        tma_load_2d(dst, &mapK, &tma_full[s], h * HD, (tile_lo + i) * T);
-        tma_load_2d(dst + TILE_BYTES, &mapV, &tma_full[s], h * HD, (tile_lo + i) * T);
-      }
+    // ===================== stage finisher 1: fp16 conversion (second half of a stage) =====================
+    // (tiles 0 .. STAGES-1 were requested by thread 0 in the prologue; the gradient issuer refills the ring)
+    for (int i = 0; i < ntiles; ++i) {
+      const int s = i % STAGES;
+      mbar_wait(&tma_full[s], (i / STAGES) & 1);
+      tile_bf16_to_f16<STAGE_BYTES / 512 / CVT_WARPS>(smem + s * STAGE_BYTES + STAGE_BYTES / CVT_WARPS, lane);
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&full[s]);
     }
   } else if (warp == 1) {
     // ===================== forward-MMA issuer =====================
@@ -308,16 +310,31 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         tc_commit(&empty[s]);          // the tile's forward MMAs completed long ago (epilogue read them)
         tc_commit(&opnd_free[b]);     // one barrier per tile parity (see the epilogue's wait)
         TTT_TR(i, 4);
+        // TMA producer duty (this thread has the slack; warp 0 is a stage finisher): the stage of tile
+        // i - 1, whose gradient MMAs were issued an iteration ago and are normally complete by now, is
+        // refilled with tile i - 1 + STAGES
+        if (i >= 1 && i - 1 + STAGES < ntiles) {
+          const int j = i - 1 + STAGES, sj = (i - 1) % STAGES;
+          mbar_wait(&empty[sj], ((i - 1) / STAGES) & 1);
+          TTT_TR(j, 12);
+          mbar_arrive_expect_tx(&tma_full[sj], STAGE_BYTES);
+          uint8_t* dst = smem + sj * STAGE_BYTES;
+          tma_load_2d(dst, &mapK, &tma_full[sj], h * HD, (tile_lo + j) * T);
+          tma_load_2d(dst + TILE_BYTES, &mapV, &tma_full[sj], h * HD, (tile_lo + j) * T);
+        }
         if (++s == STAGES) { s = 0; dk = d0; } else { dk += ST_OFF; }
       }
       tc_commit(&grad_done);
     }
   } else if (warp == 2) {
-    // ===================== stage finisher: fp16 conversion + learning rates =====================
-    // When the TMA has landed a stage, this warp converts its K and V tiles from bf16 to fp16 in place
-    // (all MMA operands are fp16, ttt_internal.h) and puts -eta of the tile's 32 tokens (one 128-B line
-    // of lr, scaled by the CTA's power of two) into the stage's slot; then the stage is `full`. The
-    // global loads of lr run LRPF tiles ahead of the ring (register double buffer).
+    // ===================== stage finisher 0: fp16 conversion + learning rates =====================
+    // When the TMA has landed a stage, the two finisher warps (this one: the K tile, warp 0: the V tile)
+    // convert it from bf16 to fp16 in place (all MMA operands are fp16, ttt_internal.h; one warp alone
+    // needs 550-750 clk per stage next to the epilogue warps of its scheduler and becomes the kernel's
+    // critical path), and this one also puts
+    // -eta of the tile's 32 tokens (one 128-B line of lr, scaled by the CTA's power of two) into the
+    // stage's slot; the stage is `full` when all of them have arrived. The global loads of lr run LRPF
+    // tiles ahead of the ring (register double buffer).
     const float* lrh = lr + (size_t)h * M;
     auto ld_batch = [&](int i0, float (&v)[LRPF]) {
 #pragma unroll
@@ -337,11 +354,14 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         if (i < ntiles) {
           const int s = i % STAGES, it = i / STAGES;
           mbar_wait(&tma_full[s], it & 1);       // (the TMA was issued after the stage's `empty`)
-          tile_bf16_to_f16<STAGE_BYTES / 512>(smem + s * STAGE_BYTES, lane);
+          if (lane == 0 && i >= 16) TTT_TR(i, 13);
+          tile_bf16_to_f16<STAGE_BYTES / 512 / CVT_WARPS>(smem + s * STAGE_BYTES, lane);
           ne_s[s][lane] = cur[u];
+          if (lane == 0 && i >= 16) TTT_TR(i, 14);
           fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) mbar_arrive(&full[s]);
+          if (lane == 0 && i >= 16) TTT_TR(i, 15);
 
         }
       }
@@ -591,13 +611,16 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       for (int k = 0; k < CE; ++k) {
         if (ok[k]) { w[k].x -= g[k].x; w[k].y -= g[k].y; w[k].z -= g[k].z; w[k].w -= g[k].w; }
         if (renorm_n0 != nullptr) {
-          if (mat[k] != 1) {    // W1^T / W3^T: a row is a unit's fan-in vector -> back to its initial norm
-            float sq = w[k].x * w[k].x + w[k].y * w[k].y + w[k].z * w[k].z + w[k].w * w[k].w;
+          // row sums of squares: every lane of the warp takes part in the shuffles (lanes beyond e_hi
+          // carry w = 0) — a warp may straddle a matrix boundary or the end of the CTA's range, while
+          // the 16 lanes of one row always share `ok` and `mat`
+          float sq = w[k].x * w[k].x + w[k].y * w[k].y + w[k].z * w[k].z + w[k].w * w[k].w;
 #pragma unroll
-            for (int o = RQ / 2; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+          for (int o = RQ / 2; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+          if (ok[k] && mat[k] != 1) {   // W1^T / W3^T: a row is a unit's fan-in vector -> back to its initial norm
             const int j = slice * HS + r4[k] / RQ;
             const float* n0m = renorm_n0 + (mat[k] == 0 ? (size_t)h * H : (size_t)nh * H + (size_t)nh * HD + (size_t)h * H);
-            const float f = ok[k] ? n0m[j] / (sqrtf(sq) + 1e-5f) : 0.f;
+            const float f = n0m[j] / (sqrtf(sq) + 1e-5f);
             w[k].x *= f; w[k].y *= f; w[k].z *= f; w[k].w *= f;
           } else if (ok[k]) {   // W2: fan-in = column; finished by renorm_w2_kernel from per-CTA partials
             colacc.x = fmaf(w[k].x, w[k].x, colacc.x); colacc.y = fmaf(w[k].y, w[k].y, colacc.y);
@@ -723,38 +746,50 @@ int bf16_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V
   rc = make_token_map(ctx, &mapV, V, M, (int64_t)c.nh * c.hd, ld, upd::T);
   if (rc != TTT_OK) return rc;
   const size_t smem = (size_t)upd::STAGES * upd::STAGE_BYTES + 1024;
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (!(ctx->attr_done & ATTR_UPD)) {
     TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_update_kernel<false>,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
                  "bf16_update_kernel smem attr");
     TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_update_kernel<true>,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
                  "bf16_update_kernel smem attr");
-    attr_set = true;
+    int per_sm = 0;            // CTAs the device can really hold at once (MPS / green contexts shrink it)
+    TTT_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bf16_update_kernel<false>,
+                                                                    upd::THREADS, smem),
+                 "bf16_update_kernel occupancy");
+    ctx->upd_coop_ctas = per_sm * ctx->sm_count;
+    ctx->attr_done |= ATTR_UPD;
   }
   const int nslices = c.hidden / upd::HS;
   float* P = ctx->partials + (size_t)ctx->n_partials * 3 * ctx->mat_elems;
   dim3 grid(splits, nslices, c.nh);
   // fused commit: the CTAs of a (head, slice) group wait on one another, so they must all be
-  // resident -> cooperative launch (fails instead of deadlocking if the device cannot hold them)
-  fuse_commit = fuse_commit && (int)(grid.x * grid.y * grid.z) <= ctx->sm_count;
+  // resident -> cooperative launch, only when the device can hold the whole grid; if that launch is
+  // refused all the same, the plain launch + commit kernel path below is taken (same results)
+  fuse_commit = fuse_commit && (int)(grid.x * grid.y * grid.z) <= ctx->upd_coop_ctas;
   const ttt_wop_t* Wb = ctx->Wb;
   float* loss_part = ctx->loss_part;
   int Mi = (int)M, nh = c.nh, H = c.hidden;
-  float* Wm = fuse_commit ? ctx->Wm : nullptr;
-  ttt_wop_t* Wbw = fuse_commit ? ctx->Wb : nullptr;
   unsigned* ctr = ctx->sync_ctr;
-  if (fuse_commit) ctx->sync_target += (unsigned)splits;
-  unsigned target = ctx->sync_target;
-  const float* rn0 = (fuse_commit && c.renorm) ? ctx->n0 : nullptr;
   float* rcs = ctx->colsq;
-  void* args[] = {&mapK, &mapV, &Wb, &lr, &P, &loss_part, &Mi, &nh, &H, &tiles, &tps, &Wm, &Wbw, &ctr, &target,
-                  &rn0, &rcs};
   const void* fn = want_loss ? (const void*)bf16_update_kernel<true> : (const void*)bf16_update_kernel<false>;
-  cudaError_t e = fuse_commit ? cudaLaunchCooperativeKernel(fn, grid, dim3(upd::THREADS), args, smem, s)
-                              : cudaLaunchKernel(fn, grid, dim3(upd::THREADS), args, smem, s);
-  if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, "bf16_update_kernel launch", e);
+  for (;;) {
+    float* Wm = fuse_commit ? ctx->Wm : nullptr;
+    ttt_wop_t* Wbw = fuse_commit ? ctx->Wb : nullptr;
+    unsigned target = ctx->sync_target + (fuse_commit ? (unsigned)splits : 0u);
+    const float* rn0 = (fuse_commit && c.renorm) ? ctx->n0 : nullptr;
+    void* args[] = {&mapK, &mapV, &Wb, &lr, &P, &loss_part, &Mi, &nh, &H, &tiles, &tps, &Wm, &Wbw, &ctr,
+                    &target, &rn0, &rcs};
+    cudaError_t e = fuse_commit ? cudaLaunchCooperativeKernel(fn, grid, dim3(upd::THREADS), args, smem, s)
+                                : cudaLaunchKernel(fn, grid, dim3(upd::THREADS), args, smem, s);
+    if (e == cudaSuccess) {
+      ctx->sync_target = target;         // only a launch that happened moves the counters' target
+      break;
+    }
+    if (!fuse_commit) return set_error(ctx, TTT_ERR_CUDA, "bf16_update_kernel launch", e);
+    cudaGetLastError();                  // cooperative launch refused: clear it, take the plain path
+    fuse_commit = false;
+  }
   TTT_LAUNCH_CHECK(ctx, "bf16_update_kernel");
   *used = fuse_commit ? 0 : splits;
   *loss_rows = splits * nslices;

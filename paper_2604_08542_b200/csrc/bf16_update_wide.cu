@@ -44,7 +44,8 @@ constexpr int HD = 128;        // head dimension (forward MMA K, gradient MMA N)
 constexpr int T = 32;          // tokens per tile (forward MMA N, gradient MMA K)
 constexpr int STAGES = 5;      // K/V shared-memory ring
 constexpr int EPI_WARPS = 8;
-constexpr int THREADS = (4 + EPI_WARPS) * 32;
+constexpr int CVT_WARPS = 4;   // stage finishers: warps 2, 3 and the two warps after the epilogue warps
+constexpr int THREADS = (4 + EPI_WARPS + CVT_WARPS - 2) * 32;
 constexpr int SUB_BYTES = T * 128;          // one [T x 64] bf16 sub-tile (half of hd), 128-B swizzled
 constexpr int TILE_BYTES = 2 * SUB_BYTES;   // K or V tile
 constexpr int STAGE_BYTES = 2 * TILE_BYTES;
@@ -120,7 +121,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
   };
 
   if (tid == 0) {
-    for (int s = 0; s < STAGES; ++s) { mbar_init(&tma_full[s], 1); mbar_init(&full[s], 2); mbar_init(&empty[s], 1); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&tma_full[s], 1); mbar_init(&full[s], CVT_WARPS); mbar_init(&empty[s], 1); }
     mbar_init(&w_full, 1);
     mbar_init(&fwd_full, 1);
     mbar_init(&xbg_free, 1);
@@ -261,11 +262,12 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
 #endif
     }
   } else if (warp == 2) {
-    // ===================== stage finisher 1: K tile -> fp16, learning rates =====================
-    // When the TMA has landed a stage, this warp converts its K tile from bf16 to fp16 in place (all MMA
-    // operands are fp16, ttt_internal.h; warp 3 does the V tile) and puts -eta of the tile's 32 tokens
-    // (one 128-B line of lr, scaled by the CTA's power of two) into the stage's slot; the global loads
-    // of lr run LRPF tiles ahead of the ring (register double buffer)
+    // ===================== stage finisher 0: fp16 conversion, learning rates =====================
+    // When the TMA has landed a stage, the CVT_WARPS finisher warps convert its K and V tiles from bf16
+    // to fp16 in place, a quarter of the 16 KB each (all MMA operands are fp16, ttt_internal.h), and this
+    // one also puts -eta of the tile's 32 tokens (one 128-B line of lr, scaled by the CTA's power of
+    // two) into the stage's slot; the global loads of lr run LRPF tiles ahead of the ring (register
+    // double buffer)
     constexpr int LRPF = 4;
     auto ld_batch = [&](int g0, float (&v)[LRPF]) {
 #pragma unroll
@@ -290,7 +292,7 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
         if (gi < total) {
           const int s = gi % STAGES, it = gi / STAGES;
           mbar_wait(&tma_full[s], it & 1);       // (the TMA was issued after the stage's `empty`)
-          tile_bf16_to_f16<TILE_BYTES / 512>(ring + s * STAGE_BYTES, lane);
+          tile_bf16_to_f16<STAGE_BYTES / 512 / CVT_WARPS>(ring + s * STAGE_BYTES, lane);
           ne_s[s][lane] = cur[u];
           fence_proxy_async_smem();
           __syncwarp();
@@ -300,12 +302,13 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
 #pragma unroll
       for (int u = 0; u < LRPF; ++u) cur[u] = nxt[u];
     }
-  } else if (warp == 3) {
-    // ===================== stage finisher 2: V tile -> fp16 =====================
+  } else if (warp == 3 || warp >= 4 + EPI_WARPS) {
+    // ===================== stage finishers 1 .. CVT_WARPS-1: fp16 conversion =====================
+    const int part = warp == 3 ? 1 : warp - (4 + EPI_WARPS) + 2;
     for (int gi = 0; gi < total; ++gi) {
       const int s = gi % STAGES;
       mbar_wait(&tma_full[s], (gi / STAGES) & 1);
-      tile_bf16_to_f16<TILE_BYTES / 512>(ring + s * STAGE_BYTES + TILE_BYTES, lane);
+      tile_bf16_to_f16<STAGE_BYTES / 512 / CVT_WARPS>(ring + s * STAGE_BYTES + part * (STAGE_BYTES / CVT_WARPS), lane);
       fence_proxy_async_smem();
       __syncwarp();
       if (lane == 0) mbar_arrive(&full[s]);
@@ -503,15 +506,14 @@ int bf16_accumulate_wide(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat
   // bf16 operand copy of the weights as one [3 nh H][hd] matrix, boxes of [128 rows][64]
   rc = make_token_map(ctx, &mapW, ctx->Wb, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, updw::HS);
   if (rc != TTT_OK) return rc;
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (!(ctx->attr_done & ATTR_UPDW)) {
     TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_update_wide_kernel<false>,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            (int)updw::SMEM_BYTES), "bf16_update_wide_kernel smem attr");
     TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(bf16_update_wide_kernel<true>,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            (int)updw::SMEM_BYTES), "bf16_update_wide_kernel smem attr");
-    attr_set = true;
+    ctx->attr_done |= ATTR_UPDW;
   }
   float* P = ctx->partials + (size_t)ctx->n_partials * 3 * ctx->mat_elems;
   if (want_loss)

@@ -382,11 +382,10 @@ int launch_ns_tc(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s) {
   const size_t stage = (size_t)c.hidden * nstc::W_LD * sizeof(float);
   if (stage > smem) smem = stage;
   smem += 1024;
-  static size_t attr_smem = 0;
-  if (smem > attr_smem) {
+  if (smem > ctx->attr_smem_ns) {
     TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ns_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            (int)smem), "ns_tc_kernel smem attr");
-    attr_smem = smem;
+    ctx->attr_smem_ns = smem;
   }
   const uint32_t alloc = c.hidden <= 256 ? 256 : 512;
   cudaLaunchConfig_t cfg = {};

@@ -382,11 +382,10 @@ int ns_tc_wide_supported(const ttt_config* cfg) {
 
 int launch_ns_tc_wide(ttt_ctx* ctx, bool fuse_commit, cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (!(ctx->attr_done & ATTR_NSW)) {
     TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ns_tc_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            (int)nsw::SMEM_BYTES), "ns_tc_wide_kernel smem attr");
-    attr_set = true;
+    ctx->attr_done |= ATTR_NSW;
   }
   const int nc = c.hidden / nsw::RB;                       // cluster size: one CTA per 128-row block
   cudaLaunchConfig_t cfg = {};

@@ -429,12 +429,11 @@ int launch_commit(ttt_ctx* ctx, cudaStream_t s) {
     if (rc != TTT_OK) return rc;
     const size_t smem = ((size_t)2 * c.hd * (c.hd + 1) + (size_t)NS_ROWS * (c.hd + 1) +
                          NS_THREADS / 32) * sizeof(float);
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!(ctx->attr_done & ATTR_NS_F32)) {
       TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(newton_schulz_kernel,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              200 * 1024), "newton_schulz smem attr");
-      attr_set = true;
+      ctx->attr_done |= ATTR_NS_F32;
     }
     // linear test mode: only mat 0 carries a gradient (mats 1, 2 are identically zero)
     const int n_mats = c.linear_fast_weight ? c.nh : 3 * c.nh;

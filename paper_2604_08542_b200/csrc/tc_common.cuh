@@ -488,14 +488,18 @@ __device__ __forceinline__ uint32_t bf16x2_to_f16x2(uint32_t w) {
 // MMAs that read the tile: fence.proxy.async, then the arrive on the stage's barrier.
 template <int CPL>
 __device__ __forceinline__ void tile_bf16_to_f16(uint8_t* tile, int lane) {
+  constexpr int B = CPL < 8 ? CPL : 8;        // loads in flight per lane
+#ifdef TTT_EXP_NOCVT       // timing experiment only
+  return;
+#endif
   uint4* p = reinterpret_cast<uint4*>(tile) + lane;
 #pragma unroll
-  for (int k0 = 0; k0 < CPL; k0 += 4) {
-    uint4 v[4];
+  for (int k0 = 0; k0 < CPL; k0 += B) {
+    uint4 v[B];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) v[u] = p[32 * (k0 + u)];
+    for (int u = 0; u < B; ++u) v[u] = p[32 * (k0 + u)];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
+    for (int u = 0; u < B; ++u) {
       v[u].x = bf16x2_to_f16x2(v[u].x); v[u].y = bf16x2_to_f16x2(v[u].y);
       v[u].z = bf16x2_to_f16x2(v[u].z); v[u].w = bf16x2_to_f16x2(v[u].w);
       p[32 * (k0 + u)] = v[u];

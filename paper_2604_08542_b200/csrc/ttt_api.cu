@@ -12,6 +12,25 @@ using namespace ttt;
 
 namespace {
 
+thread_local char g_create_err[256] = "";
+
+int create_fail(int status, const char* fmt, long long a = 0, long long b = 0) {
+  snprintf(g_create_err, sizeof(g_create_err), fmt, a, b);
+  return status;
+}
+
+// makes the context's device current for the duration of an entry point
+struct DeviceGuard {
+  int prev = -1, want;
+  explicit DeviceGuard(const ttt_ctx* ctx) : want(ctx->cfg.device) {
+    if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+    if (prev != want) cudaSetDevice(want);
+  }
+  ~DeviceGuard() {
+    if (prev >= 0 && prev != want) cudaSetDevice(prev);
+  }
+};
+
 int fail(ttt_ctx* ctx, int status, const char* fmt, long long a = 0, long long b = 0) {
   if (ctx) snprintf(ctx->err, sizeof(ctx->err), fmt, a, b);
   return status;
@@ -117,29 +136,48 @@ int check_apply_args(ttt_ctx* ctx, const void* Q, const void* O, int64_t M, int6
 extern "C" {
 
 int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
-  if (!out || !cfg) return TTT_ERR_ARG;
+  g_create_err[0] = 0;
+  if (!out || !cfg) return create_fail(TTT_ERR_ARG, "out and cfg must not be NULL");
   if (cfg->nh < 1 || cfg->hd < 1 || cfg->hidden < 1 || cfg->max_tokens < 1 || cfg->ns_iters < 0 ||
       (cfg->renorm != 0 && cfg->renorm != 1) ||
       (cfg->linear_fast_weight != 0 && cfg->linear_fast_weight != 1) ||
+      (cfg->cuda_core_fallback != 0 && cfg->cuda_core_fallback != 1) || cfg->reserved != 0 ||
       (cfg->act_dtype != TTT_F32 && cfg->act_dtype != TTT_BF16))
-    return TTT_ERR_ARG;
-  if (cfg->hd % 4 != 0 || cfg->hidden % 4 != 0 || cfg->hd > 128) return TTT_ERR_SHAPE;
-  if (cfg->linear_fast_weight && cfg->hidden != cfg->hd) return TTT_ERR_SHAPE;
-  if (cfg->ns_iters > 0 && cfg->hidden < cfg->hd) return TTT_ERR_UNSUPPORTED;
+    return create_fail(TTT_ERR_ARG, "a ttt_config field is out of range");
+  if (cfg->hd % 4 != 0 || cfg->hidden % 4 != 0 || cfg->hd > 128)
+    return create_fail(TTT_ERR_SHAPE, "hd = %lld, hidden = %lld: both must be multiples of 4 and hd <= 128",
+                       cfg->hd, cfg->hidden);
+  if (cfg->linear_fast_weight && cfg->hidden != cfg->hd)
+    return create_fail(TTT_ERR_SHAPE, "linear test mode needs hidden == hd");
+  if (cfg->ns_iters > 0 && cfg->hidden < cfg->hd)
+    return create_fail(TTT_ERR_UNSUPPORTED, "Newton-Schulz needs hidden >= hd");
   if (cfg->act_dtype == TTT_BF16) {
-    char why[256];
-    if (!bf16_supported(cfg, why, sizeof(why))) return TTT_ERR_UNSUPPORTED;
+    char why[200];
+    if (!bf16_supported(cfg, why, sizeof(why))) return create_fail(TTT_ERR_UNSUPPORTED, why);
+    if (!cfg->cuda_core_fallback && !(bf16_update_tensor_path(cfg) && bf16_apply_tensor_path(cfg)))
+      return create_fail(TTT_ERR_UNSUPPORTED,
+                         "bf16: no tcgen05 kernel for hd = %lld, hidden = %lld (tensor kernels: hd 64 with "
+                         "hidden 128|256, hd 128 with hidden %% 128 == 0); cfg.cuda_core_fallback = 1 "
+                         "selects the fp32 CUDA-core kernels", cfg->hd, cfg->hidden);
+    if (!cfg->cuda_core_fallback && cfg->ns_iters > 0 && !ns_tc_supported(cfg))
+      return create_fail(TTT_ERR_UNSUPPORTED, "bf16: no tensor-core Newton-Schulz kernel for hidden = %lld",
+                         cfg->hidden);
   }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev)
-    return TTT_ERR_CUDA;
-  if (cudaSetDevice(cfg->device) != cudaSuccess) return TTT_ERR_CUDA;
+    return create_fail(TTT_ERR_CUDA, "device %lld does not exist", cfg->device);
+  int prev_dev = -1;
+  cudaGetDevice(&prev_dev);
+  struct Restore { int d; ~Restore() { if (d >= 0) cudaSetDevice(d); } } restore{prev_dev};
+  if (cudaSetDevice(cfg->device) != cudaSuccess) return create_fail(TTT_ERR_CUDA, "cudaSetDevice failed");
   cudaDeviceProp prop;
-  if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) return TTT_ERR_CUDA;
-  if (prop.major != 10) return TTT_ERR_UNSUPPORTED;  // sm_100a only; no fallback
+  if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess)
+    return create_fail(TTT_ERR_CUDA, "cudaGetDeviceProperties failed");
+  if (prop.major != 10)   // sm_100a only; no fallback
+    return create_fail(TTT_ERR_UNSUPPORTED, "device has compute capability %lld.x, sm_100a is required", prop.major);
 
   ttt_ctx* ctx = new (std::nothrow) ttt_ctx();
-  if (!ctx) return TTT_ERR_NOMEM;
+  if (!ctx) return create_fail(TTT_ERR_NOMEM, "out of host memory");
   memset(ctx, 0, sizeof(*ctx));
   ctx->cfg = *cfg;
   ctx->sm_count = prop.multiProcessorCount;
@@ -197,15 +235,25 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
   if (!ok) {
     cudaGetLastError();
     ttt_destroy(ctx);
-    return TTT_ERR_NOMEM;
+    return create_fail(TTT_ERR_NOMEM, "device memory allocation failed");
   }
   *out = ctx;
   return TTT_OK;
 }
 
+const char* ttt_create_error(void) { return g_create_err; }
+
+int ttt_kernel_path(const ttt_ctx* ctx, int* update_tc, int* apply_tc) {
+  if (!ctx) return TTT_ERR_ARG;
+  const bool bf16 = ctx->cfg.act_dtype == TTT_BF16;
+  if (update_tc) *update_tc = bf16 && !ctx->upd_via_f32;
+  if (apply_tc) *apply_tc = bf16 && !ctx->app_via_f32;
+  return TTT_OK;
+}
+
 void ttt_destroy(ttt_ctx* ctx) {
   if (!ctx) return;
-  cudaSetDevice(ctx->cfg.device);
+  DeviceGuard dg(ctx);
   cudaDeviceSynchronize();
   cudaFree(ctx->Wm); cudaFree(ctx->Wb); cudaFree(ctx->Wq); cudaFree(ctx->n0); cudaFree(ctx->colsq);
   cudaFree(ctx->G); cudaFree(ctx->partials); cudaFree(ctx->loss_part); cudaFree(ctx->loss_blk); cudaFree(ctx->sync_ctr); cudaFree(ctx->ns_scratch); cudaFree(ctx->stage[0]); cudaFree(ctx->stage[1]);
@@ -216,6 +264,7 @@ void ttt_destroy(ttt_ctx* ctx) {
 int ttt_init(ttt_ctx* ctx, const float* W1, const float* W2, const float* W3, void* stream) {
   if (!ctx) return TTT_ERR_ARG;
   if (!W1 || !W2 || !W3) return fail(ctx, TTT_ERR_ARG, "W1, W2 and W3 must not be NULL");
+  DeviceGuard dg(ctx);
   int rc = launch_init(ctx, W1, W2, W3, static_cast<cudaStream_t>(stream));
   if (rc != TTT_OK) return rc;
   ctx->initialised = true;
@@ -229,6 +278,7 @@ int ttt_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, 
   if (!ctx) return TTT_ERR_ARG;
   int rc = check_update_args(ctx, K, V, lr, M, ld);
   if (rc != TTT_OK || M == 0) return rc;
+  DeviceGuard dg(ctx);
   rc = do_accumulate(ctx, K, V, lr, M, ld, loss, static_cast<cudaStream_t>(stream));
   return rc < 0 ? rc : TTT_OK;
 }
@@ -237,6 +287,7 @@ int ttt_commit(ttt_ctx* ctx, void* stream) {
   if (!ctx) return TTT_ERR_ARG;
   if (!ctx->initialised) return fail(ctx, TTT_ERR_STATE, "ttt_init has not been called");
   if (ctx->n_partials == 0 && !ctx->G_valid) return TTT_OK;  // nothing pending
+  DeviceGuard dg(ctx);
   return launch_commit(ctx, static_cast<cudaStream_t>(stream));
 }
 
@@ -245,6 +296,7 @@ int ttt_pending_gradient(ttt_ctx* ctx, float** G, int64_t* n_elements, void* str
   if (!ctx->initialised) return fail(ctx, TTT_ERR_STATE, "ttt_init has not been called");
   if (ctx->n_partials == 0 && !ctx->G_valid)
     return fail(ctx, TTT_ERR_STATE, "no pending gradient (call ttt_accumulate first)");
+  DeviceGuard dg(ctx);
   int rc = launch_reduce_pending(ctx, static_cast<cudaStream_t>(stream));
   if (rc != TTT_OK) return rc;
   *G = ctx->G;
@@ -257,6 +309,7 @@ int ttt_update(ttt_ctx* ctx, const void* K, const void* V, const float* lr, int6
   if (!ctx) return TTT_ERR_ARG;
   int rc = check_update_args(ctx, K, V, lr, M, ld);
   if (rc != TTT_OK || M == 0) return rc;
+  DeviceGuard dg(ctx);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   rc = do_accumulate(ctx, K, V, lr, M, ld, loss, s, true);
   if (rc < 0) return rc;
@@ -267,6 +320,7 @@ int ttt_apply(ttt_ctx* ctx, const void* Q, void* O, int64_t M, int64_t ld, void*
   if (!ctx) return TTT_ERR_ARG;
   int rc = check_apply_args(ctx, Q, O, M, ld);
   if (rc != TTT_OK || M == 0) return rc;
+  DeviceGuard dg(ctx);
   return do_apply(ctx, Q, O, M, ld, static_cast<cudaStream_t>(stream));
 }
 
@@ -277,6 +331,7 @@ int ttt_chunk_step(ttt_ctx* ctx, const void* Q, const void* K, const void* V, co
   if (rc != TTT_OK) return rc;
   rc = check_apply_args(ctx, Q, O, M, ld);
   if (rc != TTT_OK || M == 0) return rc;
+  DeviceGuard dg(ctx);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   rc = do_accumulate(ctx, K, V, lr, M, ld, loss, s, true);
   if (rc < 0) return rc;
@@ -296,6 +351,7 @@ int ttt_get_weights(ttt_ctx* ctx, float* W1, float* W2, float* W3, void* stream)
   if (!ctx) return TTT_ERR_ARG;
   if (!ctx->initialised) return fail(ctx, TTT_ERR_STATE, "ttt_init has not been called");
   if (!W1 || !W2 || !W3) return fail(ctx, TTT_ERR_ARG, "W1, W2 and W3 must not be NULL");
+  DeviceGuard dg(ctx);
   return launch_get_weights(ctx, W1, W2, W3, static_cast<cudaStream_t>(stream));
 }
 
@@ -317,6 +373,6 @@ const char* ttt_strerror(int status) {
 
 const char* ttt_last_error(const ttt_ctx* ctx) { return ctx ? ctx->err : ""; }
 
-const char* ttt_version(void) { return "ttt-b200 0.1 (sm_100a)"; }
+const char* ttt_version(void) { return "ttt-b200 0.2 (sm_100a)"; }
 
 }  // extern "C"

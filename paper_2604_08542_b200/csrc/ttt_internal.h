@@ -80,7 +80,14 @@ struct ttt_ctx {
 
   // bf16 path: driver entry point for cuTensorMapEncodeTiled
   void* encode_tiled;
+
+  // per-context launch state (function attributes are per device; nothing process-global)
+  uint32_t attr_done;          // bit k: the opt-in shared-memory size of kernel k has been set (ATTR_*)
+  size_t attr_smem_apply, attr_smem_ns;   // high-water marks of the kernels with a shape-dependent size
+  int max_pairs;               // hd = 128 apply: co-resident CTA pairs (0 = not queried yet, < 0 = none)
+  int upd_coop_ctas;           // hd = 64 update: co-resident CTAs of the cooperative launch (0 = not queried)
 };
+enum { ATTR_UPD = 1, ATTR_UPD_LOSS = 2, ATTR_UPDW = 4, ATTR_APPW = 8, ATTR_NSW = 16, ATTR_NS_F32 = 32 };
 
 namespace ttt {
 
@@ -127,13 +134,10 @@ int bf16_supported(const ttt_config* cfg, char* why, size_t why_len);
 // 1 if a tcgen05 kernel covers the shape, 0 if bf16 I/O must go through the fp32 CUDA-core path
 int bf16_update_tensor_path(const ttt_config* cfg);
 int bf16_apply_tensor_path(const ttt_config* cfg);
-// hd = 128 apply kernel (bf16_apply_wide.cu)
+// hd = 128 apply kernel on CTA pairs (bf16_apply_wide_pair.cu)
 int bf16_apply_wide_supported(const ttt_config* cfg);
-// the same on CTA pairs (bf16_apply_wide_pair.cu)
 int bf16_apply_wide_pair(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
                          cudaStream_t s);
-int bf16_apply_wide(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
-                    cudaStream_t s);
 // hd = 128 update kernel (bf16_update_wide.cu)
 int bf16_update_wide_supported(const ttt_config* cfg);
 int bf16_accumulate_wide(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V, const float* lr,

@@ -1,8 +1,9 @@
 """Parity of the CUDA path (through the C ABI) against the float64 oracle, same seeded inputs.
 
 Tolerances (BASELINE.json:north_star): err(X) = max|X_gpu - X_ora| /
-max|X_ora| per tensor (reading P17). fp32 path: <= 1e-4 on every chunk's O and on the final
-fast weights. bf16 path: <= 2e-2 on outputs and updated fast weights after the final chunk.
+max|X_ora| per tensor and PER HEAD, worst head asserted (reading P17, tests/parity_metrics.py).
+fp32 path: <= 1e-4 on every chunk's O and on the final fast weights. bf16 path: <= 2e-2 on outputs
+and updated fast weights after the final chunk (asserted on EVERY chunk's outputs).
 """
 import numpy as np
 import pytest
@@ -10,6 +11,7 @@ import torch
 
 import ttt_inputs as ti
 from oracle.ttt_oracle import OracleTTT, rel_err
+from parity_metrics import worst_head_tokens, worst_head_weights
 
 pytestmark = pytest.mark.gpu
 
@@ -40,10 +42,10 @@ def _run_stream(w: ti.TTTWorkload, check_loss=True):
         loss = torch.zeros(w.nh, dtype=torch.float32, device=dev)
         O = gpu.ttt_chunk_step(Q.to(dev), K.to(dev), V.to(dev), lr.to(dev), loss=loss)
         O_ref, loss_ref = ora.chunk_step(Q, K, V, lr)
-        errs_o.append(rel_err(O.float().cpu(), O_ref))
+        errs_o.append(worst_head_tokens(O.float().cpu(), O_ref, w.nh))
         errs_l.append(rel_err(loss.cpu(), loss_ref))
-    g1, g2, g3 = (x.cpu() for x in gpu.ttt_get_weights())
-    errs_w = [rel_err(g1, ora.W1), rel_err(g2, ora.W2), rel_err(g3, ora.W3)]
+    g = [x.cpu() for x in gpu.ttt_get_weights()]
+    errs_w = [worst_head_weights([a], [b]) for a, b in zip(g, (ora.W1, ora.W2, ora.W3))]
     gpu.close()
     return errs_o, errs_w, errs_l
 
@@ -189,25 +191,6 @@ def test_bf16_wide_head_gradient_and_apply(M):
     gpu.close()
 
 
-def test_bf16_wide_head_apply_single_cta_variant():
-    """The hd = 128 apply runs on CTA pairs by default (bf16_apply_wide_pair.cu). The single-CTA
-    kernel (bf16_apply_wide.cu, selected with TTT_APPLY_WIDE_PAIR=0 when the library is first used,
-    hence a fresh process) is kept for A/B measurements: the hd-128 parity cases — many units per
-    CTA, ragged tails, chunks smaller than a tile, the cfg5-shaped stream, bitwise determinism — pass
-    with it too."""
-    import os
-    import subprocess
-    import sys
-    env = dict(os.environ, TTT_APPLY_WIDE_PAIR="0")
-    r = subprocess.run([sys.executable, "-m", "pytest", os.path.abspath(__file__), "-q", "-x", "-m", "gpu", "-k",
-                        "wide_head_gradient_and_apply or wide_head_more_pairs or cfg5_shape or tiny_chunks "
-                        "or determinism"],
-                       env=env, capture_output=True, text=True, timeout=900,
-                       cwd=os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
-    assert r.returncode == 0, r.stdout[-3000:] + r.stderr[-2000:]
-    assert " passed" in r.stdout and "failed" not in r.stdout
-
-
 def test_bf16_wide_head_more_pairs_than_sms():
     """hd = 128 gradient kernel when (head, slice) pairs outnumber the SMs: 40 heads x 4 slices = 160
     pairs, so a CTA's unit range crosses several pair boundaries (one segment per pair)."""
@@ -325,6 +308,13 @@ def test_accumulate_commit_equals_update_on_concatenation(hd):
     b.ttt_update(torch.cat([K0, K1]), torch.cat([V0, V1]), torch.cat([l0, l1], dim=1).contiguous())
     for x, y in zip(a.ttt_get_weights(), b.ttt_get_weights()):
         assert rel_err(x.cpu(), y.cpu()) <= 1e-5
+    # ... and both against the oracle's statement of Eq. 10: gradients of the two chunks at the SAME W
+    # summed, one update
+    cW = [x.cpu() for x in (W1, W2, W3)]
+    ora = OracleTTT(*cW)
+    G = [sum(t) for t in zip(*(ora.grad(K.cpu(), V.cpu(), l.cpu())[:3] for K, V, l in ((K0, V0, l0), (K1, V1, l1))))]
+    expect = [cW[0].double().numpy() - G[0], cW[1].double().numpy() - G[1], cW[2].double().numpy() - G[2]]
+    assert worst_head_weights([x.cpu() for x in a.ttt_get_weights()], expect) <= TOL_BF16
     a.close(); b.close()
 
 
@@ -379,9 +369,9 @@ def _full_size_stream(name, n_chunks, heads):
         O = gpu.ttt_chunk_step(Q.to(dev), K.to(dev), V.to(dev), lr.to(dev))
         O_ref, _ = ora.chunk_step(Q[:, cols].contiguous(), K[:, cols].contiguous(),
                                   V[:, cols].contiguous(), lr[heads].contiguous())
-        errs.append(rel_err(O[:, cols.to(dev)].float().cpu(), O_ref))
+        errs.append(worst_head_tokens(O[:, cols.to(dev)].float().cpu(), O_ref, len(heads)))
     g = [x.cpu()[heads] for x in gpu.ttt_get_weights()]
-    errs_w = [rel_err(g[0], ora.W1), rel_err(g[1], ora.W2), rel_err(g[2], ora.W3)]
+    errs_w = [worst_head_weights([a], [b]) for a, b in zip(g, (ora.W1, ora.W2, ora.W3))]
     gpu.close()
     return errs, errs_w
 
@@ -471,3 +461,105 @@ def test_long_stream_is_stable_and_per_chunk_time_is_flat():
     assert all(bool(torch.isfinite(x).all()) for x in g.ttt_get_weights())
     assert np.median(t[40:]) <= 1.25 * np.median(t[:20]), (np.median(t[:20]), np.median(t[40:]))
     g.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# boundary: no silent CUDA-core fallback
+# ------------------------------------------------------------------------------------------------
+def test_bf16_shape_without_tensor_kernel_is_rejected_unless_opted_in():
+    """include/ttt.h: a bf16 shape no tcgen05 kernel takes (hd 64 / hidden 512) is TTT_ERR_UNSUPPORTED
+    with a reason, never a silent slow path; cfg.cuda_core_fallback = 1 opts into the fp32 CUDA-core
+    kernels, which ttt_kernel_path reports, and those still match the oracle."""
+    from paper_2604_08542_b200 import TTT, TTT_BF16, TTTError
+    dev = torch.device("cuda", 0)
+    with pytest.raises(TTTError) as e:
+        TTT(2, 64, 512, TTT_BF16, max_tokens=256)
+    assert e.value.status == -5 and "cuda_core_fallback" in str(e.value)
+    t = TTT(2, 64, 128, TTT_BF16, max_tokens=256)
+    assert t.kernel_path() == (True, True)
+    t.close()
+    w = _bf16_workload("cfg2", nh=2, hidden=512, tokens_per_frame=100, frames_per_chunk=2, n_frames=2)
+    W1, W2, W3 = ti.fast_weights(w)
+    Q, K, V, lr = ti.TokenStream(w).next_chunk()
+    t = TTT(w.nh, w.hd, w.hidden, TTT_BF16, max_tokens=w.chunk_tokens, cuda_core_fallback=1)
+    assert t.kernel_path() == (False, False)
+    t.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    O = t.ttt_chunk_step(Q.to(dev), K.to(dev), V.to(dev), lr.to(dev))
+    ora = OracleTTT(W1, W2, W3)
+    O_ref, _ = ora.chunk_step(Q, K, V, lr)
+    assert worst_head_tokens(O.float().cpu(), O_ref, w.nh) <= TOL_BF16
+    assert worst_head_weights([x.cpu() for x in t.ttt_get_weights()], ora.weights()) <= TOL_BF16
+    t.close()
+
+
+@pytest.mark.parametrize("nh", [16, 7])
+def test_bf16_fused_commit_renorm_when_warps_straddle_the_commit_ranges(nh):
+    """Fused commit + re-normalisation with hd 64 / hidden 128: nh = 16 gives 9 token splits per (head,
+    slice), i.e. commit ranges of 688 float4 whose ends fall inside a warp and inside the W2 block
+    (the row-norm shuffles must be executed by every lane); nh = 7 gives 21 splits. 3 chunks."""
+    w = _bf16_workload("cfg4", nh=nh, hidden=128, tokens_per_frame=24 * 32 + 7, frames_per_chunk=1, n_frames=3)
+    errs_o, errs_w, errs_l = _run_stream(w)
+    assert max(errs_o) <= TOL_BF16, errs_o
+    assert max(errs_w) <= TOL_BF16, errs_w
+    assert max(errs_l) <= TOL_LOSS_BF16, errs_l
+
+
+# ------------------------------------------------------------------------------------------------
+# north_star's bar "after the FINAL chunk", at full size: the whole 63-chunk cfg4 stream and the whole
+# 32-chunk cfg5 stream through the CUDA path (all heads, the launch configuration bench.py times) and
+# through the float64 oracle (two heads each; heads are independent, so this is exact per head; the
+# oracle's OpenMP is over heads, the two streams run in two threads: ~7 minutes of wall time).
+# Kept LAST in the file. Asserts err(O_c) <= 2e-2 for EVERY chunk and err(W) <= 2e-2 after the last,
+# per head, worst head; writes the per-chunk curves to gpurun_out/ (DESIGN.md section 7's table).
+# ------------------------------------------------------------------------------------------------
+def _full_stream_curve(name, heads, out):
+    from parity_metrics import per_head_err_tokens, per_head_err_weights
+    dev = torch.device("cuda", 0)
+    w = ti.CONFIGS[name]
+    W1, W2, W3 = ti.fast_weights(w)
+    cols = torch.cat([torch.arange(h * w.hd, (h + 1) * w.hd) for h in heads])
+    ora = OracleTTT(W1[heads], W2[heads], W3[heads], ns_iters=w.ns_iters, renorm=w.renorm)
+    gpu = _mk(w)
+    gpu.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    rows = []
+    for c, (Q, K, V, lr) in enumerate(ti.TokenStream(w)):
+        O = gpu.ttt_chunk_step(Q.to(dev), K.to(dev), V.to(dev), lr.to(dev))
+        O_ref, _ = ora.chunk_step(Q[:, cols].contiguous(), K[:, cols].contiguous(),
+                                  V[:, cols].contiguous(), lr[heads].contiguous())
+        eo = per_head_err_tokens(O[:, cols.to(dev)].float().cpu(), O_ref, len(heads))
+        g = [x.cpu()[heads] for x in gpu.ttt_get_weights()]
+        ew = [max(per_head_err_weights(a, b)[i] for a, b in zip(g, (ora.W1, ora.W2, ora.W3)))
+              for i in range(len(heads))]
+        rows.append((c, Q.shape[0], max(eo), max(ew), float(np.sqrt(np.mean(np.asarray(O_ref) ** 2)))))
+    gpu.close()
+    out[name] = rows
+
+
+def test_cfg4_and_cfg5_full_streams_meet_the_bar_on_every_chunk():
+    import os
+    import threading
+    out = {}
+    jobs = [threading.Thread(target=_full_stream_curve, args=("cfg4", [3, 12], out)),
+            threading.Thread(target=_full_stream_curve, args=("cfg5", [2, 5], out))]
+    for j in jobs:
+        j.start()
+    for j in jobs:
+        j.join()
+    assert set(out) == {"cfg4", "cfg5"}, "a stream thread failed"
+    try:                                    # the curves, for DESIGN.md (scratch folder of a gpurun call)
+        root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+        os.makedirs(os.path.join(root, "gpurun_out"), exist_ok=True)
+        for name, rows in out.items():
+            with open(os.path.join(root, "gpurun_out", f"parity_full_stream_{name}.txt"), "w") as f:
+                f.write("# chunk tokens err_O(worst head) err_W(worst head, worst matrix) rms(O_ref)\n")
+                for r in rows:
+                    f.write("%d %d %.3e %.3e %.3e\n" % r)
+    except OSError:
+        pass
+    for name, n_chunks in (("cfg4", 63), ("cfg5", 32)):
+        rows = out[name]
+        assert len(rows) == n_chunks
+        worst_o = max(r[2] for r in rows)
+        assert worst_o <= TOL_BF16, (name, "outputs", [(r[0], r[2]) for r in rows if r[2] > TOL_BF16])
+        assert rows[-1][3] <= TOL_BF16, (name, "final weights", rows[-1])
+        assert max(r[3] for r in rows) <= TOL_BF16, (name, "weights", [(r[0], r[3]) for r in rows if r[3] > TOL_BF16])
