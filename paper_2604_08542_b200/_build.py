@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libttt_b200.so")
-SOURCES = ["ttt_api.cu", "state_kernels.cu", "f32_path.cu", "bf16_update.cu", "bf16_update_wide.cu", "bf16_apply.cu", "bf16_apply_wide_pair.cu", "ns_tc.cu", "ns_tc_wide.cu"]
+SOURCES = ["ttt_api.cu", "state_kernels.cu", "f32_path.cu", "bf16_update.cu", "bf16_update_wide.cu", "bf16_apply.cu", "bf16_apply_wide_pair.cu", "bf16_large.cu", "ns_tc.cu", "ns_tc_wide.cu"]
 HEADERS = ["ttt_internal.h", "tc_common.cuh", os.path.join("..", "..", "include", "ttt.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-cudart", "static"]

@@ -1,0 +1,489 @@
+// bf16_large.cu — the TTT hot path for LARGE head dimensions: the shape the paper itself ships, one
+// head of hd = d = 1024 with hidden H = k hd, k in {1, 2, 4} (PAPER.md:382 after Eq. 13; Table 3,
+// PAPER.md:242), and in general hd a multiple of 256, H a multiple of 128.
+//
+// With hd >= 256 nothing of a (head, hidden-slice) fits on one SM any more: the three fp32 gradient
+// slices [128 x hd] alone exceed TMEM, and a hidden slice of the weights exceeds shared memory. On the
+// other hand every contraction now has all three dimensions >= 256, and the flop-per-byte ratio of the
+// layer (~ hd) lets the hidden activations go through HBM once. So the path is four tiled GEMMs, all
+// tcgen05 bf16 x bf16 -> fp32 with TMA-fed shared-memory operands and persistent CTAs:
+//   update  (Eq. 8 with Eq. 9, Eq. 12)
+//     F_u   x | b = K [W1 | W3] and g0 = V W2^T per [128 tokens x 128 hidden] tile (contraction over hd in
+//           64-wide chunks), fused SwiGLU forward + backward epilogue -> dA, dB, Hd' = -eta Hd (bf16, HBM)
+//     G     G1^T = dA^T K, G3^T = dB^T K, G2 = Hd'^T V per [128 hidden x 256 hd] tile (contraction over ALL
+//           tokens of the chunk, both operands MN-major), dense fp32 gradient out (+= pending)
+//     commit_plain_kernel (state_kernels.cu): W <- W - G
+//   apply   (Eq. 4)
+//     F_a   x | b = Q [W1 | W3], epilogue Hq = SiLU(x) b (bf16, HBM)
+//     D     O = Hq W2 per [128 tokens x 256 hd] tile (contraction over H, B = W2 rows MN-major)
+// Operands are bf16 on this path (weights: the bf16 copy Wq; activations: bf16 keeps fp32's range, so the
+// gradient operands need no learning-rate scaling); Newton-Schulz / re-normalisation are not offered
+// here (the paper defines neither; ttt_create rejects them for hd > 128).
+#include <stdio.h>
+
+#include "tc_common.cuh"
+#include "ttt_internal.h"
+
+namespace ttt {
+
+int make_token_map(ttt_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int64_t cols,
+                   int64_t ld, int box_rows);  // bf16_update.cu
+
+namespace lg {
+constexpr int TM = 128;            // rows of an output tile = TMEM lanes
+constexpr int KC = 64;             // contraction chunk (one 128-byte swizzled row of bf16)
+constexpr int THREADS = 384;       // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warp 3 idle, warps 4-11 epilogue
+constexpr int EPI_WARPS = 8;
+constexpr int BOX = TM * 128;      // bytes of a [128 rows x 64] bf16 box (16 KB); a [64 x 64] box is BOX / 2
+// forward kernels: stage = token chunk(s) + weight-row chunks
+constexpr int F_STAGE_U = 5 * BOX, F_STAGES_U = 2;     // K, [W1 | W3], V, W2
+constexpr int F_STAGE_A = 3 * BOX, F_STAGES_A = 4;     // Q, [W1 | W3]
+constexpr uint32_t C_XB = 0, C_G = 256;                // x | b [128 x 256] fp32, g0 [128 x 128] fp32
+// MN-major-B kernels: stage = A 16 KB + B 32 KB, two accumulators [128 x 256] fp32
+constexpr int M_STAGE = 3 * BOX, M_STAGES = 4;
+constexpr int TN = 256;
+}  // namespace lg
+
+// ------------------------------------------------------------------------------------------------
+// F: forward products + SwiGLU epilogue. UPD: update (x | b | g0 -> dA, dB, Hd'); else apply (-> Hq).
+// Work item = (token tile tt, hidden slice s, head h), slice fastest; persistent CTAs.
+// ------------------------------------------------------------------------------------------------
+template <bool UPD, bool LOSS>
+__global__ void __launch_bounds__(lg::THREADS, 1)
+ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapV,
+                  const __grid_constant__ CUtensorMap mapW, const float* __restrict__ lr,
+                  __nv_bfloat16* __restrict__ act0, __nv_bfloat16* __restrict__ act1,
+                  __nv_bfloat16* __restrict__ act2, float* __restrict__ loss_part, int M, int nh, int hd,
+                  int H, int n_items) {
+  using namespace lg;
+  constexpr int STAGE = UPD ? F_STAGE_U : F_STAGE_A;
+  constexpr int STAGES = UPD ? F_STAGES_U : F_STAGES_A;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
+  __shared__ uint64_t full[STAGES], empty[STAGES], acc_full, acc_empty;
+  __shared__ uint32_t tmem_base_s;
+  __shared__ float loss_red[EPI_WARPS];
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int nslices = H / TM, ntt = (M + TM - 1) / TM, nkc = hd / KC;
+  if (tid == 0) {
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    mbar_init(&acc_full, 1);
+    mbar_init(&acc_empty, EPI_WARPS);
+    fence_mbar_init();
+    tma_prefetch_desc(&mapX);
+    tma_prefetch_desc(&mapW);
+    if (UPD) tma_prefetch_desc(&mapV);
+  }
+  if (warp == 2) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tb = tmem_base_s;
+  // programmatic dependent launch: the weights (commit) / activations come from the kernel before
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+
+  auto item = [&](int id, int& h, int& tt, int& s) {
+    s = id % nslices;
+    const int r = id / nslices;
+    tt = r % ntt;
+    h = r / ntt;
+  };
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (elect_one()) {
+      int g = 0;                                       // running chunk counter over all items
+      for (int id = blockIdx.x; id < n_items; id += gridDim.x) {
+        int h, tt, s;
+        item(id, h, tt, s);
+        for (int kc = 0; kc < nkc; ++kc, ++g) {
+          const int st = g % STAGES;
+          if (g >= STAGES) mbar_wait(&empty[st], ((g / STAGES) - 1) & 1);
+          mbar_arrive_expect_tx(&full[st], STAGE);
+          uint8_t* dst = smem + st * STAGE;
+          tma_load_2d(dst, &mapX, &full[st], h * hd + kc * KC, tt * TM);                               // K or Q chunk
+          tma_load_2d(dst + BOX, &mapW, &full[st], kc * KC, (0 * nh + h) * H + s * TM);               // W1^T rows
+          tma_load_2d(dst + 2 * BOX, &mapW, &full[st], kc * KC, (2 * nh + h) * H + s * TM);           // W3^T rows
+          if (UPD) {
+            tma_load_2d(dst + 3 * BOX, &mapV, &full[st], h * hd + kc * KC, tt * TM);                  // V chunk
+            tma_load_2d(dst + 4 * BOX, &mapW, &full[st], kc * KC, (1 * nh + h) * H + s * TM);         // W2 rows
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (elect_one()) {
+      constexpr uint32_t idesc_xb = umma_idesc_bf16(TM, 256, 0, 0);   // A = token chunk, B = [W1 ; W3] rows, K-major
+      constexpr uint32_t idesc_g = umma_idesc_bf16(TM, 128, 0, 0);    // A = V chunk, B = W2 rows
+      const uint64_t d0 = umma_smem_desc_sw128(sbase, 16, 1024);
+      int g = 0, n = 0;
+      for (int id = blockIdx.x; id < n_items; id += gridDim.x, ++n) {
+        if (n > 0) { mbar_wait(&acc_empty, (n - 1) & 1); tc_fence_after(); }   // epilogue has read the accumulators
+        for (int kc = 0; kc < nkc; ++kc, ++g) {
+          const int st = g % STAGES;
+          mbar_wait(&full[st], (g / STAGES) & 1);
+          tc_fence_after();
+          const uint64_t ds = d0 + (uint64_t)(st * (STAGE >> 4));
+#pragma unroll
+          for (int k = 0; k < KC / 16; ++k) {
+            umma_ss(tb + C_XB, ds + 2 * k, ds + (BOX >> 4) + 2 * k, idesc_xb, (kc > 0) | k);
+            if (UPD) umma_ss(tb + C_G, ds + 3 * (BOX >> 4) + 2 * k, ds + 4 * (BOX >> 4) + 2 * k, idesc_g, (kc > 0) | k);
+          }
+          tc_commit(&empty[st]);
+        }
+        tc_commit(&acc_full);
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================== epilogue: thread = token row (TMEM lane), 8 groups of 16 hidden columns =====================
+    const int q = warp & 3, half = (warp - 4) >> 2;
+    const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
+    const uint64_t HALF2 = pack2(0.5f, 0.5f), ONE2 = pack2(1.0f, 1.0f), NONE2 = pack2(-1.0f, -1.0f);
+    int n = 0;
+    for (int id = blockIdx.x; id < n_items; id += gridDim.x, ++n) {
+      int h, tt, s;
+      item(id, h, tt, s);
+      const int tok = tt * TM + q * 32 + lane;
+      float nef = 0.f;
+      if (UPD && tok < M) nef = -__ldg(lr + (size_t)h * M + tok);
+      const uint64_t ne = pack2(nef, nef);
+      uint64_t loss2 = 0ull;
+      mbar_wait(&acc_full, n & 1);
+      tc_fence_after();
+      const size_t row_off = (size_t)tok * ((size_t)nh * H) + (size_t)h * H + (size_t)s * TM;
+#pragma unroll 1
+      for (int c = 4 * half; c < 4 * half + 4; ++c) {
+        uint32_t rx[16], rb[16], rg[16];
+        tmem_ld_x16(tb + lane_base + C_XB + 16 * c, rx);
+        tmem_ld_x16(tb + lane_base + C_XB + 128 + 16 * c, rb);
+        if (UPD) tmem_ld_x16(tb + lane_base + C_G + 16 * c, rg);
+        tc_wait_ld();
+        uint32_t pa[8], pb[8], ph[8];
+#pragma unroll
+        for (int e = 0; e < 16; e += 2) {
+          const uint64_t x = fmul2(pack2u(rx[e], rx[e + 1]), HALF2);            // a / 2
+          const uint64_t bb = pack2u(rb[e], rb[e + 1]);
+          float x0, x1;
+          unpack2(x, x0, x1);
+          const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
+          const uint64_t S = ffma2(x, th, x);                                   // SiLU(a) = a sigmoid(a)
+          const uint64_t hdv = fmul2(S, bb);                                    // Hd (update) / Hq (apply)
+          if (UPD) {
+            const uint64_t g = fmul2(ne, pack2u(rg[e], rg[e + 1]));             // dHd = (-eta v) W2^T
+            const uint64_t p = fadd2(th, ONE2);                                 // 2 sigmoid(a)
+            const uint64_t m = ffma2(th, NONE2, ONE2);                          // 2 (1 - sigmoid(a))
+            const uint64_t t1 = fmul2(ffma2(S, m, p), HALF2);                   // SiLU'(a)
+            pa[e >> 1] = pack_bf16x2_from2(fmul2(fmul2(g, bb), t1));            // dA
+            pb[e >> 1] = pack_bf16x2_from2(fmul2(g, S));                        // dB
+            ph[e >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));                     // Hd' = -eta Hd
+            if (LOSS) loss2 = ffma2(hdv, g, loss2);
+          } else {
+            ph[e >> 1] = pack_bf16x2_from2(hdv);
+          }
+        }
+        if (tok < M) {
+          if (UPD) {
+            uint4* d0p = reinterpret_cast<uint4*>(act0 + row_off + 16 * c);
+            uint4* d1p = reinterpret_cast<uint4*>(act1 + row_off + 16 * c);
+            d0p[0] = make_uint4(pa[0], pa[1], pa[2], pa[3]); d0p[1] = make_uint4(pa[4], pa[5], pa[6], pa[7]);
+            d1p[0] = make_uint4(pb[0], pb[1], pb[2], pb[3]); d1p[1] = make_uint4(pb[4], pb[5], pb[6], pb[7]);
+          }
+          uint4* d2p = reinterpret_cast<uint4*>((UPD ? act2 : act0) + row_off + 16 * c);
+          d2p[0] = make_uint4(ph[0], ph[1], ph[2], ph[3]); d2p[1] = make_uint4(ph[4], ph[5], ph[6], ph[7]);
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&acc_empty);
+      if (UPD && LOSS) {
+        float l0, l1;
+        unpack2(loss2, l0, l1);
+        float loss = l0 + l1;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) loss += __shfl_xor_sync(0xffffffffu, loss, o);
+        asm volatile("bar.sync 1, 256;" ::: "memory");       // loss_red of the previous item has been read
+        if (lane == 0) loss_red[warp - 4] = loss;
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        if (warp == 4 && lane == 0) {
+          float t = 0.f;
+          for (int w = 0; w < EPI_WARPS; ++w) t += loss_red[w];
+          loss_part[(size_t)(tt * nslices + s) * nh + h] = t;
+        }
+      }
+    }
+  }
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) tmem_dealloc(tb, 512);
+}
+
+// ------------------------------------------------------------------------------------------------
+// G / D: D [128 x 256] (+)= A . B with B MN-major ([contraction rows][256 output columns] in memory).
+//   GRAD (A_MN):  tile (matrix j, hidden block hb, hd block nb, head h), contraction over the chunk's tokens;
+//                 A = act_j [tokens][hidden] (MN-major), B = K (j = 0, 2) or V (j = 1) [tokens][hd];
+//                 out: G[j][h][hb 128 + row][nb 256 + col] (+= when `accumulate`)
+//   DOWN:         tile (token tile tt, hd block nb, head h), contraction over H;
+//                 A = Hq [tokens][hidden] (K-major), B = W2 rows [hidden][hd]; out: O bf16
+// Accumulators are double-buffered in TMEM: the epilogue of a tile overlaps the next tile's main loop.
+// ------------------------------------------------------------------------------------------------
+template <bool GRAD>
+__global__ void __launch_bounds__(lg::THREADS, 1)
+ld_mn_gemm_kernel(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
+                  const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ CUtensorMap mapB0,
+                  const __grid_constant__ CUtensorMap mapB1, float* __restrict__ G,
+                  __nv_bfloat16* __restrict__ O, int64_t ldo, int M, int nh, int hd, int H, int n_items,
+                  int accumulate) {
+  using namespace lg;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
+  __shared__ uint64_t full[M_STAGES], empty[M_STAGES], acc_full[2], acc_empty[2];
+  __shared__ uint32_t tmem_base_s;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int nnb = hd / TN;                                  // hd blocks of 256
+  const int nhb = H / TM, ntt = (M + TM - 1) / TM;
+  const int nkc = GRAD ? (M + KC - 1) / KC : H / KC;
+  if (tid == 0) {
+    for (int s = 0; s < M_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&acc_full[b], 1); mbar_init(&acc_empty[b], EPI_WARPS); }
+    fence_mbar_init();
+    tma_prefetch_desc(&mapA0);
+    tma_prefetch_desc(&mapB0);
+  }
+  if (warp == 2) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tb = tmem_base_s;
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+
+  // GRAD: id -> (j, h, hb, nb), nb fastest (the four hd blocks of a hidden block share their A stream);
+  // DOWN: id -> (h, tt, nb)
+  auto item = [&](int id, int& j, int& h, int& rb, int& nb) {
+    nb = id % nnb;
+    int r = id / nnb;
+    if (GRAD) { rb = r % nhb; r /= nhb; h = r % nh; j = r / nh; }
+    else { rb = r % ntt; h = r / ntt; j = 0; }
+  };
+
+  if (warp == 0) {
+    if (elect_one()) {
+      int g = 0;
+      for (int id = blockIdx.x; id < n_items; id += gridDim.x) {
+        int j, h, rb, nb;
+        item(id, j, h, rb, nb);
+        const CUtensorMap* mA = GRAD ? (j == 0 ? &mapA0 : j == 1 ? &mapA2 : &mapA1) : &mapA0;   // dA, Hd', dB
+        const CUtensorMap* mB = GRAD ? (j == 1 ? &mapB1 : &mapB0) : &mapB0;                      // K | V ; W2 rows
+        for (int kc = 0; kc < nkc; ++kc, ++g) {
+          const int st = g % M_STAGES;
+          if (g >= M_STAGES) mbar_wait(&empty[st], ((g / M_STAGES) - 1) & 1);
+          mbar_arrive_expect_tx(&full[st], M_STAGE);
+          uint8_t* dst = smem + st * M_STAGE;
+          if (GRAD) {
+            // A: two [64 tokens x 64 hidden] atoms (hidden halves of the block)
+            tma_load_2d(dst, mA, &full[st], h * H + rb * TM, kc * KC);
+            tma_load_2d(dst + BOX / 2, mA, &full[st], h * H + rb * TM + 64, kc * KC);
+            // B: four [64 tokens x 64 hd] atoms
+            for (int a = 0; a < 4; ++a)
+              tma_load_2d(dst + BOX + a * (BOX / 2), mB, &full[st], h * hd + nb * TN + 64 * a, kc * KC);
+          } else {
+            tma_load_2d(dst, mA, &full[st], h * H + kc * KC, rb * TM);              // Hq [128 tokens x 64 hidden]
+            for (int a = 0; a < 4; ++a)                                             // W2 rows [64 hidden x 64 hd] x 4
+              tma_load_2d(dst + BOX + a * (BOX / 2), mB, &full[st], nb * TN + 64 * a, (1 * nh + h) * H + kc * KC);
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (elect_one()) {
+      constexpr uint32_t idesc = umma_idesc_bf16(TM, TN, GRAD ? 1 : 0, 1);
+      const uint64_t dA = GRAD ? umma_smem_desc_sw128(sbase, BOX / 2, 1024) : umma_smem_desc_sw128(sbase, 16, 1024);
+      const uint64_t dB = umma_smem_desc_sw128(sbase + BOX, BOX / 2, 1024);
+      int g = 0, n = 0;
+      for (int id = blockIdx.x; id < n_items; id += gridDim.x, ++n) {
+        const int ab = n & 1;
+        if (n >= 2) { mbar_wait(&acc_empty[ab], ((n >> 1) - 1) & 1); tc_fence_after(); }
+        const uint32_t acc = tb + ab * TN;
+        for (int kc = 0; kc < nkc; ++kc, ++g) {
+          const int st = g % M_STAGES;
+          mbar_wait(&full[st], (g / M_STAGES) & 1);
+          tc_fence_after();
+          const uint64_t so = (uint64_t)(st * (M_STAGE >> 4));
+#pragma unroll
+          for (int k = 0; k < KC / 16; ++k)            // MN-major: +2048 B per 16-row K step; K-major: +32 B
+            umma_ss(acc, dA + so + (GRAD ? 128 * k : 2 * k), dB + so + 128 * k, idesc, (kc > 0) | k);
+          tc_commit(&empty[st]);
+        }
+        tc_commit(&acc_full[ab]);
+      }
+    }
+  } else if (warp >= 4) {
+    const int q = warp & 3, half = (warp - 4) >> 2;
+    const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
+    int n = 0;
+    for (int id = blockIdx.x; id < n_items; id += gridDim.x, ++n) {
+      int j, h, rb, nb;
+      item(id, j, h, rb, nb);
+      const int ab = n & 1;
+      const int row = rb * TM + q * 32 + lane;
+      mbar_wait(&acc_full[ab], (n >> 1) & 1);
+      tc_fence_after();
+#pragma unroll 1
+      for (int c = 0; c < 4; ++c) {                    // 32 columns per TMEM round trip
+        uint32_t r[32];
+        tmem_ld_x32(tb + lane_base + ab * TN + 128 * half + 32 * c, r);
+        tc_wait_ld();
+        const int col = nb * TN + 128 * half + 32 * c;
+        if (GRAD) {
+          float4* dst = reinterpret_cast<float4*>(G + (((size_t)j * nh + h) * H + row) * hd + col);
+#pragma unroll
+          for (int v = 0; v < 8; ++v) {
+            float4 o = make_float4(__uint_as_float(r[4 * v]), __uint_as_float(r[4 * v + 1]),
+                                   __uint_as_float(r[4 * v + 2]), __uint_as_float(r[4 * v + 3]));
+            if (accumulate) { const float4 p = dst[v]; o.x += p.x; o.y += p.y; o.z += p.z; o.w += p.w; }
+            dst[v] = o;
+          }
+        } else if (row < M) {
+          uint4* dst = reinterpret_cast<uint4*>(O + (size_t)row * ldo + (size_t)h * hd + col);
+#pragma unroll
+          for (int v = 0; v < 4; ++v)
+            dst[v] = make_uint4(pack_bf16x2(__uint_as_float(r[8 * v]), __uint_as_float(r[8 * v + 1])),
+                                pack_bf16x2(__uint_as_float(r[8 * v + 2]), __uint_as_float(r[8 * v + 3])),
+                                pack_bf16x2(__uint_as_float(r[8 * v + 4]), __uint_as_float(r[8 * v + 5])),
+                                pack_bf16x2(__uint_as_float(r[8 * v + 6]), __uint_as_float(r[8 * v + 7])));
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&acc_empty[ab]);
+    }
+  }
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) tmem_dealloc(tb, 512);
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+int bf16_large_supported(const ttt_config* cfg) {
+  return cfg->act_dtype == TTT_BF16 && cfg->hd >= 256 && cfg->hd % 256 == 0 && cfg->hd <= 2048 &&
+         cfg->hidden % 128 == 0 && cfg->ns_iters == 0 && cfg->renorm == 0 && !cfg->linear_fast_weight;
+}
+
+int64_t bf16_large_loss_rows(const ttt_config* cfg) {
+  return ((cfg->max_tokens + lg::TM - 1) / lg::TM) * (cfg->hidden / lg::TM);
+}
+
+template <typename Kern, typename... Args>
+static int launch_pdl(ttt_ctx* ctx, const char* what, Kern kern, int grid, size_t smem, cudaStream_t s, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(lg::THREADS);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  cudaError_t e = cudaLaunchKernelEx(&cfg, kern, args...);
+  if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, what, e);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, what, e);
+  ctx->launches += 1;
+  return TTT_OK;
+}
+
+static int large_attrs(ttt_ctx* ctx) {
+  if (ctx->attr_done & ATTR_LARGE) return TTT_OK;
+  const int su = lg::F_STAGE_U * lg::F_STAGES_U + 1024, sa = lg::F_STAGE_A * lg::F_STAGES_A + 1024;
+  const int sm = lg::M_STAGE * lg::M_STAGES + 1024;
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, su), "ld_forward smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, su), "ld_forward smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sa), "ld_forward smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_mn_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "ld_mn_gemm smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_mn_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "ld_mn_gemm smem attr");
+  ctx->attr_done |= ATTR_LARGE;
+  return TTT_OK;
+}
+
+// steps 1-5: forward + epilogue, then the three gradient GEMMs into the dense pending gradient G
+int bf16_large_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V, const float* lr,
+                          int64_t M, int64_t ld, bool want_loss, int* loss_rows, cudaStream_t s) {
+  const ttt_config& c = ctx->cfg;
+  int rc = large_attrs(ctx);
+  if (rc != TTT_OK) return rc;
+  const int64_t HW = (int64_t)c.nh * c.hidden;
+  CUtensorMap mK, mV, mW, mA0, mA1, mA2, mK64, mV64;
+  if ((rc = make_token_map(ctx, &mK, K, M, (int64_t)c.nh * c.hd, ld, lg::TM)) != TTT_OK) return rc;
+  if ((rc = make_token_map(ctx, &mV, V, M, (int64_t)c.nh * c.hd, ld, lg::TM)) != TTT_OK) return rc;
+  if ((rc = make_token_map(ctx, &mW, ctx->Wq, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, lg::TM)) != TTT_OK) return rc;
+  if ((rc = make_token_map(ctx, &mA0, ctx->lact[0], M, HW, HW, 64)) != TTT_OK) return rc;
+  if ((rc = make_token_map(ctx, &mA1, ctx->lact[1], M, HW, HW, 64)) != TTT_OK) return rc;
+  if ((rc = make_token_map(ctx, &mA2, ctx->lact[2], M, HW, HW, 64)) != TTT_OK) return rc;
+  if ((rc = make_token_map(ctx, &mK64, K, M, (int64_t)c.nh * c.hd, ld, 64)) != TTT_OK) return rc;
+  if ((rc = make_token_map(ctx, &mV64, V, M, (int64_t)c.nh * c.hd, ld, 64)) != TTT_OK) return rc;
+  const int ntt = (int)((M + lg::TM - 1) / lg::TM), nsl = c.hidden / lg::TM;
+  int n_items = c.nh * ntt * nsl;
+  int grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
+  const size_t su = (size_t)lg::F_STAGE_U * lg::F_STAGES_U + 1024;
+  int Mi = (int)M, nh = c.nh, hd = c.hd, H = c.hidden;
+  if (want_loss)
+    rc = launch_pdl(ctx, "ld_forward_kernel (update)", ld_forward_kernel<true, true>, grid, su, s, mK, mV, mW, lr,
+                    ctx->lact[0], ctx->lact[1], ctx->lact[2], ctx->loss_part, Mi, nh, hd, H, n_items);
+  else
+    rc = launch_pdl(ctx, "ld_forward_kernel (update)", ld_forward_kernel<true, false>, grid, su, s, mK, mV, mW, lr,
+                    ctx->lact[0], ctx->lact[1], ctx->lact[2], ctx->loss_part, Mi, nh, hd, H, n_items);
+  if (rc != TTT_OK) return rc;
+  *loss_rows = ntt * nsl;
+  n_items = 3 * c.nh * nsl * (c.hd / lg::TN);
+  grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
+  const size_t sm = (size_t)lg::M_STAGE * lg::M_STAGES + 1024;
+  int accumulate = ctx->G_valid ? 1 : 0;
+  __nv_bfloat16* nullo = nullptr;
+  int64_t ldo = 0;
+  rc = launch_pdl(ctx, "ld_mn_gemm_kernel (gradient)", ld_mn_gemm_kernel<true>, grid, sm, s, mA0, mA1, mA2, mK64, mV64,
+                  ctx->G, nullo, ldo, Mi, nh, hd, H, n_items, accumulate);
+  if (rc != TTT_OK) return rc;
+  ctx->G_valid = true;
+  return TTT_OK;
+}
+
+int bf16_large_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
+                     cudaStream_t s) {
+  const ttt_config& c = ctx->cfg;
+  int rc = large_attrs(ctx);
+  if (rc != TTT_OK) return rc;
+  const int64_t HW = (int64_t)c.nh * c.hidden;
+  CUtensorMap mQ, mW, mHq, mW64;
+  if ((rc = make_token_map(ctx, &mQ, Q, M, (int64_t)c.nh * c.hd, ld, lg::TM)) != TTT_OK) return rc;
+  if ((rc = make_token_map(ctx, &mW, ctx->Wq, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, lg::TM)) != TTT_OK) return rc;
+  if ((rc = make_token_map(ctx, &mHq, ctx->lact[0], M, HW, HW, lg::TM)) != TTT_OK) return rc;
+  if ((rc = make_token_map(ctx, &mW64, ctx->Wq, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, 64)) != TTT_OK) return rc;
+  const int ntt = (int)((M + lg::TM - 1) / lg::TM), nsl = c.hidden / lg::TM;
+  int n_items = c.nh * ntt * nsl;
+  int grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
+  const size_t sa = (size_t)lg::F_STAGE_A * lg::F_STAGES_A + 1024;
+  int Mi = (int)M, nh = c.nh, hd = c.hd, H = c.hidden;
+  const float* nolr = nullptr;
+  __nv_bfloat16* nob = nullptr;
+  float* nof = nullptr;
+  rc = launch_pdl(ctx, "ld_forward_kernel (apply)", ld_forward_kernel<false, false>, grid, sa, s, mQ, mQ, mW, nolr,
+                  ctx->lact[0], nob, nob, nof, Mi, nh, hd, H, n_items);
+  if (rc != TTT_OK) return rc;
+  n_items = c.nh * ntt * (c.hd / lg::TN);
+  grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
+  const size_t sm = (size_t)lg::M_STAGE * lg::M_STAGES + 1024;
+  int accumulate = 0;
+  return launch_pdl(ctx, "ld_mn_gemm_kernel (down projection)", ld_mn_gemm_kernel<false>, grid, sm, s, mHq, mHq, mHq,
+                    mW64, mW64, nof, O, ld, Mi, nh, hd, H, n_items, accumulate);
+}
+
+}  // namespace ttt

@@ -707,6 +707,7 @@ static void update_split(const ttt_ctx* ctx, int64_t M, int* tiles_total, int* t
 }
 
 int bf16_partials_needed(const ttt_ctx* ctx, int64_t M) {
+  if (ctx->large) return 0;            // the gradient GEMMs write the dense gradient
   if (ctx->cfg.hd == 128) return bf16_wide_partials_needed(ctx, M);
   int a, b, s;
   update_split(ctx, M, &a, &b, &s);
@@ -717,10 +718,10 @@ static int narrow_tensor_path(const ttt_config* cfg) {
   return cfg->hd == 64 && (cfg->hidden == 128 || cfg->hidden == 256) && !cfg->linear_fast_weight;
 }
 int bf16_apply_tensor_path(const ttt_config* cfg) {
-  return narrow_tensor_path(cfg) || bf16_apply_wide_supported(cfg);
+  return narrow_tensor_path(cfg) || bf16_apply_wide_supported(cfg) || bf16_large_supported(cfg);
 }
 int bf16_update_tensor_path(const ttt_config* cfg) {
-  return narrow_tensor_path(cfg) || bf16_update_wide_supported(cfg);
+  return narrow_tensor_path(cfg) || bf16_update_wide_supported(cfg) || bf16_large_supported(cfg);
 }
 
 // bf16 token tensors are accepted for every shape the fp32 path takes; shapes outside the tcgen05

@@ -48,29 +48,32 @@ __global__ void init_load_kernel(const float* __restrict__ W1, const float* __re
   __nv_bfloat16* dstq = Wq ? Wq + mat * me + (size_t)h * H * hd : nullptr;
   if (mat == 1) {  // W2 [H][hd]: straight copy + column sums of squares over this CTA's rows
     const float* src = W2 + (size_t)h * H * hd;
-    float colacc[4] = {0.f, 0.f, 0.f, 0.f};
-    for (int r = ty; r < 32; r += 8) {
-      const int j = j0 + r;
-      if (j >= H) break;
+    for (int cb = 0; cb < hd; cb += 128) {           // 128 columns at a time (hd > 128: the paper's shape)
+      float colacc[4] = {0.f, 0.f, 0.f, 0.f};
+      for (int r = ty; r < 32; r += 8) {
+        const int j = j0 + r;
+        if (j >= H) break;
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const int i = tx + 32 * c;
-        if (i < hd) {
-          const float v = src[(size_t)j * hd + i];
-          dst[(size_t)j * hd + i] = v;
-          dstb[(size_t)j * hd + i] = ttt_to_wop(v);
-          if (dstq) dstq[(size_t)j * hd + i] = __float2bfloat16_rn(v);
-          colacc[c] = fmaf(v, v, colacc[c]);
+        for (int c = 0; c < 4; ++c) {
+          const int i = cb + tx + 32 * c;
+          if (i < hd) {
+            const float v = src[(size_t)j * hd + i];
+            dst[(size_t)j * hd + i] = v;
+            dstb[(size_t)j * hd + i] = ttt_to_wop(v);
+            if (dstq) dstq[(size_t)j * hd + i] = __float2bfloat16_rn(v);
+            colacc[c] = fmaf(v, v, colacc[c]);
+          }
         }
       }
-    }
+      __syncthreads();
 #pragma unroll
-    for (int c = 0; c < 4; ++c) cs[ty][tx + 32 * c] = colacc[c];
-    __syncthreads();
-    for (int i = ty * 32 + tx; i < hd; i += 256) {
-      float t = 0.f;
-      for (int w = 0; w < 8; ++w) t += cs[w][i];
-      colsq[((size_t)h * gridDim.x + blockIdx.x) * hd + i] = t;
+      for (int c = 0; c < 4; ++c) cs[ty][tx + 32 * c] = colacc[c];
+      __syncthreads();
+      for (int i = ty * 32 + tx; i < 128 && cb + i < hd; i += 256) {
+        float t = 0.f;
+        for (int w = 0; w < 8; ++w) t += cs[w][i];
+        colsq[((size_t)h * gridDim.x + blockIdx.x) * hd + cb + i] = t;
+      }
     }
     return;
   }
@@ -367,6 +370,25 @@ renorm_w2_kernel(float* __restrict__ Wm, ttt_wop_t* __restrict__ Wb, __nv_bfloat
   }
 }
 
+// plain commit for the large-dimension path (hd > 128: no Newton-Schulz, no re-normalisation):
+// W <- W - G element-wise (Eq. 8), fp32 master + fp16 and bf16 operand copies.
+__global__ void __launch_bounds__(256)
+commit_plain_kernel(float* __restrict__ Wm, ttt_wop_t* __restrict__ Wb, __nv_bfloat16* __restrict__ Wq,
+                    const float* __restrict__ G, size_t n4) {
+  const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n4) return;
+  float4 w = reinterpret_cast<const float4*>(Wm)[e];
+  const float4 g = reinterpret_cast<const float4*>(G)[e];
+  w.x -= g.x; w.y -= g.y; w.z -= g.z; w.w -= g.w;
+  reinterpret_cast<float4*>(Wm)[e] = w;
+  reinterpret_cast<uint2*>(Wb)[e] = make_uint2(ttt_pack_wop2(w.x, w.y), ttt_pack_wop2(w.z, w.w));
+  if (Wq) {
+    const __nv_bfloat162 lo = __floats2bfloat162_rn(w.x, w.y), hi = __floats2bfloat162_rn(w.z, w.w);
+    reinterpret_cast<uint2*>(Wq)[e] = make_uint2(*reinterpret_cast<const uint32_t*>(&lo),
+                                                  *reinterpret_cast<const uint32_t*>(&hi));
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
@@ -420,6 +442,14 @@ int launch_renorm_w2(ttt_ctx* ctx, int nblk, cudaStream_t s) {
 
 int launch_commit(ttt_ctx* ctx, cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
+  if (ctx->large) {                       // hd > 128: the gradient GEMMs left the dense gradient in G
+    const size_t n4 = 3 * ctx->mat_elems / 4;
+    commit_plain_kernel<<<(unsigned)((n4 + 255) / 256), 256, 0, s>>>(ctx->Wm, ctx->Wb, ctx->Wq, ctx->G, n4);
+    TTT_LAUNCH_CHECK(ctx, "commit_plain_kernel");
+    ctx->G_valid = false;
+    ctx->n_partials = 0;
+    return TTT_OK;
+  }
   if (c.ns_iters > 0 && ns_tc_supported(&c)) {
     // tensor-core NS; folds the partial sets itself and, without renorm, commits W <- W - NS(g)
     int rc = launch_ns_tc(ctx, c.renorm == 0, s);

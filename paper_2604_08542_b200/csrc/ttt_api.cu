@@ -65,6 +65,13 @@ int do_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, i
     if (rc != TTT_OK) return rc;
     K = ctx->stage[0]; V = ctx->stage[1]; ld = d;
   }
+  if (ctx->large) {                  // hd >= 256: forward + gradient GEMMs, dense pending gradient
+    int loss_rows = 0;
+    int rc = bf16_large_accumulate(ctx, static_cast<const __nv_bfloat16*>(K), static_cast<const __nv_bfloat16*>(V),
+                                   lr, M, ld, loss != nullptr, &loss_rows, s);
+    if (rc == TTT_OK && loss != nullptr) rc = launch_loss_reduce(ctx, loss_rows, loss, s);
+    return rc;
+  }
   const int need = bf16 ? bf16_partials_needed(ctx, M) : f32_partials_needed(ctx, M);
   if (need > ctx->cap_partials)
     return fail(ctx, TTT_ERR_SHAPE, "internal: %lld partial sets needed, capacity %lld", need,
@@ -101,6 +108,8 @@ int do_apply(ttt_ctx* ctx, const void* Q, void* O, int64_t M, int64_t ld, cudaSt
     if (rc == TTT_OK) rc = launch_f32_to_bf16(ctx, ctx->stage[1], static_cast<__nv_bfloat16*>(O), ld, M, s);
     return rc;
   }
+  if (ctx->large)
+    return bf16_large_apply(ctx, static_cast<const __nv_bfloat16*>(Q), static_cast<__nv_bfloat16*>(O), M, ld, s);
   if (ctx->cfg.act_dtype == TTT_BF16)
     return bf16_apply(ctx, static_cast<const __nv_bfloat16*>(Q), static_cast<__nv_bfloat16*>(O), M,
                       ld, s);
@@ -144,8 +153,9 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
       (cfg->cuda_core_fallback != 0 && cfg->cuda_core_fallback != 1) || cfg->reserved != 0 ||
       (cfg->act_dtype != TTT_F32 && cfg->act_dtype != TTT_BF16))
     return create_fail(TTT_ERR_ARG, "a ttt_config field is out of range");
-  if (cfg->hd % 4 != 0 || cfg->hidden % 4 != 0 || cfg->hd > 128)
-    return create_fail(TTT_ERR_SHAPE, "hd = %lld, hidden = %lld: both must be multiples of 4 and hd <= 128",
+  if (cfg->hd % 4 != 0 || cfg->hidden % 4 != 0 || (cfg->hd > 128 && !bf16_large_supported(cfg)))
+    return create_fail(TTT_ERR_SHAPE, "hd = %lld, hidden = %lld: both must be multiples of 4 and hd <= 128 (bf16 "
+                       "without Newton-Schulz / renorm also: hd a multiple of 256 up to 2048, hidden a multiple of 128)",
                        cfg->hd, cfg->hidden);
   if (cfg->linear_fast_weight && cfg->hidden != cfg->hd)
     return create_fail(TTT_ERR_SHAPE, "linear test mode needs hidden == hd");
@@ -184,6 +194,7 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
   ctx->mat_elems = (size_t)cfg->nh * cfg->hidden * cfg->hd;
   const size_t set = 3 * ctx->mat_elems;
   const bool is_bf16 = cfg->act_dtype == TTT_BF16;
+  ctx->large = bf16_large_supported(cfg) != 0;
   ctx->upd_via_f32 = is_bf16 && !bf16_update_tensor_path(cfg);
   ctx->app_via_f32 = is_bf16 && !bf16_apply_tensor_path(cfg);
   const bool bf16 = is_bf16 && !ctx->upd_via_f32;          // update on the tensor cores
@@ -193,6 +204,7 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
                                 : f32_partials_needed(ctx, cfg->max_tokens));
   if (ctx->cap_partials < 4) ctx->cap_partials = 4;
   ctx->cap_loss_rows = ctx->cap_partials * ((cfg->hidden + 127) / 128);
+  if (ctx->large) ctx->cap_loss_rows = (int)bf16_large_loss_rows(cfg);
   const int nblk = (cfg->hidden + 15) / 16 + 160;   // commit row blocks, or (slices x splits) of the fused commit
 
   bool ok = true;
@@ -201,13 +213,16 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
   };
   alloc((void**)&ctx->Wm, set * sizeof(float));
   alloc((void**)&ctx->Wb, set * sizeof(ttt_wop_t));
-  if (is_bf16 && bf16_apply_wide_supported(cfg)) alloc((void**)&ctx->Wq, set * sizeof(__nv_bfloat16));
+  if (is_bf16 && (bf16_apply_wide_supported(cfg) || ctx->large)) alloc((void**)&ctx->Wq, set * sizeof(__nv_bfloat16));
+  if (ctx->large)
+    for (int i = 0; i < 3; ++i)
+      alloc((void**)&ctx->lact[i], (size_t)cfg->max_tokens * cfg->nh * cfg->hidden * sizeof(__nv_bfloat16));
   alloc((void**)&ctx->n0, ((size_t)2 * cfg->nh * cfg->hidden + (size_t)cfg->nh * cfg->hd) * sizeof(float));
   alloc((void**)&ctx->colsq, (size_t)cfg->nh * nblk * cfg->hd * sizeof(float));
   alloc((void**)&ctx->G, set * sizeof(float));
-  alloc((void**)&ctx->partials, (size_t)ctx->cap_partials * set * sizeof(float));
+  alloc((void**)&ctx->partials, (ctx->large ? (size_t)4 : (size_t)ctx->cap_partials * set) * sizeof(float));
   alloc((void**)&ctx->loss_part, (size_t)ctx->cap_loss_rows * cfg->nh * sizeof(float));
-  if (bf16) {
+  if (bf16 && !ctx->large) {
     const size_t nctr = (size_t)cfg->nh * ((cfg->hidden + 127) / 128);
     alloc((void**)&ctx->sync_ctr, nctr * sizeof(unsigned));
     if (ok && cudaMemset(ctx->sync_ctr, 0, nctr * sizeof(unsigned)) != cudaSuccess) ok = false;
@@ -255,7 +270,7 @@ void ttt_destroy(ttt_ctx* ctx) {
   if (!ctx) return;
   DeviceGuard dg(ctx);
   cudaDeviceSynchronize();
-  cudaFree(ctx->Wm); cudaFree(ctx->Wb); cudaFree(ctx->Wq); cudaFree(ctx->n0); cudaFree(ctx->colsq);
+  cudaFree(ctx->Wm); cudaFree(ctx->Wb); cudaFree(ctx->Wq); cudaFree(ctx->lact[0]); cudaFree(ctx->lact[1]); cudaFree(ctx->lact[2]); cudaFree(ctx->n0); cudaFree(ctx->colsq);
   cudaFree(ctx->G); cudaFree(ctx->partials); cudaFree(ctx->loss_part); cudaFree(ctx->loss_blk); cudaFree(ctx->sync_ctr); cudaFree(ctx->ns_scratch); cudaFree(ctx->stage[0]); cudaFree(ctx->stage[1]);
   for (int i = 0; i < 3; ++i) cudaFree(ctx->act[i]);
   delete ctx;

@@ -70,6 +70,11 @@ struct ttt_ctx {
   bool upd_via_f32, app_via_f32;   // per call family: update (accumulate) / apply
   float* stage[2];
 
+  // large-dimension path (hd >= 256, bf16_large.cu): hidden activations dA | dB | Hd' (update) and Hq
+  // (apply, lact[0]) as bf16 [max_tokens][nh * hidden]; the pending gradient is the dense G only
+  bool large;
+  __nv_bfloat16* lact[3];
+
   // bf16 path: group-barrier counters of the fused commit ([nh][hidden/128]) and their running target
   // hd = 128 Newton-Schulz: partial Gram matrices [3 nh][hidden/128][2][128 x 128] fp32
   float* ns_scratch;
@@ -87,7 +92,8 @@ struct ttt_ctx {
   int max_pairs;               // hd = 128 apply: co-resident CTA pairs (0 = not queried yet, < 0 = none)
   int upd_coop_ctas;           // hd = 64 update: co-resident CTAs of the cooperative launch (0 = not queried)
 };
-enum { ATTR_UPD = 1, ATTR_UPD_LOSS = 2, ATTR_UPDW = 4, ATTR_APPW = 8, ATTR_NSW = 16, ATTR_NS_F32 = 32 };
+enum { ATTR_UPD = 1, ATTR_UPD_LOSS = 2, ATTR_UPDW = 4, ATTR_APPW = 8, ATTR_NSW = 16, ATTR_NS_F32 = 32,
+       ATTR_LARGE = 64 };
 
 namespace ttt {
 
@@ -144,6 +150,13 @@ int bf16_accumulate_wide(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat
                          int64_t M, int64_t ld, bool want_loss, int* used, int* loss_rows,
                          cudaStream_t s);
 int bf16_wide_partials_needed(const ttt_ctx* ctx, int64_t M);
+// large-dimension path (bf16_large.cu): hd a multiple of 256, plain update
+int bf16_large_supported(const ttt_config* cfg);
+int64_t bf16_large_loss_rows(const ttt_config* cfg);
+int bf16_large_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat16* V, const float* lr,
+                          int64_t M, int64_t ld, bool want_loss, int* loss_rows, cudaStream_t s);
+int bf16_large_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int64_t M, int64_t ld,
+                     cudaStream_t s);
 // strided bf16 [M][cols] (row stride ld) <-> dense fp32 [M][cols]
 int launch_bf16_to_f32(ttt_ctx* ctx, const __nv_bfloat16* src, int64_t ld, float* dst, int64_t M, cudaStream_t s);
 int launch_f32_to_bf16(ttt_ctx* ctx, const float* src, __nv_bfloat16* dst, int64_t ld, int64_t M, cudaStream_t s);

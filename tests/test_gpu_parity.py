@@ -505,6 +505,58 @@ def test_bf16_fused_commit_renorm_when_warps_straddle_the_commit_ranges(nh):
 
 
 # ------------------------------------------------------------------------------------------------
+# large head dimensions: the shape the paper ships (nh = 1, hd = d = 1024, k in {1, 2, 4};
+# Table 3) on the four-GEMM path of bf16_large.cu, cut-down token counts (the float64 oracle
+# runs one head on one core). Plain Eq. 8 update as the paper defines it; small lr, K L2-normalised:
+# the literal recurrence is explosive at these sizes.
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nh,hd,H,M,chunks", [
+    (2, 256, 384, 333, 3),        # generic indexing: two heads, three hidden slices, ragged token tiles
+    (1, 1024, 1024, 600, 2),      # paper shape, k = 1 (state size 1M)
+    (1, 1024, 4096, 300, 1),      # paper shape, k = 4 (state size 4M)
+])
+def test_bf16_large_head_dimension_parity(nh, hd, H, M, chunks):
+    w = ti.scaled(ti.CONFIGS["cfg2"], nh=nh, hd=hd, hidden=H, tokens_per_frame=M, frames_per_chunk=1,
+                  n_frames=chunks, lr=0.002, rho=0.5)
+    gpu = _mk(w)
+    assert gpu.kernel_path() == (True, True)
+    gpu.close()
+    errs_o, errs_w, errs_l = _run_stream(w)
+    assert max(errs_o) <= TOL_BF16, errs_o
+    assert max(errs_w) <= TOL_BF16, errs_w
+    assert max(errs_l) <= TOL_LOSS_BF16, errs_l
+
+
+def test_bf16_large_accumulate_commit_and_rejected_options():
+    """Eq. 10 on the large-dimension path (two accumulates at the same W, one commit == the oracle's summed
+    gradient step) and the options the path does not offer (Newton-Schulz, renorm: TTT_ERR_SHAPE)."""
+    from paper_2604_08542_b200 import TTT, TTT_BF16, TTTError
+    dev = torch.device("cuda", 0)
+    for kw in (dict(ns_iters=5), dict(renorm=1)):
+        with pytest.raises(TTTError) as e:
+            TTT(1, 1024, 1024, TTT_BF16, max_tokens=256, **kw)
+        assert e.value.status == -2
+    w = ti.scaled(ti.CONFIGS["cfg2"], nh=1, hd=512, hidden=512, tokens_per_frame=200, frames_per_chunk=1,
+                  n_frames=2, lr=0.002)
+    W1, W2, W3 = ti.fast_weights(w)
+    (Q0, K0, V0, l0), (Q1, K1, V1, l1) = list(ti.TokenStream(w))
+    a = _mk(w)
+    a.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    a.ttt_accumulate(K0.to(dev), V0.to(dev), l0.to(dev))
+    a.ttt_accumulate(K1.to(dev), V1.to(dev), l1.to(dev))
+    G = a.ttt_pending_gradient().cpu()                         # [3, nh, H, hd]
+    ora = OracleTTT(W1, W2, W3)
+    g = [sum(t) for t in zip(*(ora.grad(K, V, l)[:3] for K, V, l in ((K0, V0, l0), (K1, V1, l1))))]
+    assert rel_err(G[0].transpose(1, 2), g[0]) <= 1e-2
+    assert rel_err(G[1], g[1]) <= 1e-2
+    assert rel_err(G[2].transpose(1, 2), g[2]) <= 1e-2
+    a.ttt_commit()
+    expect = [W1.double().numpy() - g[0], W2.double().numpy() - g[1], W3.double().numpy() - g[2]]
+    assert worst_head_weights([x.cpu() for x in a.ttt_get_weights()], expect) <= TOL_BF16
+    a.close()
+
+
+# ------------------------------------------------------------------------------------------------
 # north_star's bar "after the FINAL chunk", at full size: the whole 63-chunk cfg4 stream and the whole
 # 32-chunk cfg5 stream through the CUDA path (all heads, the launch configuration bench.py times) and
 # through the float64 oracle (two heads each; heads are independent, so this is exact per head; the
