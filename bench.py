@@ -4,14 +4,15 @@
 Metric (BASELINE.json:metric): "TTT update+apply tokens/s on 1 B200; % of dense-BF16 tensor peak".
 A step = one `ttt_chunk_step` (update Eq. 8 then apply Eq. 4, all heads) over one chunk of the
 workload. The metric names no config, so the default run times ALL FOUR performance configs of
-BASELINE.json (cfg2 .. cfg5) in one process: the top-level `value` / `ms_per_step` /
-`config.workload` are those of cfg5, the largest single-GPU configuration, and `workloads` carries
-the same numbers (with their own `roofline`) for every config. Every step is a new chunk of a
+BASELINE.json (cfg2 .. cfg5) in one process, plus the paper's own shape (paper_k4: one head of 1024,
+hidden 4096, 82 440-token chunks): the top-level `value` / `ms_per_step` /
+`config.workload` are those of cfg5, the largest single-GPU configuration of BASELINE.json, and
+`workloads` carries the same numbers (with their own `roofline`) for every workload. Every step is a new chunk of a
 sequence: the fast weights are reset with `ttt_init` between steps (outside the per-step CUDA
 events, inside the outer bracket), inputs rotate over distinct resident sets larger than 2x L2.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg3|cfg4|cfg5|all]
-                  [--impl reference]
+                  [--impl reference]          (also --workload paper_k4 | paper_k1)
 
 N > 1: launched by torchrun (RANK / LOCAL_RANK / WORLD_SIZE in the environment) every rank runs its
 own independent sequences (weak scaling, no collective on the data path — heads and sequences are
@@ -37,7 +38,7 @@ sys.path.insert(0, ROOT)
 import ttt_inputs as ti  # noqa: E402
 
 L2_BYTES = 126 * 2 ** 20
-PERF_WORKLOADS = ("cfg2", "cfg3", "cfg4", "cfg5")
+PERF_WORKLOADS = ("cfg2", "cfg3", "cfg4", "cfg5", "paper_k4")   # BASELINE.json's four + the paper's own shape
 HEADLINE = "cfg5"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the workload's dominant kernel, from the
@@ -163,7 +164,7 @@ def config_of(w: ti.TTTWorkload, world: int) -> dict:
 # --------------------------------------------------------------------------------------------
 # tokens of one chunk an oracle step works on (all heads, OpenMP over heads): sized so that a step
 # takes a few seconds on the box's cores; cfg5's full chunk would take ~13 s
-REF_TOKENS = {"cfg2": 10992, "cfg3": 10992, "cfg4": 16384, "cfg5": 8192}
+REF_TOKENS = {"cfg2": 10992, "cfg3": 10992, "cfg4": 16384, "cfg5": 8192, "paper_k4": 384, "paper_k1": 1024}
 
 
 def _oracle_sample(w: ti.TTTWorkload):
@@ -302,7 +303,8 @@ def measure(args, w, rank, local_rank, world, clocks, peaks, want_e2e):
     upd_tflops = upd_flops / (k_ms[0] * 1e-3) / 1e12
     app_tflops = flops_per_chunk(w, M, "apply") / (k_ms[2] * 1e-3) / 1e12
     step_tflops = flops_per_chunk(w, M, "step") / (ms_per_step * 1e-3) / 1e12
-    upd_kernel = ("bf16_update_wide_kernel" if w.hd == 128 else "bf16_update_kernel") \
+    upd_kernel = ("ld_forward_kernel + ld_mn_gemm_kernel (gradient)" if w.hd > 128 else
+                  "bf16_update_wide_kernel" if w.hd == 128 else "bf16_update_kernel") \
         if w.act_dtype == "bf16" else "f32 path"
     tr = TRAFFIC.get(w.name)
     roofline = {"kernel": upd_kernel, "bound": "tensor", "achieved": upd_tflops,
