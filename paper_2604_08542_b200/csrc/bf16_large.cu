@@ -35,10 +35,14 @@ constexpr int KC = 64;             // contraction chunk (one 128-byte swizzled r
 constexpr int THREADS = 384;       // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warp 3 idle, warps 4-11 epilogue
 constexpr int EPI_WARPS = 8;
 constexpr int BOX = TM * 128;      // bytes of a [128 rows x 64] bf16 box (16 KB); a [64 x 64] box is BOX / 2
-// forward kernels: stage = token chunk(s) + weight-row chunks
-constexpr int F_STAGE_U = 5 * BOX, F_STAGES_U = 2;     // K, [W1 | W3], V, W2
-constexpr int F_STAGE_A = 3 * BOX, F_STAGES_A = 4;     // Q, [W1 | W3]
-constexpr uint32_t C_XB = 0, C_G = 256;                // x | b [128 x 256] fp32, g0 [128 x 128] fp32
+// forward kernels: stage = token chunk + weight-row chunks, 48 KB: [K or Q | W1 | W3] for x | b, or
+// [V | W2 | -] for g0. The update runs the two contractions one after the other through the SAME ring
+// (a stage holding all five boxes is 80 KB: only two fit, and the TMA round trip was exposed on every
+// chunk — 28 K clk per item against 18 K of MMA work)
+// plus the epilogue's TMA-store staging tiles (three for the update, one for the apply)
+constexpr int F_STAGE = 3 * BOX, F_STAGES_U = 3, F_STAGES_A = 4;
+constexpr int F_SMEM_U = F_STAGES_U * F_STAGE + 3 * BOX + 1024, F_SMEM_A = F_STAGES_A * F_STAGE + BOX + 1024;
+constexpr uint32_t C_XB = 0, C_G = 256;                // x | b [128 x 256] fp32; g0 [128 x 128] fp32, two buffers
 // MN-major-B kernels: stage = A 16 KB + B 32 KB, two accumulators [128 x 256] fp32
 constexpr int M_STAGE = 3 * BOX, M_STAGES = 4;
 constexpr int TN = 256;
@@ -51,17 +55,18 @@ constexpr int TN = 256;
 template <bool UPD, bool LOSS>
 __global__ void __launch_bounds__(lg::THREADS, 1)
 ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapV,
-                  const __grid_constant__ CUtensorMap mapW, const float* __restrict__ lr,
-                  __nv_bfloat16* __restrict__ act0, __nv_bfloat16* __restrict__ act1,
-                  __nv_bfloat16* __restrict__ act2, float* __restrict__ loss_part, int M, int nh, int hd,
+                  const __grid_constant__ CUtensorMap mapW, const __grid_constant__ CUtensorMap mapO0,
+                  const __grid_constant__ CUtensorMap mapO1, const __grid_constant__ CUtensorMap mapO2,
+                  const float* __restrict__ lr, float* __restrict__ loss_part, int M, int nh, int hd,
                   int H, int n_items) {
   using namespace lg;
-  constexpr int STAGE = UPD ? F_STAGE_U : F_STAGE_A;
+  constexpr int STAGE = F_STAGE;
   constexpr int STAGES = UPD ? F_STAGES_U : F_STAGES_A;
+  // TMEM: update x | b (256 columns) + two g0 buffers (2 x 128); apply two x | b buffers
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
-  __shared__ uint64_t full[STAGES], empty[STAGES], acc_full, acc_empty;
+  __shared__ uint64_t full[STAGES], empty[STAGES], acc_full[2], acc_empty[2];
   __shared__ uint32_t tmem_base_s;
   __shared__ float loss_red[EPI_WARPS];
 
@@ -69,11 +74,11 @@ ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constan
   const int nslices = H / TM, ntt = (M + TM - 1) / TM, nkc = hd / KC;
   if (tid == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
-    mbar_init(&acc_full, 1);
-    mbar_init(&acc_empty, EPI_WARPS);
+    for (int b = 0; b < 2; ++b) { mbar_init(&acc_full[b], 1); mbar_init(&acc_empty[b], EPI_WARPS); }
     fence_mbar_init();
     tma_prefetch_desc(&mapX);
     tma_prefetch_desc(&mapW);
+    tma_prefetch_desc(&mapO0);
     if (UPD) tma_prefetch_desc(&mapV);
   }
   if (warp == 2) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
@@ -98,17 +103,20 @@ ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constan
       for (int id = blockIdx.x; id < n_items; id += gridDim.x) {
         int h, tt, s;
         item(id, h, tt, s);
-        for (int kc = 0; kc < nkc; ++kc, ++g) {
+        for (int kc = 0; kc < (UPD ? 2 : 1) * nkc; ++kc, ++g) {
           const int st = g % STAGES;
           if (g >= STAGES) mbar_wait(&empty[st], ((g / STAGES) - 1) & 1);
-          mbar_arrive_expect_tx(&full[st], STAGE);
           uint8_t* dst = smem + st * STAGE;
-          tma_load_2d(dst, &mapX, &full[st], h * hd + kc * KC, tt * TM);                               // K or Q chunk
-          tma_load_2d(dst + BOX, &mapW, &full[st], kc * KC, (0 * nh + h) * H + s * TM);               // W1^T rows
-          tma_load_2d(dst + 2 * BOX, &mapW, &full[st], kc * KC, (2 * nh + h) * H + s * TM);           // W3^T rows
-          if (UPD) {
-            tma_load_2d(dst + 3 * BOX, &mapV, &full[st], h * hd + kc * KC, tt * TM);                  // V chunk
-            tma_load_2d(dst + 4 * BOX, &mapW, &full[st], kc * KC, (1 * nh + h) * H + s * TM);         // W2 rows
+          if (UPD && kc < nkc) {                         // update, first pass: g0 = V W2^T
+            mbar_arrive_expect_tx(&full[st], 2 * BOX);
+            tma_load_2d(dst, &mapV, &full[st], h * hd + kc * KC, tt * TM);                            // V chunk
+            tma_load_2d(dst + BOX, &mapW, &full[st], kc * KC, (1 * nh + h) * H + s * TM);             // W2 rows
+          } else {                                       // x | b = (K or Q) [W1 | W3]
+            const int k2 = UPD ? kc - nkc : kc;
+            mbar_arrive_expect_tx(&full[st], 3 * BOX);
+            tma_load_2d(dst, &mapX, &full[st], h * hd + k2 * KC, tt * TM);                             // K or Q chunk
+            tma_load_2d(dst + BOX, &mapW, &full[st], k2 * KC, (0 * nh + h) * H + s * TM);             // W1^T rows
+            tma_load_2d(dst + 2 * BOX, &mapW, &full[st], k2 * KC, (2 * nh + h) * H + s * TM);         // W3^T rows
           }
         }
       }
@@ -121,99 +129,142 @@ ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constan
       const uint64_t d0 = umma_smem_desc_sw128(sbase, 16, 1024);
       int g = 0, n = 0;
       for (int id = blockIdx.x; id < n_items; id += gridDim.x, ++n) {
-        if (n > 0) { mbar_wait(&acc_empty, (n - 1) & 1); tc_fence_after(); }   // epilogue has read the accumulators
-        for (int kc = 0; kc < nkc; ++kc, ++g) {
+        // update: g0 first, into the g buffer of this item's parity (its last reader, the epilogue of item
+        // n - 2, finished before the x | b pass of item n - 1 began), then x | b once the epilogue of item
+        // n - 1 has read the previous x | b: that epilogue runs under this item's g0 pass.
+        // apply: x | b double-buffered, the epilogue of item n - 2 must have read buffer n & 1.
+        const int ab = UPD ? 0 : (n & 1);
+        const uint32_t cxb = tb + C_XB + ab * 256, cg = tb + C_G + (n & 1) * 128;
+        if (!UPD && n >= 2) { mbar_wait(&acc_empty[ab], ((n >> 1) - 1) & 1); tc_fence_after(); }
+        for (int kc = 0; kc < (UPD ? 2 : 1) * nkc; ++kc, ++g) {
           const int st = g % STAGES;
+          if (UPD && kc == nkc && n > 0) { mbar_wait(&acc_empty[0], (n - 1) & 1); tc_fence_after(); }
           mbar_wait(&full[st], (g / STAGES) & 1);
           tc_fence_after();
           const uint64_t ds = d0 + (uint64_t)(st * (STAGE >> 4));
+          if (UPD && kc < nkc) {
 #pragma unroll
-          for (int k = 0; k < KC / 16; ++k) {
-            umma_ss(tb + C_XB, ds + 2 * k, ds + (BOX >> 4) + 2 * k, idesc_xb, (kc > 0) | k);
-            if (UPD) umma_ss(tb + C_G, ds + 3 * (BOX >> 4) + 2 * k, ds + 4 * (BOX >> 4) + 2 * k, idesc_g, (kc > 0) | k);
+            for (int k = 0; k < KC / 16; ++k)
+              umma_ss(cg, ds + 2 * k, ds + (BOX >> 4) + 2 * k, idesc_g, (kc > 0) | k);
+          } else {
+#pragma unroll
+            for (int k = 0; k < KC / 16; ++k)
+              umma_ss(cxb, ds + 2 * k, ds + (BOX >> 4) + 2 * k, idesc_xb, (kc > (UPD ? nkc : 0)) | k);
           }
           tc_commit(&empty[st]);
         }
-        tc_commit(&acc_full);
+        tc_commit(&acc_full[ab]);
       }
     }
   } else if (warp >= 4) {
-    // ===================== epilogue: thread = token row (TMEM lane), 8 groups of 16 hidden columns =====================
+    // ===================== epilogue: thread = token row (TMEM lane) =====================
+    // The 128 hidden columns of the tile go out in two phases of 64 (one 128-byte row of bf16 per token):
+    // all eight warps work on a phase (32 rows x 32 columns each), write their operands into swizzled
+    // staging tiles [128 rows x 128 B] and one thread hands those to the TMA (a row-per-lane global store
+    // touches 32 sectors per instruction and kept the LSU busy for ~6 K clk per tile).
     const int q = warp & 3, half = (warp - 4) >> 2;
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
     const uint64_t HALF2 = pack2(0.5f, 0.5f), ONE2 = pack2(1.0f, 1.0f), NONE2 = pack2(-1.0f, -1.0f);
+    const int r = q * 32 + lane;                                  // row within the tile
+    uint8_t* stg = smem + STAGES * STAGE;                         // NOPS staging tiles of BOX bytes
+    const bool leader = tid == 4 * 32;
     int n = 0;
     for (int id = blockIdx.x; id < n_items; id += gridDim.x, ++n) {
       int h, tt, s;
       item(id, h, tt, s);
-      const int tok = tt * TM + q * 32 + lane;
+      const int ab = UPD ? 0 : (n & 1);
+      const int tok = tt * TM + r;
       float nef = 0.f;
       if (UPD && tok < M) nef = -__ldg(lr + (size_t)h * M + tok);
       const uint64_t ne = pack2(nef, nef);
       uint64_t loss2 = 0ull;
-      mbar_wait(&acc_full, n & 1);
+      mbar_wait(&acc_full[ab], (UPD ? n : (n >> 1)) & 1);
       tc_fence_after();
-      const size_t row_off = (size_t)tok * ((size_t)nh * H) + (size_t)h * H + (size_t)s * TM;
+      const uint32_t cxb = tb + lane_base + C_XB + ab * 256, cg = tb + lane_base + C_G + (n & 1) * 128;
 #pragma unroll 1
-      for (int c = 4 * half; c < 4 * half + 4; ++c) {
-        uint32_t rx[16], rb[16], rg[16];
-        tmem_ld_x16(tb + lane_base + C_XB + 16 * c, rx);
-        tmem_ld_x16(tb + lane_base + C_XB + 128 + 16 * c, rb);
-        if (UPD) tmem_ld_x16(tb + lane_base + C_G + 16 * c, rg);
-        tc_wait_ld();
-        uint32_t pa[8], pb[8], ph[8];
+      for (int p = 0; p < 2; ++p) {
+        // the staging tiles were handed to the TMA one phase ago: wait until it has read them
+        if (leader) tma_store_wait_read<0>();
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+#pragma unroll 1
+        for (int gi = 0; gi < 2; ++gi) {
+          const int cl = 2 * half + gi;                           // 16-column group within the phase's 64
+          const int c = 4 * p + cl;                               // ... within the tile's 128
+          uint32_t rx[16], rb[16], rg[16];
+          tmem_ld_x16(cxb + 16 * c, rx);
+          tmem_ld_x16(cxb + 128 + 16 * c, rb);
+          if (UPD) tmem_ld_x16(cg + 16 * c, rg);
+          tc_wait_ld();
+          if (p == 1 && gi == 1) {                                // last TMEM read of this tile: release it
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&acc_empty[ab]);
+          }
+          uint32_t pa[8], pb[8], ph[8];
 #pragma unroll
-        for (int e = 0; e < 16; e += 2) {
-          const uint64_t x = fmul2(pack2u(rx[e], rx[e + 1]), HALF2);            // a / 2
-          const uint64_t bb = pack2u(rb[e], rb[e + 1]);
-          float x0, x1;
-          unpack2(x, x0, x1);
-          const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
-          const uint64_t S = ffma2(x, th, x);                                   // SiLU(a) = a sigmoid(a)
-          const uint64_t hdv = fmul2(S, bb);                                    // Hd (update) / Hq (apply)
-          if (UPD) {
-            const uint64_t g = fmul2(ne, pack2u(rg[e], rg[e + 1]));             // dHd = (-eta v) W2^T
-            const uint64_t p = fadd2(th, ONE2);                                 // 2 sigmoid(a)
-            const uint64_t m = ffma2(th, NONE2, ONE2);                          // 2 (1 - sigmoid(a))
-            const uint64_t t1 = fmul2(ffma2(S, m, p), HALF2);                   // SiLU'(a)
-            pa[e >> 1] = pack_bf16x2_from2(fmul2(fmul2(g, bb), t1));            // dA
-            pb[e >> 1] = pack_bf16x2_from2(fmul2(g, S));                        // dB
-            ph[e >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));                     // Hd' = -eta Hd
-            if (LOSS) loss2 = ffma2(hdv, g, loss2);
-          } else {
-            ph[e >> 1] = pack_bf16x2_from2(hdv);
+          for (int e = 0; e < 16; e += 2) {
+            const uint64_t x = fmul2(pack2u(rx[e], rx[e + 1]), HALF2);            // a / 2
+            const uint64_t bb = pack2u(rb[e], rb[e + 1]);
+            float x0, x1;
+            unpack2(x, x0, x1);
+            const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
+            const uint64_t S = ffma2(x, th, x);                                   // SiLU(a) = a sigmoid(a)
+            const uint64_t hdv = fmul2(S, bb);                                    // Hd (update) / Hq (apply)
+            if (UPD) {
+              const uint64_t g = fmul2(ne, pack2u(rg[e], rg[e + 1]));             // dHd = (-eta v) W2^T
+              const uint64_t pp = fadd2(th, ONE2);                                // 2 sigmoid(a)
+              const uint64_t m = ffma2(th, NONE2, ONE2);                          // 2 (1 - sigmoid(a))
+              const uint64_t t1 = fmul2(ffma2(S, m, pp), HALF2);                  // SiLU'(a)
+              pa[e >> 1] = pack_bf16x2_from2(fmul2(fmul2(g, bb), t1));            // dA
+              pb[e >> 1] = pack_bf16x2_from2(fmul2(g, S));                        // dB
+              ph[e >> 1] = pack_bf16x2_from2(fmul2(ne, hdv));                     // Hd' = -eta Hd
+              if (LOSS) loss2 = ffma2(hdv, g, loss2);
+            } else {
+              ph[e >> 1] = pack_bf16x2_from2(hdv);
+            }
           }
+          // 16 columns = two 16-byte chunks of the row; 128-byte swizzle: chunk ^= row & 7
+          const uint32_t o0 = r * 128 + (((2 * cl) ^ (r & 7)) << 4), o1 = r * 128 + (((2 * cl + 1) ^ (r & 7)) << 4);
+          if (UPD) {
+            *reinterpret_cast<uint4*>(stg + o0) = make_uint4(pa[0], pa[1], pa[2], pa[3]);
+            *reinterpret_cast<uint4*>(stg + o1) = make_uint4(pa[4], pa[5], pa[6], pa[7]);
+            *reinterpret_cast<uint4*>(stg + BOX + o0) = make_uint4(pb[0], pb[1], pb[2], pb[3]);
+            *reinterpret_cast<uint4*>(stg + BOX + o1) = make_uint4(pb[4], pb[5], pb[6], pb[7]);
+          }
+          uint8_t* sh = stg + (UPD ? 2 * BOX : 0);
+          *reinterpret_cast<uint4*>(sh + o0) = make_uint4(ph[0], ph[1], ph[2], ph[3]);
+          *reinterpret_cast<uint4*>(sh + o1) = make_uint4(ph[4], ph[5], ph[6], ph[7]);
         }
-        if (tok < M) {
+        fence_proxy_async_smem();
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        if (leader) {                                             // rows beyond M are clipped by the tensor map
+          const int col = h * H + s * TM + 64 * p, row = tt * TM;
           if (UPD) {
-            uint4* d0p = reinterpret_cast<uint4*>(act0 + row_off + 16 * c);
-            uint4* d1p = reinterpret_cast<uint4*>(act1 + row_off + 16 * c);
-            d0p[0] = make_uint4(pa[0], pa[1], pa[2], pa[3]); d0p[1] = make_uint4(pa[4], pa[5], pa[6], pa[7]);
-            d1p[0] = make_uint4(pb[0], pb[1], pb[2], pb[3]); d1p[1] = make_uint4(pb[4], pb[5], pb[6], pb[7]);
+            tma_store_2d(&mapO0, stg, col, row);
+            tma_store_2d(&mapO1, stg + BOX, col, row);
+            tma_store_2d(&mapO2, stg + 2 * BOX, col, row);
+          } else {
+            tma_store_2d(&mapO0, stg, col, row);
           }
-          uint4* d2p = reinterpret_cast<uint4*>((UPD ? act2 : act0) + row_off + 16 * c);
-          d2p[0] = make_uint4(ph[0], ph[1], ph[2], ph[3]); d2p[1] = make_uint4(ph[4], ph[5], ph[6], ph[7]);
+          tma_store_commit();
         }
       }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&acc_empty);
       if (UPD && LOSS) {
         float l0, l1;
         unpack2(loss2, l0, l1);
         float loss = l0 + l1;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) loss += __shfl_xor_sync(0xffffffffu, loss, o);
-        asm volatile("bar.sync 1, 256;" ::: "memory");       // loss_red of the previous item has been read
-        if (lane == 0) loss_red[warp - 4] = loss;
+        if (lane == 0) loss_red[warp - 4] = loss;                // (read two barriers ago at the latest)
         asm volatile("bar.sync 1, 256;" ::: "memory");
-        if (warp == 4 && lane == 0) {
+        if (leader) {
           float t = 0.f;
           for (int w = 0; w < EPI_WARPS; ++w) t += loss_red[w];
           loss_part[(size_t)(tt * nslices + s) * nh + h] = t;
         }
       }
     }
+    if (leader) tma_store_wait<0>();                              // the activations are complete in global memory
   }
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   tc_fence_before();
@@ -403,7 +454,7 @@ static int launch_pdl(ttt_ctx* ctx, const char* what, Kern kern, int grid, size_
 
 static int large_attrs(ttt_ctx* ctx) {
   if (ctx->attr_done & ATTR_LARGE) return TTT_OK;
-  const int su = lg::F_STAGE_U * lg::F_STAGES_U + 1024, sa = lg::F_STAGE_A * lg::F_STAGES_A + 1024;
+  const int su = lg::F_SMEM_U, sa = lg::F_SMEM_A;
   const int sm = lg::M_STAGE * lg::M_STAGES + 1024;
   TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, su), "ld_forward smem attr");
   TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, su), "ld_forward smem attr");
@@ -428,19 +479,23 @@ int bf16_large_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloa
   if ((rc = make_token_map(ctx, &mA0, ctx->lact[0], M, HW, HW, 64)) != TTT_OK) return rc;
   if ((rc = make_token_map(ctx, &mA1, ctx->lact[1], M, HW, HW, 64)) != TTT_OK) return rc;
   if ((rc = make_token_map(ctx, &mA2, ctx->lact[2], M, HW, HW, 64)) != TTT_OK) return rc;
+  CUtensorMap mS0, mS1, mS2;                      // the forward kernel's TMA stores: boxes of [128 tokens][64]
+  if ((rc = make_token_map(ctx, &mS0, ctx->lact[0], M, HW, HW, lg::TM)) != TTT_OK) return rc;
+  if ((rc = make_token_map(ctx, &mS1, ctx->lact[1], M, HW, HW, lg::TM)) != TTT_OK) return rc;
+  if ((rc = make_token_map(ctx, &mS2, ctx->lact[2], M, HW, HW, lg::TM)) != TTT_OK) return rc;
   if ((rc = make_token_map(ctx, &mK64, K, M, (int64_t)c.nh * c.hd, ld, 64)) != TTT_OK) return rc;
   if ((rc = make_token_map(ctx, &mV64, V, M, (int64_t)c.nh * c.hd, ld, 64)) != TTT_OK) return rc;
   const int ntt = (int)((M + lg::TM - 1) / lg::TM), nsl = c.hidden / lg::TM;
   int n_items = c.nh * ntt * nsl;
   int grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
-  const size_t su = (size_t)lg::F_STAGE_U * lg::F_STAGES_U + 1024;
+  const size_t su = (size_t)lg::F_SMEM_U;
   int Mi = (int)M, nh = c.nh, hd = c.hd, H = c.hidden;
   if (want_loss)
-    rc = launch_pdl(ctx, "ld_forward_kernel (update)", ld_forward_kernel<true, true>, grid, su, s, mK, mV, mW, lr,
-                    ctx->lact[0], ctx->lact[1], ctx->lact[2], ctx->loss_part, Mi, nh, hd, H, n_items);
+    rc = launch_pdl(ctx, "ld_forward_kernel (update)", ld_forward_kernel<true, true>, grid, su, s, mK, mV, mW,
+                    mS0, mS1, mS2, lr, ctx->loss_part, Mi, nh, hd, H, n_items);
   else
-    rc = launch_pdl(ctx, "ld_forward_kernel (update)", ld_forward_kernel<true, false>, grid, su, s, mK, mV, mW, lr,
-                    ctx->lact[0], ctx->lact[1], ctx->lact[2], ctx->loss_part, Mi, nh, hd, H, n_items);
+    rc = launch_pdl(ctx, "ld_forward_kernel (update)", ld_forward_kernel<true, false>, grid, su, s, mK, mV, mW,
+                    mS0, mS1, mS2, lr, ctx->loss_part, Mi, nh, hd, H, n_items);
   if (rc != TTT_OK) return rc;
   *loss_rows = ntt * nsl;
   n_items = 3 * c.nh * nsl * (c.hd / lg::TN);
@@ -470,13 +525,12 @@ int bf16_large_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int
   const int ntt = (int)((M + lg::TM - 1) / lg::TM), nsl = c.hidden / lg::TM;
   int n_items = c.nh * ntt * nsl;
   int grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
-  const size_t sa = (size_t)lg::F_STAGE_A * lg::F_STAGES_A + 1024;
+  const size_t sa = (size_t)lg::F_SMEM_A;
   int Mi = (int)M, nh = c.nh, hd = c.hd, H = c.hidden;
   const float* nolr = nullptr;
-  __nv_bfloat16* nob = nullptr;
   float* nof = nullptr;
-  rc = launch_pdl(ctx, "ld_forward_kernel (apply)", ld_forward_kernel<false, false>, grid, sa, s, mQ, mQ, mW, nolr,
-                  ctx->lact[0], nob, nob, nof, Mi, nh, hd, H, n_items);
+  rc = launch_pdl(ctx, "ld_forward_kernel (apply)", ld_forward_kernel<false, false>, grid, sa, s, mQ, mQ, mW,
+                  mHq, mHq, mHq, nolr, nof, Mi, nh, hd, H, n_items);
   if (rc != TTT_OK) return rc;
   n_items = c.nh * ntt * (c.hd / lg::TN);
   grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
