@@ -19,14 +19,6 @@
 #include "tc_common.cuh"
 #include "ttt_internal.h"
 
-#ifdef TTT_TRACE
-__device__ long long g_app_trace[16];
-extern "C" int ttt_debug_app_trace(long long* host) { return (int)cudaMemcpyFromSymbol(host, g_app_trace, sizeof(g_app_trace)); }
-#define APP_TR(k) do { if (blockIdx.x == 0 && blockIdx.y == 0) g_app_trace[k] = clock64(); } while (0)
-#else
-#define APP_TR(k) do { } while (0)
-#endif
-
 namespace ttt {
 
 int make_token_map(ttt_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int64_t cols,
@@ -61,7 +53,6 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   __shared__ uint32_t tmem_base_s;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  if (tid == 0) APP_TR(0);
   const int h = blockIdx.y;
   const int nsl = H / NS;                                    // steps per tile
   // tiles of this CTA: blockIdx.x, blockIdx.x + gridDim.x, ...
@@ -103,9 +94,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   tc_fence_after();
   // programmatic dependent launch: everything above overlapped the tail of the preceding kernel
   // (the commit that produces the weights); nothing below may run before it has completed
-  if (tid == 0) APP_TR(1);
   asm volatile("griddepcontrol.wait;" ::: "memory");
-  if (tid == 0) APP_TR(2);
   const uint32_t tb = tmem_base_s;
   if (tb != 0) __trap();      // all 512 columns belong to this CTA: the issuer uses absolute columns
 
@@ -149,7 +138,6 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       constexpr uint32_t idesc_d = umma_idesc(TM, HD, 0, 1, TTT_FMT_F16, TTT_FMT_F16);      // A = Hq (fp16), B = W2 rows, MN-major
       const uint64_t d13 = umma_smem_desc_sw128(sbase, 16, 1024);
       const uint64_t d2 = umma_smem_desc_sw128(sbase + nsl * 16384, 8192, 1024);
-      APP_TR(3);
       // forward of step st+1 is issued before the down projection of step st
       int f_tl = 0, f_n = 0;     // (tile, step) of the next forward
       int d_tl = 0, d_n = 0;     // (tile, step) of the next down projection
@@ -183,14 +171,11 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       // the forward MMAs run two steps ahead of the down projection: one buffer per warpgroup in
       // the epilogue, the third being filled
       fwd();
-      APP_TR(4);
       if (total_steps > 1) fwd();
       for (int st = 0; st < total_steps; ++st) {
         if (st + 2 < total_steps) fwd();
         down();
-        if (st == 0) APP_TR(5);
       }
-      APP_TR(6);
     }
   } else if (warp >= 4 && warp < IO_WARP0) {
     // ===================== SwiGLU epilogue warpgroups =====================
@@ -295,7 +280,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
       for (int tl = 0; tl < my_tiles; ++tl) load_q(tl);
     } else {
       for (int tl = 0; tl < my_tiles; ++tl) store_o(tl);
-      if (tid == IO_WARP0 * 32) { APP_TR(7); tma_store_wait<0>(); APP_TR(8); }
+      if (tid == IO_WARP0 * 32) { tma_store_wait<0>(); }
     }
   }
   tc_fence_before();

@@ -26,22 +26,6 @@
 #include "tc_common.cuh"
 #include "ttt_internal.h"
 
-#ifdef TTT_TRACE
-__device__ long long g_appp_trace[32];
-extern "C" int ttt_debug_appp_trace(long long* host) { return (int)cudaMemcpyFromSymbol(host, g_appp_trace, sizeof(g_appp_trace)); }
-#define PP_ACC(k) do { pp_acc[k] += clock64() - pp_t; pp_t = clock64(); } while (0)
-// timeline of one steady-state step (g == PP_G) of CTA pair 0, rank 0: clock64 marks of every role
-__device__ long long g_appp_tl[16];
-__device__ unsigned long long g_appp_span[2 * 80];   // globaltimer at start / end of rank 0 of every pair
-extern "C" int ttt_debug_appp_span(unsigned long long* host) { return (int)cudaMemcpyFromSymbol(host, g_appp_span, sizeof(g_appp_span)); }
-extern "C" int ttt_debug_appp_timeline(long long* host) { return (int)cudaMemcpyFromSymbol(host, g_appp_tl, sizeof(g_appp_tl)); }
-#define PP_G 44
-#define PP_TL(cond, k) do { if ((cond) && cid == 0 && rank == 0) g_appp_tl[k] = clock64(); } while (0)
-#else
-#define PP_ACC(k) do { } while (0)
-#define PP_TL(cond, k) do { } while (0)
-#endif
-
 namespace ttt {
 
 int make_token_map(ttt_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int64_t cols,
@@ -90,9 +74,6 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
   const int my_units = cid < nunits ? (nunits - cid + ncl - 1) / ncl : 0;
   const int G = my_units * nstep;                // steps of this pair, all units
 
-#ifdef TTT_TRACE
-  if (tid == 0 && rank == 0 && cid < 80) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); g_appp_span[2 * cid] = t; }
-#endif
   if (tid == 0) {
     for (int s = 0; s < NST; ++s) { mbar_init(&w_full[s], 1); mbar_init(&w_empty[s], 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(&q_full[b], 1); mbar_init(&q_free[b], 1); }
@@ -138,9 +119,6 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
         for (int n = 0; n < nstep; ++n, ++g) {
           const int s = g % NST;
           if (g >= NST) mbar_wait(&w_empty[s], ((g / NST) - 1) & 1);
-#ifdef TTT_EXP_NOWLOAD     // timing experiment only: the ring is filled once, later steps reuse stale weights
-          if (g >= NST) { if (rank == 0) mbar_arrive(&w_full[s]); continue; }
-#endif
           if (rank == 0) mbar_arrive_expect_tx(&w_full[s], 2 * WSTAGE_BYTES);
           const uint32_t bar = mapa_u32(&w_full[s], 0);
           uint8_t* dst = wring + s * WSTAGE_BYTES;
@@ -171,16 +149,11 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
         // suspended try_wait wakes ~230 clk after the phase completes.
         if (n == 0) mbar_wait(&q_full[qb], qph);
         mbar_wait(&w_full[st], sph);
-        PP_TL(g == PP_G, 0);
-        PP_TL(g == PP_G + NF, 10);
         if (g >= NF) {
           mbar_wait_spin(&w_empty[sw], swph);
           if (++sw == NST) { sw = 0; swph ^= 1; }
         }
         tc_fence_after();
-        PP_TL(g == PP_G, 1);
-        PP_TL(g == PP_G + NF, 11);
-        PP_TL(g == PP_G, 2);
         const uint64_t a0 = dq + (uint64_t)(qb * (QTILE_BYTES >> 4));
         const uint64_t b0 = dwf + (uint64_t)(st * (WSTAGE_BYTES >> 4));
         const uint32_t acc = C_F + fb * 128;
@@ -189,7 +162,6 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
           umma_ss2(acc, a0 + (uint64_t)((k >> 2) * (QSUB_BYTES >> 4) + (k & 3) * 2),
                    b0 + (uint64_t)((k >> 2) * (BOX_BYTES >> 4) + (k & 3) * 2), idesc_f, k > 0);
         tc_commit2(&f_full[fb]);
-        PP_TL(g == PP_G, 3);
         if (++n == nstep) { tc_commit2(&q_free[qb]); n = 0; if (qb) qph ^= 1; qb ^= 1; }
         if (++st == NST) { st = 0; sph ^= 1; }
         if (++fb == NF) fb = 0;
@@ -200,47 +172,24 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
     if (rank == 0 && elect_one() && G > 0) {
       constexpr uint32_t idesc_d = umma_idesc(2 * TM, HD, 0, 1, TTT_FMT_BF16, TTT_FMT_BF16);          // A = Hq (TMEM), B = W2 rows, MN-major
       const uint64_t dw2 = umma_smem_desc_sw128(sbase + 2 * QTILE_BYTES + W2_OFF, BOX_BYTES, 1024);
-#ifdef TTT_TRACE
-      long long pp_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-      long long pp_t = clock64();
-      const long long pp_start = pp_t;
-      unsigned long long pp_gt0;
-      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(pp_gt0));
-#endif
       // O(unit) (+)= Hq(step g) W2[step rows]; the step's W2 rows landed with its forward rows
       // (w_full was waited on by the forward issuer before F(g), which precedes Hq(g))
       int n = 0, u = 0, st = 0, fb = 0;
       uint32_t fph = 0;
       for (int g = 0; g < G; ++g) {
         if (n == 0 && u > 0) mbar_wait_spin(&o_free, (u - 1) & 1);   // O of the previous unit has been read
-        PP_ACC(3);
-        PP_TL(g == PP_G, 8);
         mbar_wait_spin(&hq_ready[fb], fph);
         tc_fence_after();
-        PP_TL(g == PP_G, 9);
-        PP_ACC(4);
         const uint64_t b0 = dw2 + (uint64_t)(st * (WSTAGE_BYTES >> 4));
         const uint32_t hq = C_F + fb * 128;
 #pragma unroll
         for (int k = 0; k < HSTEP / 16; ++k)             // +2048 B per 16 hidden rows
           umma_ts2(C_O, hq + 8 * k, b0 + 128 * k, idesc_d, (n > 0) | k);
         tc_commit2(&w_empty[st]);
-        PP_TL(g == PP_G, 12);
         if (++n == nstep) { tc_commit2(&o_full); n = 0; ++u; }
         if (++st == NST) st = 0;
         if (++fb == NF) { fb = 0; fph ^= 1; }
-        PP_ACC(6);
       }
-#ifdef TTT_TRACE
-      if (cid == 0) {
-        for (int k = 0; k < 8; ++k) g_appp_trace[k] = pp_acc[k];
-        g_appp_trace[8] = clock64() - pp_start;
-        g_appp_trace[9] = G;
-        unsigned long long pp_gt1;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(pp_gt1));
-        g_appp_trace[13] = (long long)(pp_gt1 - pp_gt0);      // ns: SM clock = [8] / [13] GHz
-      }
-#endif
     }
   } else if (warp >= 4 && warp < DRAIN_WARP0) {
     // ===================== SwiGLU epilogue warps =====================
@@ -253,42 +202,27 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
     const uint64_t HALF2 = pack2(0.5f, 0.5f);
     int fb = 0;
     uint32_t fph = 0;
-#ifdef TTT_TRACE
-    long long pp_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    long long pp_t = clock64();
-#endif
     for (int g = 0; g < G; ++g) {
       const uint32_t buf = lane_base + C_F + fb * 128;
-      PP_TL(g == PP_G && warp == 4 && lane == 0, 4);
       mbar_wait(&f_full[fb], fph);
       tc_fence_after();
-      PP_TL(g == PP_G && warp == 4 && lane == 0, 5);
-      PP_ACC(0);
       uint32_t rx[16], rb[16];
       tmem_ld_x16(buf + 16 * cg, rx);
       tmem_ld_x16(buf + 64 + 16 * cg, rb);
       tc_wait_ld();
       tc_fence_before();
-      PP_ACC(1);
       // every epilogue warp holds its x | b: x may be overwritten by Hq (named barrier 1, 16 warps)
       asm volatile("bar.sync 1, 512;" ::: "memory");
-      PP_ACC(2);
       uint32_t ph[8];
 #pragma unroll
       for (int c = 0; c < 16; c += 2) {
         const uint64_t x = fmul2(pack2u(rx[c], rx[c + 1]), HALF2);   // a / 2
         float x0, x1;
         unpack2(x, x0, x1);
-#ifdef TTT_EXP_NOMATH      // timing experiment only: no MUFU work
-        const uint64_t th = x;
-#else
         const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
-#endif
         const uint64_t S = ffma2(x, th, x);                          // SiLU(a) = a/2 (1 + tanh(a/2))
         ph[c >> 1] = pack_bf16x2_from2(fmul2(S, pack2u(rb[c], rb[c + 1])));
       }
-      PP_TL(g == PP_G && warp == 4 && lane == 0, 6);
-      PP_ACC(3);
       tmem_st_x8(buf + 8 * cg, ph);
       tc_wait_st();
       tc_fence_before();
@@ -296,28 +230,17 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
       if (lane == 0) {
         if (rank == 0) mbar_arrive(&hq_ready[fb]); else mbar_arrive_remote(&hq_ready[fb], 0);
       }
-      PP_TL(g == PP_G && warp == 4 && lane == 0, 7);
       if (++fb == NF) { fb = 0; fph ^= 1; }
-      PP_ACC(4);
     }
-#ifdef TTT_TRACE
-    if (cid == 0 && warp == 4 && lane == 0)
-      for (int k = 0; k < 5; ++k) g_appp_trace[(rank ? 24 : 16) + k] = pp_acc[k];
-#endif
   } else if (warp >= DRAIN_WARP0) {
     // ===================== O drain warps: O(unit) -> bf16 -> global =====================
     const int q = warp & 3, half = (warp - DRAIN_WARP0) >> 2;
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
     const int row = q * 32 + lane;                         // token row of the tile = TMEM lane
-#ifdef TTT_TRACE
-    long long pp_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    long long pp_t = clock64();
-#endif
     for (int u = 0; u < my_units; ++u) {
       const int unit = cid + u * ncl, h = unit / npairs, p = unit % npairs;
       mbar_wait(&o_full, u & 1);
       tc_fence_after();
-      PP_ACC(0);
       const int64_t tok = (int64_t)(2 * p + (int)rank) * TM + row;
       // this thread's 64 columns are pulled into registers (packed to bf16 on the fly) before the
       // first store: the single O accumulator is released after two TMEM round trips — the drain
@@ -332,7 +255,6 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
         for (int v = 0; v < 16; ++v)
           pk[16 * part + v] = pack_bf16x2(__uint_as_float(ro[2 * v]), __uint_as_float(ro[2 * v + 1]));
       }
-      PP_ACC(1);
       tc_fence_before();
       __syncwarp();
       if (lane == 0) {
@@ -343,12 +265,7 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
 #pragma unroll
         for (int v = 0; v < 8; ++v) dst[v] = make_uint4(pk[4 * v], pk[4 * v + 1], pk[4 * v + 2], pk[4 * v + 3]);
       }
-      PP_ACC(2);
     }
-#ifdef TTT_TRACE
-    if (cid == 0 && rank == 0 && warp == DRAIN_WARP0 && lane == 0)
-      for (int k = 0; k < 3; ++k) g_appp_trace[10 + k] = pp_acc[k];
-#endif
   }
   // neither CTA may leave (or free TMEM) while the pair's MMAs, remote arrivals or multicast commits
   // can still touch it
@@ -356,9 +273,6 @@ bf16_apply_wide_pair_kernel(const __grid_constant__ CUtensorMap mapW, const __gr
   __syncthreads();
   cluster_sync_all();
   if (warp == 0) tmem_dealloc2(tb, 512);
-#ifdef TTT_TRACE
-  if (tid == 0 && rank == 0 && cid < 80) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); g_appp_span[2 * cid + 1] = t; }
-#endif
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -39,40 +39,6 @@
 #include "tc_common.cuh"
 #include "ttt_internal.h"
 
-#ifdef TTT_TRACE   // debug builds only: per-tile clock timeline of CTA (0,0,0), staged in smem
-__device__ long long g_ttt_trace[64 * 16];
-__device__ unsigned long long g_ttt_time[4];      // globaltimer ns + clock64 at start / end of CTA (0,0,0)
-extern "C" int ttt_debug_time(unsigned long long* host) {
-  return (int)cudaMemcpyFromSymbol(host, g_ttt_time, sizeof(g_ttt_time));
-}
-__device__ unsigned long long g_ttt_cta_time[2 * 256];   // globaltimer at start / end of every CTA
-extern "C" int ttt_debug_cta_time(unsigned long long* host) {
-  return (int)cudaMemcpyFromSymbol(host, g_ttt_cta_time, sizeof(g_ttt_cta_time));
-}
-__device__ unsigned g_ttt_trace2[32 * 16 * 4];   // [tile][epilogue warp][got, loaded, math, done]
-#define TTT_TR2(i, w, k) do { if ((i) < 32 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && lane == 0) g_ttt_trace2[((i) * 16 + (w)) * 4 + (k)] = (unsigned)clock(); } while (0)
-extern "C" int ttt_debug_trace2(unsigned* host) {
-  return (int)cudaMemcpyFromSymbol(host, g_ttt_trace2, sizeof(g_ttt_trace2));
-}
-#ifdef TTT_TRACE_LIGHT     // only the start/end stamps: no probes inside the loops
-#define TTT_TR(i, k) do { } while (0)
-#undef TTT_TR2
-#define TTT_TR2(i, w, k) do { } while (0)
-#else
-#define TTT_TR(i, k)                                                                  \
-  do {                                                                                \
-    if ((i) < 64 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0)            \
-      tr_s[(i) * 16 + (k)] = (unsigned)clock();                                       \
-  } while (0)
-#endif
-extern "C" int ttt_debug_trace(long long* host) {
-  return (int)cudaMemcpyFromSymbol(host, g_ttt_trace, sizeof(g_ttt_trace));
-}
-#else
-#define TTT_TR(i, k) do { } while (0)
-#define TTT_TR2(i, w, k) do { } while (0)
-#endif
-
 namespace ttt {
 
 namespace upd {
@@ -117,21 +83,6 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   __shared__ float lrmax_s[THREADS / 32];
   static_assert(THREADS % 16 == 0, "the fused commit gives 16 lanes one weight row");
   __shared__ __align__(16) float ne_s[STAGES][T];   // -eta of the stage's tokens, scaled (0 beyond M)
-#ifdef TTT_TRACE
-  __shared__ unsigned tr_s[64 * 16];
-  for (int e = threadIdx.x; e < 64 * 16; e += blockDim.x) tr_s[e] = 0;
-  __syncthreads();
-  if (threadIdx.x == 0) tr_s[15] = (unsigned)clock();
-  if (threadIdx.x == 0) {
-    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    const int lin = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
-    if (lin < 256) g_ttt_cta_time[2 * lin] = t;
-  }
-  if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) {
-    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    g_ttt_time[0] = t; g_ttt_time[1] = clock64();
-  }
-#endif
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int split = blockIdx.x, slice = blockIdx.y, h = blockIdx.z;
@@ -145,15 +96,11 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
   // warp 1 initialises the other barriers; warp 3 allocates TMEM (trace, r01e: requests left at
   // 2.3-3.6 K clk when all of this was serial in thread 0, first forward MMA at 7-9 K clk).
   if (tid == 0) {
-    TTT_TR(8, 14);
     tma_prefetch_desc(&mapK);
     tma_prefetch_desc(&mapV);
-    TTT_TR(9, 14);
 #pragma unroll
     for (int s = 0; s < STAGES; ++s) mbar_init(&tma_full[s], 1);
-    TTT_TR(10, 14);
     fence_mbar_init();
-    TTT_TR(1, 14);
     const int npre = min(ntiles, STAGES);
     for (int i = 0; i < npre; ++i) {
       mbar_arrive_expect_tx(&tma_full[i], STAGE_BYTES);
@@ -161,7 +108,6 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       tma_load_2d(dst, &mapK, &tma_full[i], h * HD, (tile_lo + i) * T);
       tma_load_2d(dst + TILE_BYTES, &mapV, &tma_full[i], h * HD, (tile_lo + i) * T);
     }
-    TTT_TR(2, 14);
   } else if (tid == 32) {
 #pragma unroll
     for (int s = 0; s < STAGES; ++s) { mbar_init(&empty[s], 1); mbar_init(&full[s], CVT_WARPS); }
@@ -212,17 +158,11 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     if (lane == 0) lrmax_s[warp] = mx;
   }
   if (warp == 3) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
-  if (tid == 96) TTT_TR(3, 14);
-  if (tid == 255) TTT_TR(4, 14);
-  if (tid == 64) TTT_TR(11, 14);
-  if (tid == 31) TTT_TR(12, 14);
-  if (tid == 33) TTT_TR(13, 14);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tb = tmem_base_s;
   if (tb != 0) __trap();      // all 512 columns belong to this CTA: the issuers use absolute columns
-  if (tid == 0) TTT_TR(0, 14);
   float eta_sc, eta_isc;      // the gradient operands carry eta * eta_sc; undone at the flush
   {
     float mx = 0.f;
@@ -258,7 +198,6 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       uint64_t dk = d0;
       for (int i = 0; i < ntiles; ++i) {
         const int b = i & 1, n = i >> 1;
-        TTT_TR(i, 0);
         // the waits of a tile are probed together (a probe costs ~90 clk even when the phase is
         // already complete), then re-waited only if a probe failed
         const uint32_t ok0 = mbar_try_wait(&full[s], ph_full);
@@ -267,7 +206,6 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         if (!ok0) mbar_wait(&full[s], ph_full);
         if (!ok1) mbar_wait(&xb_free[b], (n - 1) & 1);
         tc_fence_after();
-        TTT_TR(i, 1);
         const uint32_t acc = C_XB + b * XB_STRIDE;
 #pragma unroll
         for (int k = 0; k < HD / 16; ++k) umma_ts(acc, C_W1 + 8 * k, dk + 2 * k, idesc_f, k > 0);
@@ -278,7 +216,6 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         for (int k = 0; k < HD / 16; ++k) umma_ts(C_GG, C_W2 + 8 * k, dk + V_OFF + 2 * k, idesc_f, k > 0);
         tc_commit(&fwd_full[b]);   // one barrier per epilogue group: a parity wait only tells the
                                    // current phase from the previous one
-        TTT_TR(i, 2);
         if (++s == STAGES) { s = 0; ph_full ^= 1; dk = d0; } else { dk += ST_OFF; }
       }
     }
@@ -294,9 +231,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         const int b = i & 1, n = i >> 1;
         mbar_wait(&epi_done[b], n & 1);
         tc_fence_after();
-        TTT_TR(i, 3);
         const uint32_t acc_flag = i > 0;
-#ifndef TTT_EXP_NOGRAD
 #pragma unroll
         for (int k = 0; k < T / 16; ++k)                     // +2048 B per 16-token K step
           umma_ts(C_G1, C_H + 8 * k, dk + 128 * k, idesc_g, acc_flag | k);
@@ -306,17 +241,14 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
 #pragma unroll
         for (int k = 0; k < T / 16; ++k)
           umma_ts(C_G2, C_H + 32 + 8 * k, dk + V_OFF + 128 * k, idesc_g, acc_flag | k);
-#endif
         tc_commit(&empty[s]);          // the tile's forward MMAs completed long ago (epilogue read them)
         tc_commit(&opnd_free[b]);     // one barrier per tile parity (see the epilogue's wait)
-        TTT_TR(i, 4);
         // TMA producer duty (this thread has the slack; warp 0 is a stage finisher): the stage of tile
         // i - 1, whose gradient MMAs were issued an iteration ago and are normally complete by now, is
         // refilled with tile i - 1 + STAGES
         if (i >= 1 && i - 1 + STAGES < ntiles) {
           const int j = i - 1 + STAGES, sj = (i - 1) % STAGES;
           mbar_wait(&empty[sj], ((i - 1) / STAGES) & 1);
-          TTT_TR(j, 12);
           mbar_arrive_expect_tx(&tma_full[sj], STAGE_BYTES);
           uint8_t* dst = smem + sj * STAGE_BYTES;
           tma_load_2d(dst, &mapK, &tma_full[sj], h * HD, (tile_lo + j) * T);
@@ -354,14 +286,11 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         if (i < ntiles) {
           const int s = i % STAGES, it = i / STAGES;
           mbar_wait(&tma_full[s], it & 1);       // (the TMA was issued after the stage's `empty`)
-          if (lane == 0 && i >= 16) TTT_TR(i, 13);
           tile_bf16_to_f16<STAGE_BYTES / 512 / CVT_WARPS>(smem + s * STAGE_BYTES, lane);
           ne_s[s][lane] = cur[u];
-          if (lane == 0 && i >= 16) TTT_TR(i, 14);
           fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) mbar_arrive(&full[s]);
-          if (lane == 0 && i >= 16) TTT_TR(i, 15);
 
         }
       }
@@ -399,7 +328,6 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&w_ready);
-      if (ew == 0 && lane == 0) TTT_TR(5, 14);
     }
     uint64_t loss2 = 0ull;
     const uint64_t ONE2 = pack2(1.0f, 1.0f), NONE2 = pack2(-1.0f, -1.0f);
@@ -408,33 +336,22 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     const uint32_t hbuf = tb + lane_base + C_H + 8 * kh;
     for (int i = grp; i < ntiles; i += 2) {
       const int n = i >> 1;
-      if (ew == 0 && lane == 0) TTT_TR(i, 5);
       mbar_wait(&fwd_full[grp], n & 1);
       mbar_wait(&full[i % STAGES], (i / STAGES) & 1);      // direct acquire of the loader's -eta slot
       tc_fence_after();
       const uint2* nes = reinterpret_cast<const uint2*>(&ne_s[i % STAGES][16 * kh]);
-      if (ew == 0 && lane == 0) TTT_TR(i, 7);
-      TTT_TR2(i, ew, 0);
       uint32_t rx[16], rb[16], rg[16];
-#ifdef TTT_EXP_NOTMEM
-      for (int c = 0; c < 16; ++c) { rg[c] = 0x3c000000u + c; rx[c] = 0x3c000000u + i; rb[c] = 0x3d000000u + c; }
-#else
       tmem_ld_x16(gbuf, rg);                               // g is single-buffered: release it first
-#endif
       tc_wait_ld();
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&g_free);
-#ifndef TTT_EXP_NOTMEM
       tmem_ld_x16(xbuf, rx);
       tmem_ld_x16(xbuf + 32, rb);
-#endif
       tc_wait_ld();
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&xb_free[grp]);           // forward MMAs of tile i+2 may overwrite x | b
-      if (ew == 0 && lane == 0) TTT_TR(i, 6);
-      TTT_TR2(i, ew, 1);
       uint32_t pa[8], pb[8], ph[8];
 #pragma unroll
       for (int c = 0; c < 16; c += 2) {
@@ -445,11 +362,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         const uint64_t g = fmul2(ne, pack2u(rg[c], rg[c + 1]));   // dHd = (-eta v) W2^T
         float x0, x1;
         unpack2(x, x0, x1);
-#ifdef TTT_EXP_NOMATH
-        const uint64_t th = x;
-#else
         const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
-#endif
         const uint64_t S = ffma2(x, th, x);                  // SiLU(a) = a sigmoid(a), a = 2 x
         const uint64_t p = fadd2(th, ONE2);                  // 2 sigmoid(a)
         const uint64_t m = ffma2(th, NONE2, ONE2);           // 2 (1 - sigmoid(a))
@@ -460,37 +373,25 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         ph[c >> 1] = pack_f16x2_from2(fmul2(ne, hdv));            // Hd' = -eta Hd
         if (LOSS) loss2 = ffma2(hdv, g, loss2);
       }
-      if (ew == 0 && lane == 0) TTT_TR(i, 8);
-      TTT_TR2(i, ew, 2);
       // the operand buffer was last read by the gradient MMAs of tile i - 1
       // (an epilogue group sees every OTHER tile: on one barrier shared by both tile parities its
       // parity wait could not tell "tile i - 1 done" from "tile i - 3 done" when the gradient issuer
       // lags by two tiles, and a fast warp would overwrite operands not yet read; with one barrier per
       // tile parity the phase it waits for is always the barrier's current or latest completed one)
       if (i > 0) { mbar_wait(&opnd_free[grp ^ 1], ((i - 1) >> 1) & 1); tc_fence_after(); }
-      if (ew == 0 && lane == 0) TTT_TR(i, 10);
-#ifdef TTT_EXP_NOTMEM
-      if (pa[0] + pb[1] + ph[2] == 0x12345u) tmem_st_x8(hbuf, pa);
-#else
       tmem_st_x8(hbuf, pa);
       tmem_st_x8(hbuf + 16, pb);
       tmem_st_x8(hbuf + 32, ph);
-#endif
       tc_wait_st();
-      if (ew == 0 && lane == 0) TTT_TR(i, 11);
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&epi_done[grp]);
-      if (ew == 0 && lane == 0) TTT_TR(i, 9);
-      TTT_TR2(i, ew, 3);
     }
     // a dependent kernel (PDL) may be scheduled from here on; it still waits for this grid to finish
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // ---- flush the gradient accumulators: one fp32 partial slice per CTA ----
-    if (ew == 0 && lane == 0) TTT_TR(2, 13);
     mbar_wait(&grad_done, 0);
     tc_fence_after();
-    if (ew == 0 && lane == 0) TTT_TR(3, 13);
     float* Pset = P + (size_t)split * 3 * me;
     const uint32_t gcol[3] = {C_G1, C_G2, C_G3};
     // TMEM gives a thread 16 columns of ONE row: written to global memory directly, a warp store would
@@ -525,7 +426,6 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         dst[e] = *reinterpret_cast<const float4*>(sb + (e >> 4) * SLD + 4 * (e & 15));
       }
     }
-    if (ew == 0 && lane == 0) TTT_TR(4, 13);
     if (LOSS) {
       float l0, l1;
       unpack2(loss2, l0, l1);
@@ -559,7 +459,6 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(sync_ctr + h * nslices + slice) : "memory");
         if (clock64() - t0 > TTT_MBAR_TIMEOUT_CYCLES) __trap();
       } while ((int)(v - sync_target) < 0);
-      TTT_TR(6, 14);
     }
     __syncthreads();
     const size_t me = (size_t)nh * H * HD, set = 3 * me;
@@ -633,7 +532,6 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
         }
       }
     }
-    if (tid == 0) TTT_TR(7, 14);
     if (renorm_n0 != nullptr) {
       float4* cs = reinterpret_cast<float4*>(smem);         // the K/V ring is idle by now
       cs[tid] = colacc;
@@ -649,21 +547,6 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
       }
     }
   }
-#ifdef TTT_TRACE
-  if (threadIdx.x == 0) tr_s[16 + 15] = (unsigned)clock();
-  if (threadIdx.x == 0) {
-    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    const int lin = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
-    if (lin < 256) g_ttt_cta_time[2 * lin + 1] = t;
-  }
-  if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) {
-    unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    g_ttt_time[2] = t; g_ttt_time[3] = clock64();
-  }
-  __syncthreads();
-  if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0)
-    for (int e = threadIdx.x; e < 64 * 16; e += blockDim.x) g_ttt_trace[e] = tr_s[e];
-#endif
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -19,20 +19,6 @@
 #include "tc_common.cuh"
 #include "ttt_internal.h"
 
-#ifdef TTT_TRACE
-__device__ long long g_updw_dbg[16];
-extern "C" int ttt_debug_updw(long long* host) {
-  return (int)cudaMemcpyFromSymbol(host, g_updw_dbg, sizeof(g_updw_dbg));
-}
-#define UPDW_T0() const long long t0__ = clock64()
-#define UPDW_ACC(k) do { if (blockIdx.x == 0) g_updw_dbg[(k)] += clock64() - t0__; } while (0)
-#define UPDW_SET(k, v) do { if (blockIdx.x == 0) g_updw_dbg[(k)] = (v); } while (0)
-#else
-#define UPDW_T0() do { } while (0)
-#define UPDW_ACC(k) do { } while (0)
-#define UPDW_SET(k, v) do { } while (0)
-#endif
-
 namespace ttt {
 
 int make_token_map(ttt_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int64_t cols,
@@ -207,10 +193,6 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
         }
       };
       int gi = 0, seg = 0;
-#ifdef TTT_TRACE
-      const long long tstart = clock64();
-      if (blockIdx.x == 0) for (int k = 0; k < 8; ++k) g_updw_dbg[k] = 0;
-#endif
       while (gi < total) {
         int pair, t0;
         locate(gi, pair, t0);
@@ -225,15 +207,13 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
         for (int i = 0; i < n; ++i, ++gi) {
           const int s = gi % STAGES;
           const uint64_t st = (uint64_t)s * (STAGE_BYTES >> 4);
-          { UPDW_T0(); mbar_wait(&full[s], (gi / STAGES) & 1); UPDW_ACC(1); }
-          { UPDW_T0();
+          mbar_wait(&full[s], (gi / STAGES) & 1);
           if (i > 0) mbar_wait(&xbg_free, (gi - 1) & 1);       // x | b | g of the previous tile are in registers
-          UPDW_ACC(2); }
           tc_fence_after();
           forward(2, st, C_B);
           forward(1, st + (TILE_BYTES >> 4), C_G);
           if (i > 0) {
-            { UPDW_T0(); mbar_wait(&opnd_ready, (gi - 1) & 1); UPDW_ACC(3); }
+            mbar_wait(&opnd_ready, (gi - 1) & 1);
             tc_fence_after();
             grad_w2(st_prev, i > 1);
           }
@@ -256,10 +236,6 @@ bf16_update_wide_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_c
         tc_commit(&grad_done);
         ++seg;
       }
-#ifdef TTT_TRACE
-      UPDW_SET(0, clock64() - tstart);
-      UPDW_SET(4, (long long)total);
-#endif
     }
   } else if (warp == 2) {
     // ===================== stage finisher 0: fp16 conversion, learning rates =====================

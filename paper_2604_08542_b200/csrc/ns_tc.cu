@@ -30,16 +30,6 @@
 #include "tc_common.cuh"
 #include "ttt_internal.h"
 
-#ifdef TTT_TRACE
-__device__ long long g_ns_trace[64];
-extern "C" int ttt_debug_ns_trace(long long* host) {
-  return (int)cudaMemcpyFromSymbol(host, g_ns_trace, sizeof(g_ns_trace));
-}
-#define NS_TR(k) do { if (blockIdx.x == 0 && threadIdx.x == 0 && (k) < 64) g_ns_trace[(k)] = clock64(); } while (0)
-#else
-#define NS_TR(k) do { } while (0)
-#endif
-
 namespace ttt {
 
 namespace nstc {
@@ -97,12 +87,10 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
   uint8_t* PL = PH + 8192;
   float* S = reinterpret_cast<float*>(PL + 8192);          // [128][S_LD]
 
-  NS_TR(0);
   if (tid == 0) { mbar_init(&mma_bar, 1); fence_mbar_init(); }
   if (warp == 0) { tmem_alloc(&tmem_base_s, tmem_cols); tmem_relinquish(); }
   // programmatic dependent launch: the set-up above overlapped the tail of the gradient kernel
   asm volatile("griddepcontrol.wait;" ::: "memory");
-  NS_TR(59);
 
   // ---- load: g = (use_G ? G : 0) + sum_s P[s] (fixed order), written back to G; Frobenius norm ----
   const size_t mat_off = (size_t)blockIdx.x * H * HD;
@@ -145,7 +133,6 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
       }
     }
   }
-  NS_TR(60);
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
   if (lane == 0 && !issuer) red[warp] = acc;
@@ -160,7 +147,6 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
   }
   __syncthreads();
   const float scale = s_scale;
-  NS_TR(61);
   for (int e0 = issuer ? n4 : tid; e0 < n4; e0 += THREADS * LB) {   // same thread re-reads what it wrote
     float4 g[LB];
 #pragma unroll
@@ -187,7 +173,6 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
   }
   fence_proxy_async_smem();
   __syncthreads();
-  NS_TR(1);
 
   constexpr uint32_t idesc_gram = umma_idesc_bf16(128, 128, 1, 1);  // A, B MN-major, hi | lo atoms
   constexpr uint32_t idesc_k128 = umma_idesc_bf16(128, 128, 0, 0);  // A, B K-major, 128 rows each
@@ -245,9 +230,7 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
       for (int ks = 0; ks < H / 16; ++ks, d += 128) umma_ss(tb + C_A, d, d, idesc_gram, ks > 0);
       tc_commit(&mma_bar);
     }
-    NS_TR(2 + it * 8);
     if (!issuer) { wait_mma(); fold_export(C_A); }
-    NS_TR(3 + it * 8);
     __syncthreads();
     if (!issuer) {
       fold_import(Areg);
@@ -257,7 +240,6 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
       *reinterpret_cast<uint4*>(AL + sw128_off(frow, fch)) = lo;
     }
     end_phase();
-    NS_TR(4 + it * 8);
     // ---------------- Pm = a I + b A + c A A ----------------
     if (lead) {
 #pragma unroll
@@ -266,7 +248,6 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
       tc_commit(&mma_bar);
     }
     if (!issuer) { wait_mma(); fold_export(C_A2); }
-    NS_TR(5 + it * 8);
     __syncthreads();
     if (!issuer) {
       float pm[8];
@@ -283,7 +264,6 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
       *reinterpret_cast<uint4*>(PL + sw128_off(frow, fch)) = lo;
     }
     end_phase();
-    NS_TR(6 + it * 8);
     // ---------------- X <- X Pm ----------------
     if (lead) {
       for (int mb = 0; mb < nblk; ++mb) {
@@ -297,7 +277,6 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
       }
       tc_commit(&mma_bar);
     }
-    NS_TR(7 + it * 8);
     if (!issuer) {
       wait_mma();
       float* stage = reinterpret_cast<float*>(smem);          // last iteration: fp32 [H][W_LD]
@@ -328,9 +307,7 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
         }
       }
     }
-    NS_TR(8 + it * 8);
     end_phase();
-    NS_TR(9 + it * 8);
   }
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   // ---- coalesced write-out: fused commit W <- W - NS(g) (Eq. 8) or NS(g) -> G ----
@@ -362,7 +339,6 @@ ns_tc_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets, siz
       }
     }
   }
-  NS_TR(50);
   if (warp == 0) tmem_dealloc(tb, tmem_cols);
 }
 

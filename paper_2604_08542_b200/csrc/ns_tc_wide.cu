@@ -21,16 +21,6 @@
 #include "tc_common.cuh"
 #include "ttt_internal.h"
 
-#ifdef TTT_TRACE
-__device__ long long g_nsw_trace[64];
-extern "C" int ttt_debug_nsw_trace(long long* host) {
-  return (int)cudaMemcpyFromSymbol(host, g_nsw_trace, sizeof(g_nsw_trace));
-}
-#define NSW_TR(k) do { if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && (k) < 64) g_nsw_trace[(k)] = clock64(); } while (0)
-#else
-#define NSW_TR(k) do { } while (0)
-#endif
-
 namespace ttt {
 
 namespace nsw {
@@ -137,7 +127,6 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
     }
   };
 
-  NSW_TR(0);
   if (tid == 0) { mbar_init(&mma_bar, 1); fence_mbar_init(); }
   if (warp == 0) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
   // programmatic dependent launch: the set-up above overlapped the tail of the gradient kernel
@@ -204,7 +193,6 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
   }
   fence_proxy_async_smem();
   __syncthreads();
-  NSW_TR(1);
 
   constexpr uint32_t idesc_mn = umma_idesc_bf16(128, 128, 1, 1);   // A, B MN-major (Gram)
   constexpr uint32_t idesc_k = umma_idesc_bf16(128, 128, 0, 0);    // A, B K-major
@@ -258,7 +246,6 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
     __syncwarp();
     if (!issuer) {
       wait_mma();
-      NSW_TR(2 + it * 8);
       float v[32];
       {
         uint32_t r[32];
@@ -273,10 +260,8 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
 #pragma unroll
       for (int k = 0; k < 8; ++k) dst[tid + THREADS * k] = *reinterpret_cast<const float4*>(ex_co(k));
     }
-    NSW_TR(3 + it * 8);
     cluster_arrive();                  // release at cluster scope: orders this rank's global writes for its peers
     cluster_wait();
-    NSW_TR(4 + it * 8);
     if (!issuer) {
       float4 a[8];
 #pragma unroll
@@ -304,7 +289,6 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
       split_row32(Areg, AH, AL, trow, cs);
     }
     end_phase();
-    NSW_TR(5 + it * 8);
     // ---------------- Pm = a I + b A + c A A (A symmetric: K-major A . A^T) ----------------
     if (lead) product_k(tb + C_A2, d_ah, d_al, d_ah, d_al);
     __syncwarp();
@@ -323,7 +307,6 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
       split_row32(pm, AH, AL, trow, cs);                   // the A tiles are dead: Pm takes their place
     }
     end_phase();
-    NSW_TR(6 + it * 8);
     // ---------------- X <- X Pm (Pm symmetric: K-major X . Pm^T) ----------------
     if (lead) product_k(tb + C_X, d_xh, d_xl, d_ah, d_al);
     __syncwarp();
@@ -367,11 +350,9 @@ ns_tc_wide_kernel(float* __restrict__ G, const float* __restrict__ P, int n_sets
       }
     }
     end_phase();
-    NSW_TR(7 + it * 8);
   }
   cluster_arrive();                    // no rank may exit while another still reads its s_part
   cluster_wait();
-  NSW_TR(50);
   if (warp == 0) tmem_dealloc(tb, 512);
 }
 

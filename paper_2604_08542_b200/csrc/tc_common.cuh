@@ -489,9 +489,6 @@ __device__ __forceinline__ uint32_t bf16x2_to_f16x2(uint32_t w) {
 template <int CPL>
 __device__ __forceinline__ void tile_bf16_to_f16(uint8_t* tile, int lane) {
   constexpr int B = CPL < 8 ? CPL : 8;        // loads in flight per lane
-#ifdef TTT_EXP_NOCVT       // timing experiment only
-  return;
-#endif
   uint4* p = reinterpret_cast<uint4*>(tile) + lane;
 #pragma unroll
   for (int k0 = 0; k0 < CPL; k0 += B) {
