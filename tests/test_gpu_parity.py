@@ -527,6 +527,36 @@ def test_bf16_large_head_dimension_parity(nh, hd, H, M, chunks):
     assert max(errs_l) <= TOL_LOSS_BF16, errs_l
 
 
+@pytest.mark.parametrize("M", [1, 70, 129])
+def test_bf16_large_tiny_chunks_strided_rows_and_nonuniform_lr(M):
+    """Edge cases of the large-dimension path: chunks smaller than one token tile / one 64-token contraction
+    chunk of the gradient GEMMs, token rows with padding (ld > nh*hd), per-token learning rates of both signs
+    and zero, and the loss output."""
+    from paper_2604_08542_b200 import TTT, TTT_BF16
+    dev = torch.device("cuda", 0)
+    nh, hd, H = 1, 256, 256
+    ld = nh * hd + 40
+    g = torch.Generator().manual_seed(300 + M)
+    W1 = torch.randn(nh, hd, H, generator=g) / 16
+    W2 = torch.randn(nh, H, hd, generator=g) / 16
+    W3 = torch.randn(nh, hd, H, generator=g) / 16
+    buf = [torch.randn(M, ld, generator=g).to(torch.bfloat16) for _ in range(3)]
+    Q, K, V = (b[:, :nh * hd] for b in buf)
+    lr = (torch.rand(nh, M, generator=g) - 0.3) * 0.01
+    lr[:, ::3] = 0.0
+    t = TTT(nh, hd, H, TTT_BF16, max_tokens=256)
+    t.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+    dQ, dK, dV = (b.to(dev)[:, :nh * hd] for b in buf)
+    loss = torch.zeros(nh, device=dev)
+    O = t.ttt_chunk_step(dQ, dK, dV, lr.to(dev), loss=loss)
+    ora = OracleTTT(W1, W2, W3)
+    O_ref, loss_ref = ora.chunk_step(Q.contiguous(), K.contiguous(), V.contiguous(), lr)
+    assert rel_err(O.float().cpu(), O_ref) <= TOL_BF16
+    assert max(rel_err(a.cpu(), b) for a, b in zip(t.ttt_get_weights(), ora.weights())) <= TOL_BF16
+    assert rel_err(loss.cpu(), loss_ref) <= TOL_LOSS_BF16
+    t.close()
+
+
 def test_bf16_large_accumulate_commit_and_rejected_options():
     """Eq. 10 on the large-dimension path (two accumulates at the same W, one commit == the oracle's summed
     gradient step) and the options the path does not offer (Newton-Schulz, renorm: TTT_ERR_SHAPE)."""
