@@ -42,6 +42,9 @@ constexpr int BOX = TM * 128;      // bytes of a [128 rows x 64] bf16 box (16 KB
 // plus the epilogue's TMA-store staging tiles (three for the update, one for the apply)
 constexpr int F_STAGE = 3 * BOX, F_STAGES_U = 3, F_STAGES_A = 4;
 constexpr int F_SMEM_U = F_STAGES_U * F_STAGE + 3 * BOX + 1024, F_SMEM_A = F_STAGES_A * F_STAGE + BOX + 1024;
+// CTA-pair variant: a stage is the CTA's token chunk + its HALF of the weight rows = 32 KB
+constexpr int P_STAGES_U = 5, P_STAGES_A = 6;
+constexpr int P_SMEM_U = P_STAGES_U * 2 * BOX + 3 * BOX + 1024, P_SMEM_A = P_STAGES_A * 2 * BOX + BOX + 1024;
 constexpr uint32_t C_XB = 0, C_G = 256;                // x | b [128 x 256] fp32; g0 [128 x 128] fp32, two buffers
 // MN-major-B kernels: stage = A 16 KB + B 32 KB, two accumulators [128 x 256] fp32
 constexpr int M_STAGE = 3 * BOX, M_STAGES = 4;
@@ -51,17 +54,25 @@ constexpr int TN = 256;
 // ------------------------------------------------------------------------------------------------
 // F: forward products + SwiGLU epilogue. UPD: update (x | b | g0 -> dA, dB, Hd'); else apply (-> Hq).
 // Work item = (token tile tt, hidden slice s, head h), slice fastest; persistent CTAs.
+// PAIR: the same on CTA pairs (cluster of 2, tcgen05 cta_group::2, M = 256): a pair takes two adjacent
+// token tiles (one per CTA) of a hidden slice and SHARES every B operand — rank 0 loads and holds the
+// W1^T rows (x = N columns 0-127) and rows 0-63 of the W2 slice, rank 1 the W3^T rows (b) and W2 rows
+// 64-127 — so each CTA streams and reads half of the weight bytes: the single-CTA kernel's SS-mode MMAs
+// are bound by the shared-memory pipe (ncu: 57-88 % busy, N = 128 products at 113 clk against 64).
+// Rank 0 issues every MMA; both CTAs' TMA loads complete on rank 0's `full` barriers; commits are
+// multicast to both CTAs' `empty` / `acc_full`; rank 1's epilogue warps arrive on rank 0's `acc_empty`.
 // ------------------------------------------------------------------------------------------------
-template <bool UPD, bool LOSS>
+template <bool UPD, bool LOSS, bool PAIR>
 __global__ void __launch_bounds__(lg::THREADS, 1)
 ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapV,
-                  const __grid_constant__ CUtensorMap mapW, const __grid_constant__ CUtensorMap mapO0,
+                  const __grid_constant__ CUtensorMap mapW, const __grid_constant__ CUtensorMap mapWh,
+                  const __grid_constant__ CUtensorMap mapO0,
                   const __grid_constant__ CUtensorMap mapO1, const __grid_constant__ CUtensorMap mapO2,
                   const float* __restrict__ lr, float* __restrict__ loss_part, int M, int nh, int hd,
                   int H, int n_items) {
   using namespace lg;
-  constexpr int STAGE = F_STAGE;
-  constexpr int STAGES = UPD ? F_STAGES_U : F_STAGES_A;
+  constexpr int STAGE = PAIR ? 2 * BOX : F_STAGE;
+  constexpr int STAGES = PAIR ? (UPD ? P_STAGES_U : P_STAGES_A) : (UPD ? F_STAGES_U : F_STAGES_A);
   // TMEM: update x | b (256 columns) + two g0 buffers (2 x 128); apply two x | b buffers
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -71,17 +82,27 @@ ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constan
   __shared__ float loss_red[EPI_WARPS];
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const uint32_t rank = PAIR ? cluster_rank() : 0u;
+  const int cta0 = PAIR ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;     // first item, stride over items
+  const int ncta = PAIR ? (int)(gridDim.x >> 1) : (int)gridDim.x;
   const int nslices = H / TM, ntt = (M + TM - 1) / TM, nkc = hd / KC;
+  const int ntr = PAIR ? (ntt + 1) / 2 : ntt;                           // token-tile rows of the item space
   if (tid == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(&acc_full[b], 1); mbar_init(&acc_empty[b], EPI_WARPS); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&acc_full[b], 1); mbar_init(&acc_empty[b], (PAIR ? 2 : 1) * EPI_WARPS); }
     fence_mbar_init();
     tma_prefetch_desc(&mapX);
     tma_prefetch_desc(&mapW);
     tma_prefetch_desc(&mapO0);
     if (UPD) tma_prefetch_desc(&mapV);
   }
-  if (warp == 2) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  if (PAIR) {
+    __syncthreads();
+    cluster_sync_all();            // the peer's barriers exist before anything can arrive on them
+    if (warp == 2) { tmem_alloc2(&tmem_base_s, 512); tmem_relinquish2(); }
+  } else {
+    if (warp == 2) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -92,21 +113,35 @@ ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constan
   auto item = [&](int id, int& h, int& tt, int& s) {
     s = id % nslices;
     const int r = id / nslices;
-    tt = r % ntt;
-    h = r / ntt;
+    tt = PAIR ? 2 * (r % ntr) + (int)rank : r % ntr;
+    h = r / ntr;
   };
 
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (elect_one()) {
       int g = 0;                                       // running chunk counter over all items
-      for (int id = blockIdx.x; id < n_items; id += gridDim.x) {
+      for (int id = cta0; id < n_items; id += ncta) {
         int h, tt, s;
         item(id, h, tt, s);
         for (int kc = 0; kc < (UPD ? 2 : 1) * nkc; ++kc, ++g) {
           const int st = g % STAGES;
           if (g >= STAGES) mbar_wait(&empty[st], ((g / STAGES) - 1) & 1);
           uint8_t* dst = smem + st * STAGE;
+          if (PAIR) {
+            const uint32_t bar = mapa_u32(&full[st], 0);           // rank 0's barrier collects both CTAs' bytes
+            if (UPD && kc < nkc) {                                 // g0: own V chunk, own half of the W2 rows
+              if (rank == 0) mbar_arrive_expect_tx(&full[st], 2 * (BOX + BOX / 2));
+              tma_load_2d_pair(dst, &mapV, bar, h * hd + kc * KC, tt * TM);
+              tma_load_2d_pair(dst + BOX, &mapWh, bar, kc * KC, (1 * nh + h) * H + s * TM + 64 * (int)rank);
+            } else {                                               // x | b: own K / Q chunk, W1^T (rank 0) or W3^T rows
+              const int k2 = UPD ? kc - nkc : kc;
+              if (rank == 0) mbar_arrive_expect_tx(&full[st], 4 * BOX);
+              tma_load_2d_pair(dst, &mapX, bar, h * hd + k2 * KC, tt * TM);
+              tma_load_2d_pair(dst + BOX, &mapW, bar, k2 * KC, ((rank ? 2 : 0) * nh + h) * H + s * TM);
+            }
+            continue;
+          }
           if (UPD && kc < nkc) {                         // update, first pass: g0 = V W2^T
             mbar_arrive_expect_tx(&full[st], 2 * BOX);
             tma_load_2d(dst, &mapV, &full[st], h * hd + kc * KC, tt * TM);                            // V chunk
@@ -123,12 +158,16 @@ ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constan
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
-    if (elect_one()) {
-      constexpr uint32_t idesc_xb = umma_idesc_bf16(TM, 256, 0, 0);   // A = token chunk, B = [W1 ; W3] rows, K-major
-      constexpr uint32_t idesc_g = umma_idesc_bf16(TM, 128, 0, 0);    // A = V chunk, B = W2 rows
+    if (rank == 0 && elect_one()) {
+      constexpr uint32_t idesc_xb = umma_idesc_bf16(PAIR ? 2 * TM : TM, 256, 0, 0);   // A = token chunk, B = [W1 ; W3] rows, K-major
+      constexpr uint32_t idesc_g = umma_idesc_bf16(PAIR ? 2 * TM : TM, 128, 0, 0);    // A = V chunk, B = W2 rows
       const uint64_t d0 = umma_smem_desc_sw128(sbase, 16, 1024);
+      auto mma = [&](uint32_t d, uint64_t a, uint64_t b, uint32_t idesc, uint32_t acc) {
+        if (PAIR) umma_ss2(d, a, b, idesc, acc); else umma_ss(d, a, b, idesc, acc);
+      };
+      auto commit = [&](uint64_t* bar) { if (PAIR) tc_commit2(bar); else tc_commit(bar); };
       int g = 0, n = 0;
-      for (int id = blockIdx.x; id < n_items; id += gridDim.x, ++n) {
+      for (int id = cta0; id < n_items; id += ncta, ++n) {
         // update: g0 first, into the g buffer of this item's parity (its last reader, the epilogue of item
         // n - 2, finished before the x | b pass of item n - 1 began), then x | b once the epilogue of item
         // n - 1 has read the previous x | b: that epilogue runs under this item's g0 pass.
@@ -145,15 +184,15 @@ ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constan
           if (UPD && kc < nkc) {
 #pragma unroll
             for (int k = 0; k < KC / 16; ++k)
-              umma_ss(cg, ds + 2 * k, ds + (BOX >> 4) + 2 * k, idesc_g, (kc > 0) | k);
+              mma(cg, ds + 2 * k, ds + (BOX >> 4) + 2 * k, idesc_g, (kc > 0) | k);
           } else {
 #pragma unroll
             for (int k = 0; k < KC / 16; ++k)
-              umma_ss(cxb, ds + 2 * k, ds + (BOX >> 4) + 2 * k, idesc_xb, (kc > (UPD ? nkc : 0)) | k);
+              mma(cxb, ds + 2 * k, ds + (BOX >> 4) + 2 * k, idesc_xb, (kc > (UPD ? nkc : 0)) | k);
           }
-          tc_commit(&empty[st]);
+          commit(&empty[st]);
         }
-        tc_commit(&acc_full[ab]);
+        commit(&acc_full[ab]);
       }
     }
   } else if (warp >= 4) {
@@ -169,7 +208,7 @@ ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constan
     uint8_t* stg = smem + STAGES * STAGE;                         // NOPS staging tiles of BOX bytes
     const bool leader = tid == 4 * 32;
     int n = 0;
-    for (int id = blockIdx.x; id < n_items; id += gridDim.x, ++n) {
+    for (int id = cta0; id < n_items; id += ncta, ++n) {
       int h, tt, s;
       item(id, h, tt, s);
       const int ab = UPD ? 0 : (n & 1);
@@ -198,7 +237,9 @@ ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constan
           if (p == 1 && gi == 1) {                                // last TMEM read of this tile: release it
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&acc_empty[ab]);
+            if (lane == 0) {
+              if (rank == 0) mbar_arrive(&acc_empty[ab]); else mbar_arrive_remote(&acc_empty[ab], 0);
+            }
           }
           uint32_t pa[8], pb[8], ph[8];
 #pragma unroll
@@ -260,7 +301,7 @@ ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constan
         if (leader) {
           float t = 0.f;
           for (int w = 0; w < EPI_WARPS; ++w) t += loss_red[w];
-          loss_part[(size_t)(tt * nslices + s) * nh + h] = t;
+          if (tt < ntt) loss_part[(size_t)(tt * nslices + s) * nh + h] = t;
         }
       }
     }
@@ -269,7 +310,12 @@ ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constan
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   tc_fence_before();
   __syncthreads();
-  if (warp == 2) tmem_dealloc(tb, 512);
+  if (PAIR) {
+    cluster_sync_all();            // neither CTA may leave while the pair's MMAs / remote arrivals can still touch it
+    if (warp == 2) tmem_dealloc2(tb, 512);
+  } else {
+    if (warp == 2) tmem_dealloc(tb, 512);
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -432,18 +478,24 @@ int64_t bf16_large_loss_rows(const ttt_config* cfg) {
   return ((cfg->max_tokens + lg::TM - 1) / lg::TM) * (cfg->hidden / lg::TM);
 }
 
+// `cluster` = 2 launches CTA pairs (grid = 2 x pairs)
 template <typename Kern, typename... Args>
-static int launch_pdl(ttt_ctx* ctx, const char* what, Kern kern, int grid, size_t smem, cudaStream_t s, Args... args) {
+static int launch_pdl(ttt_ctx* ctx, const char* what, Kern kern, int grid, size_t smem, cudaStream_t s, int cluster,
+                      Args... args) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(grid);
   cfg.blockDim = dim3(lg::THREADS);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = s;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
+  attr[1].id = cudaLaunchAttributeClusterDimension;
+  attr[1].val.clusterDim.x = cluster;
+  attr[1].val.clusterDim.y = 1;
+  attr[1].val.clusterDim.z = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = 1;
+  cfg.numAttrs = cluster > 1 ? 2 : 1;
   cudaError_t e = cudaLaunchKernelEx(&cfg, kern, args...);
   if (e != cudaSuccess) return set_error(ctx, TTT_ERR_CUDA, what, e);
   e = cudaGetLastError();
@@ -456,9 +508,28 @@ static int large_attrs(ttt_ctx* ctx) {
   if (ctx->attr_done & ATTR_LARGE) return TTT_OK;
   const int su = lg::F_SMEM_U, sa = lg::F_SMEM_A;
   const int sm = lg::M_STAGE * lg::M_STAGES + 1024;
-  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, su), "ld_forward smem attr");
-  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, su), "ld_forward smem attr");
-  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sa), "ld_forward smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, su), "ld_forward smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, su), "ld_forward smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sa), "ld_forward smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lg::P_SMEM_U), "ld_forward smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lg::P_SMEM_U), "ld_forward smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_forward_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lg::P_SMEM_A), "ld_forward smem attr");
+  {   // CTA pairs the device can host at once (0 -> the single-CTA kernels are used)
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(2 * (ctx->sm_count / 2));
+    cfg.blockDim = dim3(lg::THREADS);
+    cfg.dynamicSmemBytes = lg::P_SMEM_U;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, ld_forward_kernel<true, false, true>, &cfg) != cudaSuccess) { n = 0; cudaGetLastError(); }
+    ctx->ld_pairs = n;
+  }
   TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_mn_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "ld_mn_gemm smem attr");
   TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_mn_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "ld_mn_gemm smem attr");
   ctx->attr_done |= ATTR_LARGE;
@@ -486,16 +557,27 @@ int bf16_large_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloa
   if ((rc = make_token_map(ctx, &mK64, K, M, (int64_t)c.nh * c.hd, ld, 64)) != TTT_OK) return rc;
   if ((rc = make_token_map(ctx, &mV64, V, M, (int64_t)c.nh * c.hd, ld, 64)) != TTT_OK) return rc;
   const int ntt = (int)((M + lg::TM - 1) / lg::TM), nsl = c.hidden / lg::TM;
+  CUtensorMap mWh;                                 // weight rows in boxes of 64 (a CTA pair's half of the W2 slice)
+  if ((rc = make_token_map(ctx, &mWh, ctx->Wq, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, 64)) != TTT_OK) return rc;
   int n_items = c.nh * ntt * nsl;
   int grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
-  const size_t su = (size_t)lg::F_SMEM_U;
   int Mi = (int)M, nh = c.nh, hd = c.hd, H = c.hidden;
-  if (want_loss)
-    rc = launch_pdl(ctx, "ld_forward_kernel (update)", ld_forward_kernel<true, true>, grid, su, s, mK, mV, mW,
-                    mS0, mS1, mS2, lr, ctx->loss_part, Mi, nh, hd, H, n_items);
-  else
-    rc = launch_pdl(ctx, "ld_forward_kernel (update)", ld_forward_kernel<true, false>, grid, su, s, mK, mV, mW,
-                    mS0, mS1, mS2, lr, ctx->loss_part, Mi, nh, hd, H, n_items);
+  if (ctx->ld_pairs > 0) {
+    n_items = c.nh * ((ntt + 1) / 2) * nsl;          // items of a pair: two adjacent token tiles x one slice
+    grid = 2 * (n_items < ctx->ld_pairs ? n_items : ctx->ld_pairs);
+    if (want_loss)
+      rc = launch_pdl(ctx, "ld_forward_kernel (update, pairs)", ld_forward_kernel<true, true, true>, grid, (size_t)lg::P_SMEM_U, s, 2,
+                      mK, mV, mW, mWh, mS0, mS1, mS2, lr, ctx->loss_part, Mi, nh, hd, H, n_items);
+    else
+      rc = launch_pdl(ctx, "ld_forward_kernel (update, pairs)", ld_forward_kernel<true, false, true>, grid, (size_t)lg::P_SMEM_U, s, 2,
+                      mK, mV, mW, mWh, mS0, mS1, mS2, lr, ctx->loss_part, Mi, nh, hd, H, n_items);
+  } else if (want_loss) {
+    rc = launch_pdl(ctx, "ld_forward_kernel (update)", ld_forward_kernel<true, true, false>, grid, (size_t)lg::F_SMEM_U, s, 1,
+                    mK, mV, mW, mWh, mS0, mS1, mS2, lr, ctx->loss_part, Mi, nh, hd, H, n_items);
+  } else {
+    rc = launch_pdl(ctx, "ld_forward_kernel (update)", ld_forward_kernel<true, false, false>, grid, (size_t)lg::F_SMEM_U, s, 1,
+                    mK, mV, mW, mWh, mS0, mS1, mS2, lr, ctx->loss_part, Mi, nh, hd, H, n_items);
+  }
   if (rc != TTT_OK) return rc;
   *loss_rows = ntt * nsl;
   n_items = 3 * c.nh * nsl * (c.hd / lg::TN);
@@ -504,7 +586,7 @@ int bf16_large_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloa
   int accumulate = ctx->G_valid ? 1 : 0;
   __nv_bfloat16* nullo = nullptr;
   int64_t ldo = 0;
-  rc = launch_pdl(ctx, "ld_mn_gemm_kernel (gradient)", ld_mn_gemm_kernel<true>, grid, sm, s, mA0, mA1, mA2, mK64, mV64,
+  rc = launch_pdl(ctx, "ld_mn_gemm_kernel (gradient)", ld_mn_gemm_kernel<true>, grid, sm, s, 1, mA0, mA1, mA2, mK64, mV64,
                   ctx->G, nullo, ldo, Mi, nh, hd, H, n_items, accumulate);
   if (rc != TTT_OK) return rc;
   ctx->G_valid = true;
@@ -525,18 +607,24 @@ int bf16_large_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int
   const int ntt = (int)((M + lg::TM - 1) / lg::TM), nsl = c.hidden / lg::TM;
   int n_items = c.nh * ntt * nsl;
   int grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
-  const size_t sa = (size_t)lg::F_SMEM_A;
   int Mi = (int)M, nh = c.nh, hd = c.hd, H = c.hidden;
   const float* nolr = nullptr;
   float* nof = nullptr;
-  rc = launch_pdl(ctx, "ld_forward_kernel (apply)", ld_forward_kernel<false, false>, grid, sa, s, mQ, mQ, mW,
-                  mHq, mHq, mHq, nolr, nof, Mi, nh, hd, H, n_items);
+  if (ctx->ld_pairs > 0) {
+    n_items = c.nh * ((ntt + 1) / 2) * nsl;
+    grid = 2 * (n_items < ctx->ld_pairs ? n_items : ctx->ld_pairs);
+    rc = launch_pdl(ctx, "ld_forward_kernel (apply, pairs)", ld_forward_kernel<false, false, true>, grid, (size_t)lg::P_SMEM_A, s, 2,
+                    mQ, mQ, mW, mW64, mHq, mHq, mHq, nolr, nof, Mi, nh, hd, H, n_items);
+  } else {
+    rc = launch_pdl(ctx, "ld_forward_kernel (apply)", ld_forward_kernel<false, false, false>, grid, (size_t)lg::F_SMEM_A, s, 1,
+                    mQ, mQ, mW, mW64, mHq, mHq, mHq, nolr, nof, Mi, nh, hd, H, n_items);
+  }
   if (rc != TTT_OK) return rc;
   n_items = c.nh * ntt * (c.hd / lg::TN);
   grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
   const size_t sm = (size_t)lg::M_STAGE * lg::M_STAGES + 1024;
   int accumulate = 0;
-  return launch_pdl(ctx, "ld_mn_gemm_kernel (down projection)", ld_mn_gemm_kernel<false>, grid, sm, s, mHq, mHq, mHq,
+  return launch_pdl(ctx, "ld_mn_gemm_kernel (down projection)", ld_mn_gemm_kernel<false>, grid, sm, s, 1, mHq, mHq, mHq,
                     mW64, mW64, nof, O, ld, Mi, nh, hd, H, n_items, accumulate);
 }
 

@@ -91,6 +91,7 @@ struct ttt_ctx {
   size_t attr_smem_apply, attr_smem_ns;   // high-water marks of the kernels with a shape-dependent size
   int max_pairs;               // hd = 128 apply: co-resident CTA pairs (0 = not queried yet, < 0 = none)
   int upd_coop_ctas;           // hd = 64 update: co-resident CTAs of the cooperative launch (0 = not queried)
+  int ld_pairs;                // large-dimension path: co-resident CTA pairs of the forward kernel (0 = use single CTAs)
 };
 enum { ATTR_UPD = 1, ATTR_UPD_LOSS = 2, ATTR_UPDW = 4, ATTR_APPW = 8, ATTR_NSW = 16, ATTR_NS_F32 = 32,
        ATTR_LARGE = 64 };
