@@ -45,6 +45,7 @@ constexpr int F_SMEM_U = F_STAGES_U * F_STAGE + 3 * BOX + 1024, F_SMEM_A = F_STA
 // CTA-pair variant: a stage is the CTA's token chunk + its HALF of the weight rows = 32 KB
 constexpr int P_STAGES_U = 5, P_STAGES_A = 6;
 constexpr int P_SMEM_U = P_STAGES_U * 2 * BOX + 3 * BOX + 1024, P_SMEM_A = P_STAGES_A * 2 * BOX + BOX + 1024;
+constexpr int P_SMEM_M = 6 * 2 * BOX + 1024;
 constexpr uint32_t C_XB = 0, C_G = 256;                // x | b [128 x 256] fp32; g0 [128 x 128] fp32, two buffers
 // MN-major-B kernels: stage = A 16 KB + B 32 KB, two accumulators [128 x 256] fp32
 constexpr int M_STAGE = 3 * BOX, M_STAGES = 4;
@@ -326,8 +327,11 @@ ld_forward_kernel(const __grid_constant__ CUtensorMap mapX, const __grid_constan
 //   DOWN:         tile (token tile tt, hd block nb, head h), contraction over H;
 //                 A = Hq [tokens][hidden] (K-major), B = W2 rows [hidden][hd]; out: O bf16
 // Accumulators are double-buffered in TMEM: the epilogue of a tile overlaps the next tile's main loop.
+// PAIR: CTA pairs (cta_group::2, M = 256) as in the forward kernel: two adjacent row blocks (hidden blocks /
+// token tiles) share the B operand, rank r loading output columns 128 r .. 128 r + 127 of it (ncu, single
+// CTAs: shared-memory pipe 92 % busy in the gradient GEMM).
 // ------------------------------------------------------------------------------------------------
-template <bool GRAD>
+template <bool GRAD, bool PAIR>
 __global__ void __launch_bounds__(lg::THREADS, 1)
 ld_mn_gemm_kernel(const __grid_constant__ CUtensorMap mapA0, const __grid_constant__ CUtensorMap mapA1,
                   const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ CUtensorMap mapB0,
@@ -338,21 +342,34 @@ ld_mn_gemm_kernel(const __grid_constant__ CUtensorMap mapA0, const __grid_consta
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
-  __shared__ uint64_t full[M_STAGES], empty[M_STAGES], acc_full[2], acc_empty[2];
+  constexpr int STAGE = PAIR ? 2 * BOX : M_STAGE;           // pairs: A 16 KB + the CTA's half of B 16 KB
+  constexpr int STAGES = PAIR ? 6 : M_STAGES;
+  __shared__ uint64_t full[STAGES], empty[STAGES], acc_full[2], acc_empty[2];
   __shared__ uint32_t tmem_base_s;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const uint32_t rank = PAIR ? cluster_rank() : 0u;
+  const int cta0 = PAIR ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
+  const int ncta = PAIR ? (int)(gridDim.x >> 1) : (int)gridDim.x;
   const int nnb = hd / TN;                                  // hd blocks of 256
   const int nhb = H / TM, ntt = (M + TM - 1) / TM;
+  const int nrb = GRAD ? nhb : ntt;                         // row blocks; pairs take two adjacent ones
+  const int nrr = PAIR ? (nrb + 1) / 2 : nrb;
   const int nkc = GRAD ? (M + KC - 1) / KC : H / KC;
   if (tid == 0) {
-    for (int s = 0; s < M_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(&acc_full[b], 1); mbar_init(&acc_empty[b], EPI_WARPS); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&acc_full[b], 1); mbar_init(&acc_empty[b], (PAIR ? 2 : 1) * EPI_WARPS); }
     fence_mbar_init();
     tma_prefetch_desc(&mapA0);
     tma_prefetch_desc(&mapB0);
   }
-  if (warp == 2) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  if (PAIR) {
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == 2) { tmem_alloc2(&tmem_base_s, 512); tmem_relinquish2(); }
+  } else {
+    if (warp == 2) { tmem_alloc(&tmem_base_s, 512); tmem_relinquish(); }
+  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -360,27 +377,45 @@ ld_mn_gemm_kernel(const __grid_constant__ CUtensorMap mapA0, const __grid_consta
   asm volatile("griddepcontrol.wait;" ::: "memory");
 
   // GRAD: id -> (j, h, hb, nb), nb fastest (the four hd blocks of a hidden block share their A stream);
-  // DOWN: id -> (h, tt, nb)
+  // DOWN: id -> (h, tt, nb). A pair's rank 1 may get a row block one past the end (odd count): it runs the
+  // MMAs with whatever the loads return and stores nothing.
   auto item = [&](int id, int& j, int& h, int& rb, int& nb) {
     nb = id % nnb;
     int r = id / nnb;
-    if (GRAD) { rb = r % nhb; r /= nhb; h = r % nh; j = r / nh; }
-    else { rb = r % ntt; h = r / ntt; j = 0; }
+    rb = PAIR ? 2 * (r % nrr) + (int)rank : r % nrr;
+    r /= nrr;
+    if (GRAD) { h = r % nh; j = r / nh; }
+    else { h = r; j = 0; }
   };
 
   if (warp == 0) {
     if (elect_one()) {
       int g = 0;
-      for (int id = blockIdx.x; id < n_items; id += gridDim.x) {
+      for (int id = cta0; id < n_items; id += ncta) {
         int j, h, rb, nb;
         item(id, j, h, rb, nb);
         const CUtensorMap* mA = GRAD ? (j == 0 ? &mapA0 : j == 1 ? &mapA2 : &mapA1) : &mapA0;   // dA, Hd', dB
         const CUtensorMap* mB = GRAD ? (j == 1 ? &mapB1 : &mapB0) : &mapB0;                      // K | V ; W2 rows
         for (int kc = 0; kc < nkc; ++kc, ++g) {
-          const int st = g % M_STAGES;
-          if (g >= M_STAGES) mbar_wait(&empty[st], ((g / M_STAGES) - 1) & 1);
+          const int st = g % STAGES;
+          if (g >= STAGES) mbar_wait(&empty[st], ((g / STAGES) - 1) & 1);
+          uint8_t* dst = smem + st * STAGE;
+          if (PAIR) {
+            const uint32_t bar = mapa_u32(&full[st], 0);
+            if (rank == 0) mbar_arrive_expect_tx(&full[st], 4 * BOX);
+            if (GRAD) {
+              tma_load_2d_pair(dst, mA, bar, h * H + rb * TM, kc * KC);
+              tma_load_2d_pair(dst + BOX / 2, mA, bar, h * H + rb * TM + 64, kc * KC);
+              for (int a = 0; a < 2; ++a)               // this CTA's two of the four hd atoms
+                tma_load_2d_pair(dst + BOX + a * (BOX / 2), mB, bar, h * hd + nb * TN + 128 * (int)rank + 64 * a, kc * KC);
+            } else {
+              tma_load_2d_pair(dst, mA, bar, h * H + kc * KC, rb * TM);
+              for (int a = 0; a < 2; ++a)
+                tma_load_2d_pair(dst + BOX + a * (BOX / 2), mB, bar, nb * TN + 128 * (int)rank + 64 * a, (1 * nh + h) * H + kc * KC);
+            }
+            continue;
+          }
           mbar_arrive_expect_tx(&full[st], M_STAGE);
-          uint8_t* dst = smem + st * M_STAGE;
           if (GRAD) {
             // A: two [64 tokens x 64 hidden] atoms (hidden halves of the block)
             tma_load_2d(dst, mA, &full[st], h * H + rb * TM, kc * KC);
@@ -397,37 +432,40 @@ ld_mn_gemm_kernel(const __grid_constant__ CUtensorMap mapA0, const __grid_consta
       }
     }
   } else if (warp == 1) {
-    if (elect_one()) {
-      constexpr uint32_t idesc = umma_idesc_bf16(TM, TN, GRAD ? 1 : 0, 1);
+    if (rank == 0 && elect_one()) {
+      constexpr uint32_t idesc = umma_idesc_bf16(PAIR ? 2 * TM : TM, TN, GRAD ? 1 : 0, 1);
       const uint64_t dA = GRAD ? umma_smem_desc_sw128(sbase, BOX / 2, 1024) : umma_smem_desc_sw128(sbase, 16, 1024);
       const uint64_t dB = umma_smem_desc_sw128(sbase + BOX, BOX / 2, 1024);
       int g = 0, n = 0;
-      for (int id = blockIdx.x; id < n_items; id += gridDim.x, ++n) {
+      for (int id = cta0; id < n_items; id += ncta, ++n) {
         const int ab = n & 1;
         if (n >= 2) { mbar_wait(&acc_empty[ab], ((n >> 1) - 1) & 1); tc_fence_after(); }
         const uint32_t acc = tb + ab * TN;
         for (int kc = 0; kc < nkc; ++kc, ++g) {
-          const int st = g % M_STAGES;
-          mbar_wait(&full[st], (g / M_STAGES) & 1);
+          const int st = g % STAGES;
+          mbar_wait(&full[st], (g / STAGES) & 1);
           tc_fence_after();
-          const uint64_t so = (uint64_t)(st * (M_STAGE >> 4));
+          const uint64_t so = (uint64_t)(st * (STAGE >> 4));
 #pragma unroll
-          for (int k = 0; k < KC / 16; ++k)            // MN-major: +2048 B per 16-row K step; K-major: +32 B
-            umma_ss(acc, dA + so + (GRAD ? 128 * k : 2 * k), dB + so + 128 * k, idesc, (kc > 0) | k);
-          tc_commit(&empty[st]);
+          for (int k = 0; k < KC / 16; ++k) {          // MN-major: +2048 B per 16-row K step; K-major: +32 B
+            if (PAIR) umma_ss2(acc, dA + so + (GRAD ? 128 * k : 2 * k), dB + so + 128 * k, idesc, (kc > 0) | k);
+            else umma_ss(acc, dA + so + (GRAD ? 128 * k : 2 * k), dB + so + 128 * k, idesc, (kc > 0) | k);
+          }
+          if (PAIR) tc_commit2(&empty[st]); else tc_commit(&empty[st]);
         }
-        tc_commit(&acc_full[ab]);
+        if (PAIR) tc_commit2(&acc_full[ab]); else tc_commit(&acc_full[ab]);
       }
     }
   } else if (warp >= 4) {
     const int q = warp & 3, half = (warp - 4) >> 2;
     const uint32_t lane_base = static_cast<uint32_t>(q * 32) << 16;
     int n = 0;
-    for (int id = blockIdx.x; id < n_items; id += gridDim.x, ++n) {
+    for (int id = cta0; id < n_items; id += ncta, ++n) {
       int j, h, rb, nb;
       item(id, j, h, rb, nb);
       const int ab = n & 1;
       const int row = rb * TM + q * 32 + lane;
+      const bool live = rb < nrb;                      // (a pair's rank 1 one past the last row block)
       mbar_wait(&acc_full[ab], (n >> 1) & 1);
       tc_fence_after();
 #pragma unroll 1
@@ -436,6 +474,7 @@ ld_mn_gemm_kernel(const __grid_constant__ CUtensorMap mapA0, const __grid_consta
         tmem_ld_x32(tb + lane_base + ab * TN + 128 * half + 32 * c, r);
         tc_wait_ld();
         const int col = nb * TN + 128 * half + 32 * c;
+        if (!live) continue;
         if (GRAD) {
           float4* dst = reinterpret_cast<float4*>(G + (((size_t)j * nh + h) * H + row) * hd + col);
 #pragma unroll
@@ -457,13 +496,20 @@ ld_mn_gemm_kernel(const __grid_constant__ CUtensorMap mapA0, const __grid_consta
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&acc_empty[ab]);
+      if (lane == 0) {
+        if (rank == 0) mbar_arrive(&acc_empty[ab]); else mbar_arrive_remote(&acc_empty[ab], 0);
+      }
     }
   }
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   tc_fence_before();
   __syncthreads();
-  if (warp == 2) tmem_dealloc(tb, 512);
+  if (PAIR) {
+    cluster_sync_all();
+    if (warp == 2) tmem_dealloc2(tb, 512);
+  } else {
+    if (warp == 2) tmem_dealloc(tb, 512);
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -530,8 +576,10 @@ static int large_attrs(ttt_ctx* ctx) {
     if (cudaOccupancyMaxActiveClusters(&n, ld_forward_kernel<true, false, true>, &cfg) != cudaSuccess) { n = 0; cudaGetLastError(); }
     ctx->ld_pairs = n;
   }
-  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_mn_gemm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "ld_mn_gemm smem attr");
-  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_mn_gemm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "ld_mn_gemm smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_mn_gemm_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "ld_mn_gemm smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_mn_gemm_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "ld_mn_gemm smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_mn_gemm_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lg::P_SMEM_M), "ld_mn_gemm smem attr");
+  TTT_CUDA_TRY(ctx, cudaFuncSetAttribute(ld_mn_gemm_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lg::P_SMEM_M), "ld_mn_gemm smem attr");
   ctx->attr_done |= ATTR_LARGE;
   return TTT_OK;
 }
@@ -580,14 +628,21 @@ int bf16_large_accumulate(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloa
   }
   if (rc != TTT_OK) return rc;
   *loss_rows = ntt * nsl;
-  n_items = 3 * c.nh * nsl * (c.hd / lg::TN);
-  grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
-  const size_t sm = (size_t)lg::M_STAGE * lg::M_STAGES + 1024;
   int accumulate = ctx->G_valid ? 1 : 0;
   __nv_bfloat16* nullo = nullptr;
   int64_t ldo = 0;
-  rc = launch_pdl(ctx, "ld_mn_gemm_kernel (gradient)", ld_mn_gemm_kernel<true>, grid, sm, s, 1, mA0, mA1, mA2, mK64, mV64,
-                  ctx->G, nullo, ldo, Mi, nh, hd, H, n_items, accumulate);
+  if (ctx->ld_pairs > 0) {
+    n_items = 3 * c.nh * ((nsl + 1) / 2) * (c.hd / lg::TN);
+    grid = 2 * (n_items < ctx->ld_pairs ? n_items : ctx->ld_pairs);
+    rc = launch_pdl(ctx, "ld_mn_gemm_kernel (gradient, pairs)", ld_mn_gemm_kernel<true, true>, grid, (size_t)lg::P_SMEM_M, s, 2,
+                    mA0, mA1, mA2, mK64, mV64, ctx->G, nullo, ldo, Mi, nh, hd, H, n_items, accumulate);
+  } else {
+    n_items = 3 * c.nh * nsl * (c.hd / lg::TN);
+    grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
+    rc = launch_pdl(ctx, "ld_mn_gemm_kernel (gradient)", ld_mn_gemm_kernel<true, false>, grid,
+                    (size_t)lg::M_STAGE * lg::M_STAGES + 1024, s, 1, mA0, mA1, mA2, mK64, mV64,
+                    ctx->G, nullo, ldo, Mi, nh, hd, H, n_items, accumulate);
+  }
   if (rc != TTT_OK) return rc;
   ctx->G_valid = true;
   return TTT_OK;
@@ -620,11 +675,17 @@ int bf16_large_apply(ttt_ctx* ctx, const __nv_bfloat16* Q, __nv_bfloat16* O, int
                     mQ, mQ, mW, mW64, mHq, mHq, mHq, nolr, nof, Mi, nh, hd, H, n_items);
   }
   if (rc != TTT_OK) return rc;
+  int accumulate = 0;
+  if (ctx->ld_pairs > 0) {
+    n_items = c.nh * ((ntt + 1) / 2) * (c.hd / lg::TN);
+    grid = 2 * (n_items < ctx->ld_pairs ? n_items : ctx->ld_pairs);
+    return launch_pdl(ctx, "ld_mn_gemm_kernel (down projection, pairs)", ld_mn_gemm_kernel<false, true>, grid,
+                      (size_t)lg::P_SMEM_M, s, 2, mHq, mHq, mHq, mW64, mW64, nof, O, ld, Mi, nh, hd, H, n_items, accumulate);
+  }
   n_items = c.nh * ntt * (c.hd / lg::TN);
   grid = n_items < ctx->sm_count ? n_items : ctx->sm_count;
-  const size_t sm = (size_t)lg::M_STAGE * lg::M_STAGES + 1024;
-  int accumulate = 0;
-  return launch_pdl(ctx, "ld_mn_gemm_kernel (down projection)", ld_mn_gemm_kernel<false>, grid, sm, s, 1, mHq, mHq, mHq,
+  return launch_pdl(ctx, "ld_mn_gemm_kernel (down projection)", ld_mn_gemm_kernel<false, false>, grid,
+                    (size_t)lg::M_STAGE * lg::M_STAGES + 1024, s, 1, mHq, mHq, mHq,
                     mW64, mW64, nof, O, ld, Mi, nh, hd, H, n_items, accumulate);
 }
 
