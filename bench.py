@@ -43,7 +43,7 @@ HEADLINE = "cfg5"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the workload's dominant kernel, from the
 # `ncu --set full` captures summarised under profiles/ (file and commit named per entry)
-_CAP = "profiles/r02_ncu_full.md (commit 5afd7f3), capture "
+_CAP = "profiles/r02_ncu_full.md (commits 5afd7f3 / 3d966e7), capture "
 TRAFFIC = {
     "cfg2": {"bytes": 48692992, "capture": _CAP + "r02_cfg2_update"},
     # cfg3's dominant kernel is cfg4's (same grid, 86 instead of 344 tiles per CTA): bytes scaled from the
@@ -51,7 +51,7 @@ TRAFFIC = {
     "cfg3": {"bytes": int(191860736 * 10992 / 43968), "capture": _CAP + "r02_cfg4_update, scaled by tokens"},
     "cfg4": {"bytes": 191860736, "capture": _CAP + "r02_cfg4_update"},
     "cfg5": {"bytes": 196604672, "capture": _CAP + "r02_cfg5_update"},
-    "paper_k4": {"bytes": 2360389720 + 2915659568,
+    "paper_k4": {"bytes": 2872674800 + 4316396344,
                  "capture": _CAP + "r02_k4_forward (update) + r02_k4_mn (gradient): the two launches of ttt_accumulate"},
 }
 
