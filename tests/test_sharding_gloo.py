@@ -56,3 +56,45 @@ def test_head_sharding_world_size_2(tmp_path):
     ora = OracleTTT(W1, W2, W3, ns_iters=w.ns_iters)
     full = np.stack([ora.chunk_step(*c)[0] for c in ti.TokenStream(w)])
     np.testing.assert_array_equal(sharded, full)               # heads are bitwise independent
+
+
+# ------------------------------------------------------------------------------------------------
+# Eq. 10, the method's one exchange step: every rank takes the gradient of ITS
+# chunk at the shared W, the gradients are summed (all-reduce), every rank commits the same update. The
+# library keeps the update split for this (ttt_accumulate / ttt_pending_gradient / ttt_commit); here the
+# host-side plumbing is checked on CPU with the oracle standing in for the per-rank gradient kernel.
+# ------------------------------------------------------------------------------------------------
+def _gcs_worker(rank, world, port, out_dir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    w = ti.scaled(ti.CONFIGS["cfg2"], nh=2, tokens_per_frame=50, frames_per_chunk=1, n_frames=world)
+    W1, W2, W3 = ti.fast_weights(w)
+    chunks = list(ti.TokenStream(w))
+    Q, K, V, lr = chunks[rank]                                 # one chunk per rank
+    ora = OracleTTT(W1, W2, W3)
+    G = [torch.from_numpy(g) for g in ora.grad(K, V, lr)[:3]]  # = ttt_accumulate + ttt_pending_gradient
+    flat = torch.cat([g.reshape(-1) for g in G])
+    dist.all_reduce(flat, op=dist.ReduceOp.SUM)                # Eq. 10: g = sum over ranks
+    ofs, new = 0, []
+    for Wm, g in zip((W1, W2, W3), G):                         # = ttt_commit, identical on every rank
+        new.append(Wm.double() - flat[ofs:ofs + g.numel()].reshape(g.shape))
+        ofs += g.numel()
+    np.save(os.path.join(out_dir, f"w_rank{rank}.npy"), torch.cat([x.reshape(-1) for x in new]).numpy())
+    dist.destroy_process_group()
+
+
+def test_gradient_allreduce_equals_one_update_on_all_chunks(tmp_path):
+    world = 2
+    mp.spawn(_gcs_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    w = ti.scaled(ti.CONFIGS["cfg2"], nh=2, tokens_per_frame=50, frames_per_chunk=1, n_frames=world)
+    W1, W2, W3 = ti.fast_weights(w)
+    chunks = list(ti.TokenStream(w))
+    ora = OracleTTT(W1, W2, W3)
+    K = torch.cat([c[1] for c in chunks]); V = torch.cat([c[2] for c in chunks])
+    lr = torch.cat([c[3] for c in chunks], dim=1)
+    ora.update(K, V, lr)                                       # one update on the concatenation of all chunks
+    expect = np.concatenate([x.reshape(-1) for x in ora.weights()])
+    r0, r1 = np.load(tmp_path / "w_rank0.npy"), np.load(tmp_path / "w_rank1.npy")
+    np.testing.assert_array_equal(r0, r1)                      # every rank holds the same memory afterwards
+    np.testing.assert_allclose(r0, expect, rtol=0, atol=1e-12)
