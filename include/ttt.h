@@ -54,17 +54,23 @@ typedef enum {
 typedef enum {
   TTT_F32 = 0,  /* Q,K,V,O fp32; every contraction in fp32 FFMA (parity config 1, tol 1e-4)   */
   TTT_BF16 = 1  /* Q,K,V,O bf16, fp32 master weights, tcgen05 MMAs with fp32 accumulation. Shapes the
-                   tensor kernels take: hd = 64 with hidden 128|256, hd = 128 with hidden a multiple
-                   of 128 (<= 1024 with Newton-Schulz). Any other shape: ttt_create returns
-                   TTT_ERR_UNSUPPORTED, unless cfg.cuda_core_fallback = 1 asks for the fp32 CUDA-core
-                   kernels behind a bf16 <-> fp32 conversion (hd % 8 == 0; same semantics, ~40x slower).
-                   Token values are MMA operands as fp16 (converted on chip, exact for magnitudes in
-                   [2^-14, 65504]; smaller ones keep an absolute error <= 2^-25, larger ones clamp) */
+                   tensor kernels take: hd = 64 with hidden <= 256; hd = 128 with any hidden
+                   (<= 1024 with Newton-Schulz) — a hidden size that is not a multiple of 128 runs
+                   zero-padded to the next one; hd a multiple of 256 up to 2048 with hidden a
+                   multiple of 128 and ns_iters = renorm = 0 (the paper's own shape: nh = 1, hd = 1024,
+                   hidden 1024..4096; three bf16 activation arrays of
+                   max_tokens x nh x hidden are allocated). Any other shape with hd <= 128: ttt_create
+                   returns TTT_ERR_UNSUPPORTED, unless cfg.cuda_core_fallback = 1 asks for the fp32
+                   CUDA-core kernels behind a bf16 <-> fp32 conversion (hd % 8 == 0; same semantics,
+                   ~40x slower); hd > 128 otherwise: TTT_ERR_SHAPE.
+                   hd 64 / 128: token values are MMA operands as fp16 (converted on chip, exact for
+                   magnitudes in [2^-14, 65504]; smaller ones keep an absolute error <= 2^-25, larger
+                   ones clamp); hd >= 256: bf16 operands throughout. */
 } ttt_dtype;
 
 typedef struct {
   int32_t nh;                 /* heads (independent fast-weight sets, Eq. 13)    */
-  int32_t hd;                 /* head dimension <= 128; bf16: multiple of 8; f32: multiple of 4 */
+  int32_t hd;                 /* head dimension: f32 <= 128, multiple of 4; bf16 see ttt_dtype    */
   int32_t hidden;             /* H = hd*k, multiple of 4 (tensor paths: see ttt_dtype)           */
   int32_t act_dtype;          /* ttt_dtype of Q,K,V,O                                          */
   int32_t ns_iters;           /* 0 = plain gradient step (Eq. 8); n>0 = n Newton-Schulz iters  */
@@ -124,7 +130,9 @@ int ttt_accumulate(ttt_ctx* ctx, const void* K, const void* V, const float* lr, 
 int ttt_commit(ttt_ctx* ctx, void* stream);
 
 /* Reduce the pending partial gradients into one dense DEVICE buffer owned by the context and
- * return it: [3][nh][H][hd] fp32 = (G1^T, G2, G3^T) in the hidden-major layout the kernels use.
+ * return it: [3][nh][H'][hd] fp32 = (G1^T, G2, G3^T) in the hidden-major layout the kernels use
+ * (H' = *n_elements / (3 nh hd): H, or — bf16 tensor path with hd 64 | 128 and H not a multiple of
+ * 128 — H rounded up to one; the padded hidden units' rows are zero).
  * After the caller has modified it in place (e.g. ncclAllReduce), ttt_commit uses it as is. */
 int ttt_pending_gradient(ttt_ctx* ctx, float** G, int64_t* n_elements, void* stream);
 

@@ -159,12 +159,13 @@ class TTT:
         self._check(self._lib.ttt_commit(self._ctx, self._stream()), "ttt_commit")
 
     def ttt_pending_gradient(self) -> torch.Tensor:
-        """Borrowed view [3, nh, H, hd] fp32 of the context-owned dense pending gradient."""
+        """Borrowed view [3, nh, H', hd] fp32 of the context-owned dense pending gradient (H' = H, or H
+        rounded up to a multiple of 128 where the tensor path pads the hidden units; the pad rows are 0)."""
         p, n = ctypes.c_void_p(), ctypes.c_int64()
         self._check(self._lib.ttt_pending_gradient(self._ctx, ctypes.byref(p), ctypes.byref(n),
                                                    self._stream()), "ttt_pending_gradient")
         c = self.cfg
-        shape = (3, c.nh, c.hidden, c.hd)
+        shape = (3, c.nh, n.value // (3 * c.nh * c.hd), c.hd)
 
         class _Arr:  # __cuda_array_interface__ carrier: zero-copy view of library-owned memory
             __cuda_array_interface__ = {"shape": shape, "typestr": "<f4", "data": (p.value, False),

@@ -37,7 +37,8 @@ __device__ __forceinline__ float warp_sum(float v) {
 __global__ void init_load_kernel(const float* __restrict__ W1, const float* __restrict__ W2,
                                  const float* __restrict__ W3, float* __restrict__ Wm,
                                  ttt_wop_t* __restrict__ Wb, __nv_bfloat16* __restrict__ Wq,
-                                 float* __restrict__ n0, float* __restrict__ colsq, int nh, int hd, int H) {
+                                 float* __restrict__ n0, float* __restrict__ colsq, int nh, int hd, int H,
+                                 int Hu) {   // Hu = the caller's hidden size (rows Hu .. H-1 are zero padding)
   __shared__ float tile[32][33];
   __shared__ float cs[8][128];
   const int mat = blockIdx.z, h = blockIdx.y, j0 = blockIdx.x * 32;
@@ -47,7 +48,7 @@ __global__ void init_load_kernel(const float* __restrict__ W1, const float* __re
   ttt_wop_t* dstb = Wb + mat * me + (size_t)h * H * hd;
   __nv_bfloat16* dstq = Wq ? Wq + mat * me + (size_t)h * H * hd : nullptr;
   if (mat == 1) {  // W2 [H][hd]: straight copy + column sums of squares over this CTA's rows
-    const float* src = W2 + (size_t)h * H * hd;
+    const float* src = W2 + (size_t)h * Hu * hd;
     for (int cb = 0; cb < hd; cb += 128) {           // 128 columns at a time (hd > 128: the paper's shape)
       float colacc[4] = {0.f, 0.f, 0.f, 0.f};
       for (int r = ty; r < 32; r += 8) {
@@ -57,7 +58,7 @@ __global__ void init_load_kernel(const float* __restrict__ W1, const float* __re
         for (int c = 0; c < 4; ++c) {
           const int i = cb + tx + 32 * c;
           if (i < hd) {
-            const float v = src[(size_t)j * hd + i];
+            const float v = j < Hu ? src[(size_t)j * hd + i] : 0.f;
             dst[(size_t)j * hd + i] = v;
             dstb[(size_t)j * hd + i] = ttt_to_wop(v);
             if (dstq) dstq[(size_t)j * hd + i] = __float2bfloat16_rn(v);
@@ -77,12 +78,12 @@ __global__ void init_load_kernel(const float* __restrict__ W1, const float* __re
     }
     return;
   }
-  const float* src = (mat == 0 ? W1 : W3) + (size_t)h * hd * H;  // [hd][H]
+  const float* src = (mat == 0 ? W1 : W3) + (size_t)h * hd * Hu;  // [hd][Hu]
   float rowacc[4] = {0.f, 0.f, 0.f, 0.f};                        // rows j0 + ty + 8k
   for (int i0 = 0; i0 < hd; i0 += 32) {
     for (int r = ty; r < 32; r += 8) {
       const int i = i0 + r, j = j0 + tx;
-      tile[r][tx] = (i < hd && j < H) ? src[(size_t)i * H + j] : 0.f;
+      tile[r][tx] = (i < hd && j < Hu) ? src[(size_t)i * Hu + j] : 0.f;
     }
     __syncthreads();
 #pragma unroll
@@ -121,21 +122,21 @@ __global__ void init_colnorm_kernel(const float* __restrict__ colsq, float* __re
 // ttt_get_weights: hidden-major masters -> user layout. Same tiling as init_load_kernel.
 __global__ void get_weights_kernel(const float* __restrict__ Wm, float* __restrict__ W1,
                                    float* __restrict__ W2, float* __restrict__ W3, int nh, int hd,
-                                   int H) {
+                                   int H, int Hu) {
   __shared__ float tile[32][33];
   const int mat = blockIdx.z, h = blockIdx.y, j0 = blockIdx.x * 32;
   const size_t me = (size_t)nh * H * hd;
   const float* src = Wm + mat * me + (size_t)h * H * hd;
   if (mat == 1) {
-    float* dst = W2 + (size_t)h * H * hd;
+    float* dst = W2 + (size_t)h * Hu * hd;
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
       int j = j0 + r;
-      if (j >= H) break;
+      if (j >= Hu) break;
       for (int i = threadIdx.x; i < hd; i += 32) dst[(size_t)j * hd + i] = src[(size_t)j * hd + i];
     }
     return;
   }
-  float* dst = (mat == 0 ? W1 : W3) + (size_t)h * hd * H;
+  float* dst = (mat == 0 ? W1 : W3) + (size_t)h * hd * Hu;
   for (int i0 = 0; i0 < hd; i0 += 32) {
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
       int j = j0 + r, i = i0 + threadIdx.x;
@@ -144,7 +145,7 @@ __global__ void get_weights_kernel(const float* __restrict__ Wm, float* __restri
     __syncthreads();
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
       int i = i0 + r, j = j0 + threadIdx.x;
-      if (i < hd && j < H) dst[(size_t)i * H + j] = tile[threadIdx.x][r];
+      if (i < hd && j < Hu) dst[(size_t)i * Hu + j] = tile[threadIdx.x][r];
     }
     __syncthreads();
   }
@@ -396,7 +397,7 @@ int launch_init(ttt_ctx* ctx, const float* W1, const float* W2, const float* W3,
   const ttt_config& c = ctx->cfg;
   dim3 grid((c.hidden + 31) / 32, c.nh, 3), block(32, 8);
   init_load_kernel<<<grid, block, 0, s>>>(W1, W2, W3, ctx->Wm, ctx->Wb, ctx->Wq, ctx->n0, ctx->colsq, c.nh,
-                                          c.hd, c.hidden);
+                                          c.hd, c.hidden, ctx->user_hidden);
   TTT_LAUNCH_CHECK(ctx, "init_load_kernel");
   init_colnorm_kernel<<<c.nh, 128, 0, s>>>(ctx->colsq, ctx->n0, (int)grid.x, c.nh, c.hd, c.hidden);
   TTT_LAUNCH_CHECK(ctx, "init_colnorm_kernel");
@@ -406,7 +407,7 @@ int launch_init(ttt_ctx* ctx, const float* W1, const float* W2, const float* W3,
 int launch_get_weights(ttt_ctx* ctx, float* W1, float* W2, float* W3, cudaStream_t s) {
   const ttt_config& c = ctx->cfg;
   dim3 grid((c.hidden + 31) / 32, c.nh, 3), block(32, 8);
-  get_weights_kernel<<<grid, block, 0, s>>>(ctx->Wm, W1, W2, W3, c.nh, c.hd, c.hidden);
+  get_weights_kernel<<<grid, block, 0, s>>>(ctx->Wm, W1, W2, W3, c.nh, c.hd, c.hidden, ctx->user_hidden);
   TTT_LAUNCH_CHECK(ctx, "get_weights_kernel");
   return TTT_OK;
 }

@@ -161,6 +161,15 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
     return create_fail(TTT_ERR_SHAPE, "linear test mode needs hidden == hd");
   if (cfg->ns_iters > 0 && cfg->hidden < cfg->hd)
     return create_fail(TTT_ERR_UNSUPPORTED, "Newton-Schulz needs hidden >= hd");
+  // hd 64 | 128 on the tensor path: a hidden size that is not a multiple of 128 (k = 1 at hd 64: H = 64) runs
+  // as the next multiple with zero-padded hidden units
+  const ttt_config* ucfg = cfg;
+  ttt_config eff = *cfg;
+  if (cfg->act_dtype == TTT_BF16 && !cfg->cuda_core_fallback && !cfg->linear_fast_weight &&
+      (cfg->hd == 64 || cfg->hd == 128) && cfg->hidden % 128 != 0) {
+    eff.hidden = (cfg->hidden + 127) / 128 * 128;
+    if (bf16_update_tensor_path(&eff) && bf16_apply_tensor_path(&eff)) cfg = &eff;
+  }
   if (cfg->act_dtype == TTT_BF16) {
     char why[200];
     if (!bf16_supported(cfg, why, sizeof(why))) return create_fail(TTT_ERR_UNSUPPORTED, why);
@@ -190,6 +199,7 @@ int ttt_create(ttt_ctx** out, const ttt_config* cfg) {
   if (!ctx) return create_fail(TTT_ERR_NOMEM, "out of host memory");
   memset(ctx, 0, sizeof(*ctx));
   ctx->cfg = *cfg;
+  ctx->user_hidden = ucfg->hidden;
   ctx->sm_count = prop.multiProcessorCount;
   ctx->mat_elems = (size_t)cfg->nh * cfg->hidden * cfg->hd;
   const size_t set = 3 * ctx->mat_elems;

@@ -39,7 +39,10 @@ __device__ __forceinline__ ttt_wop_t ttt_to_wop(float v) {
 // Element (mat, h, j, i) lives at ((mat*nh + h)*H + j)*hd + i, in the fp32 master `Wm`, the bf16
 // operand copy `Wb`, the dense gradient `G` and every partial-gradient set.
 struct ttt_ctx {
-  ttt_config cfg;
+  ttt_config cfg;        // as the kernels see it: cfg.hidden is the PADDED hidden size (below)
+  int user_hidden;       // the caller's H. bf16 tensor path with hd 64 | 128: H is padded to a multiple of 128
+                         // with zero weight rows (zero units: x = b = g = 0, so their gradients and outputs
+                         // vanish and the rows stay zero); ttt_init / ttt_get_weights translate
   int sm_count;
   bool initialised;
   int64_t launches;

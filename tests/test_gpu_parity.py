@@ -463,6 +463,24 @@ def test_long_stream_is_stable_and_per_chunk_time_is_flat():
     g.close()
 
 
+@pytest.mark.parametrize("hd,H,ns,renorm", [
+    (64, 64, 0, 0),       # k = 1 of Eq. 13's sweep at hd 64: runs as 128 padded hidden units
+    (64, 64, 5, 0),       # ... with Newton-Schulz (square gradient matrices)
+    (64, 192, 0, 1),      # padded to 256, re-normalisation (pad rows have norm 0 and stay 0)
+    (128, 320, 5, 0),     # hd 128 kernels, padded to 384
+])
+def test_bf16_hidden_sizes_padded_to_128(hd, H, ns, renorm):
+    w = _bf16_workload("cfg2", nh=2, hd=hd, hidden=H, ns_iters=ns, renorm=renorm, tokens_per_frame=171,
+                       frames_per_chunk=2, n_frames=6)
+    gpu = _mk(w)
+    assert gpu.kernel_path() == (True, True)
+    gpu.close()
+    errs_o, errs_w, errs_l = _run_stream(w)
+    assert max(errs_o) <= TOL_BF16, errs_o
+    assert max(errs_w) <= TOL_BF16, errs_w
+    assert max(errs_l) <= TOL_LOSS_BF16, errs_l
+
+
 # ------------------------------------------------------------------------------------------------
 # boundary: no silent CUDA-core fallback
 # ------------------------------------------------------------------------------------------------
