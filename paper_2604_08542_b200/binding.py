@@ -172,6 +172,16 @@ class TTT:
                                         "version": 3, "strides": None}
         return torch.as_tensor(_Arr(), device=self.device)
 
+    def allreduce_pending_gradient(self, group=None) -> torch.Tensor:
+        """Eq. 10, the method's one exchange step: sum the pending fast-weight
+        gradient over the ranks of `group` IN PLACE (one NCCL all-reduce over the dense buffer that
+        ttt_pending_gradient returns, over NVLink / NVSwitch), so that the ttt_commit that follows applies the
+        same update on every rank. Plumbing only: torch.distributed carries the library's own buffer."""
+        import torch.distributed as dist
+        G = self.ttt_pending_gradient()
+        dist.all_reduce(G.view(-1), op=dist.ReduceOp.SUM, group=group)
+        return G
+
     def ttt_apply(self, Q, O: Optional[torch.Tensor] = None) -> torch.Tensor:
         M, ld = self._tok(Q, "Q")
         if O is None:

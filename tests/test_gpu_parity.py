@@ -481,6 +481,37 @@ def test_bf16_hidden_sizes_padded_to_128(hd, H, ns, renorm):
     assert max(errs_l) <= TOL_LOSS_BF16, errs_l
 
 
+def test_gradient_allreduce_between_accumulate_and_commit_nccl():
+    """Eq. 10 on the product path: ttt_accumulate -> NCCL all-reduce of the pending gradient -> ttt_commit.
+    One GPU here, so the process group has one rank (the sum is the identity) — what is exercised is the
+    call sequence on the library's own device buffer; the two-rank arithmetic is covered on CPU
+    (tests/test_sharding_gloo.py)."""
+    import socket
+    import torch.distributed as dist
+    dev = torch.device("cuda", 0)
+    w = _bf16_workload("cfg2", nh=2, tokens_per_frame=300, frames_per_chunk=1, n_frames=1)
+    W1, W2, W3 = ti.fast_weights(w)
+    Q, K, V, lr = ti.TokenStream(w).next_chunk()
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1,
+                            device_id=dev)
+    try:
+        gpu = _mk(w)
+        gpu.ttt_init(W1.to(dev), W2.to(dev), W3.to(dev))
+        gpu.ttt_accumulate(K.to(dev), V.to(dev), lr.to(dev))
+        gpu.allreduce_pending_gradient()
+        gpu.ttt_commit()
+        torch.cuda.synchronize()
+        ora = OracleTTT(W1, W2, W3)
+        ora.update(K, V, lr)
+        assert worst_head_weights([x.cpu() for x in gpu.ttt_get_weights()], ora.weights()) <= TOL_BF16
+        gpu.close()
+    finally:
+        dist.destroy_process_group()
+
+
 # ------------------------------------------------------------------------------------------------
 # boundary: no silent CUDA-core fallback
 # ------------------------------------------------------------------------------------------------
