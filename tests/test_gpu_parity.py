@@ -512,6 +512,31 @@ def test_gradient_allreduce_between_accumulate_and_commit_nccl():
         dist.destroy_process_group()
 
 
+@pytest.mark.parametrize("name,reps", [("cfg2", 12), ("cfg3", 12), ("cfg4", 12), ("cfg5", 6)])
+def test_full_size_chunk_step_is_bitwise_repeatable(name, reps):
+    """The same full-size chunk step from the same state, repeated: outputs and fast weights must be
+    bitwise identical every time (north_star: "deterministic under a fixed chunk order"). At full size
+    the update CTAs walk 39-344 token tiles and the pipeline's hand-offs shift from run to run: this is
+    the test that exposes a barrier-protocol race (round 2 found one in the hd 64 update kernel that
+    corrupted one TMEM lane quadrant of one tile in a few launches per hundred)."""
+    dev = torch.device("cuda", 0)
+    w = ti.CONFIGS[name]
+    W1, W2, W3 = (x.to(dev) for x in ti.fast_weights(w))
+    Q, K, V, lr = (x.to(dev) for x in ti.TokenStream(ti.scaled(w, n_frames=w.frames_per_chunk)).next_chunk())
+    t = _mk(w)
+    ref = None
+    for r in range(reps):
+        t.ttt_init(W1, W2, W3)
+        O = t.ttt_chunk_step(Q, K, V, lr)
+        got = [O.clone()] + [x.clone() for x in t.ttt_get_weights()]
+        if ref is None:
+            ref = got
+        else:
+            for a, b in zip(got, ref):
+                assert torch.equal(a, b), (name, r)
+    t.close()
+
+
 # ------------------------------------------------------------------------------------------------
 # boundary: no silent CUDA-core fallback
 # ------------------------------------------------------------------------------------------------
