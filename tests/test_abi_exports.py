@@ -59,3 +59,62 @@ def test_create_argument_checks_run_before_any_cuda_call(lib):
     assert lib.ttt_create(ctypes.byref(ctx), ctypes.byref(resv)) == -1
     assert lib.ttt_launch_count(None) == 0
     lib.ttt_destroy(None)                                                           # NULL is allowed
+
+
+# (nh, hd, hidden, act_dtype, ns_iters, renorm, linear, cuda_core_fallback) -> expected ttt_create outcome.
+# "ok" = the shape passes every check that precedes the device query: the call then returns 0 on a B200
+# and TTT_ERR_CUDA (-7, "device ... does not exist") on a box without one — never a shape status.
+_SHAPES = [
+    # BASELINE.json's five configs
+    ((1, 64, 128, 0, 0, 0, 0, 0), "ok"),      # cfg1: fp32 path
+    ((16, 64, 128, 1, 0, 0, 0, 0), "ok"),     # cfg2
+    ((16, 64, 256, 1, 5, 0, 0, 0), "ok"),     # cfg3
+    ((16, 64, 256, 1, 0, 1, 0, 0), "ok"),     # cfg4
+    ((8, 128, 512, 1, 5, 0, 0, 0), "ok"),     # cfg5
+    # the paper's own shape (Table 3): one head of 1024, k = 1, 2, 4
+    ((1, 1024, 1024, 1, 0, 0, 0, 0), "ok"),
+    ((1, 1024, 2048, 1, 0, 0, 0, 0), "ok"),
+    ((1, 1024, 4096, 1, 0, 0, 0, 0), "ok"),
+    ((2, 256, 384, 1, 0, 0, 0, 0), "ok"),     # large path: hd % 256 == 0, hidden % 128 == 0
+    # hidden sizes that run zero-padded to the next multiple of 128 (k = 1 at hd 64)
+    ((4, 64, 64, 1, 0, 0, 0, 0), "ok"),
+    ((4, 64, 192, 1, 5, 0, 0, 0), "ok"),
+    ((2, 128, 320, 1, 0, 1, 0, 0), "ok"),
+    # explicit CUDA-core route for a shape without a tensor kernel
+    ((2, 64, 512, 1, 0, 0, 0, 1), "ok"),
+    ((2, 32, 64, 1, 0, 0, 0, 1), "ok"),
+    # refused: no tensor kernel and no opt-in
+    ((2, 64, 512, 1, 0, 0, 0, 0), -5),
+    ((2, 32, 64, 1, 0, 0, 0, 0), -5),
+    ((2, 128, 2048, 1, 5, 0, 0, 0), -5),      # hd 128 Newton-Schulz: hidden <= 1024
+    ((2, 64, 32, 0, 5, 0, 0, 0), -5),         # Newton-Schulz needs hidden >= hd
+    # refused: shape outside every path
+    ((1, 1024, 4096, 1, 5, 0, 0, 0), -2),     # large path offers no Newton-Schulz
+    ((1, 1024, 4096, 1, 0, 1, 0, 0), -2),     # ... and no re-normalisation
+    ((1, 1024, 4096, 0, 0, 0, 0, 0), -2),     # fp32 path: hd <= 128
+    ((1, 192, 384, 1, 0, 0, 0, 0), -2),       # hd > 128 must be a multiple of 256
+    ((1, 4096, 4096, 1, 0, 0, 0, 0), -2),     # hd <= 2048
+    ((1, 1024, 1000, 1, 0, 0, 0, 0), -2),     # large path: hidden % 128 == 0
+    ((1, 64, 96, 0, 0, 0, 1, 0), -2),         # linear test mode needs hidden == hd
+    ((1, 64, 130, 1, 0, 0, 0, 0), -2),        # hidden % 4 == 0
+]
+
+
+@pytest.mark.parametrize("shape,expect", _SHAPES)
+def test_supported_shape_set_is_decided_before_the_device_query(lib, shape, expect):
+    """include/ttt.h's shape table (ttt_dtype comment) as data: which configs ttt_create takes and
+    which status the others get. Runs with or without a GPU."""
+    from paper_2604_08542_b200.binding import _Config
+    nh, hd, hidden, dt, ns, renorm, linear, fb = shape
+    cfg = _Config(nh, hd, hidden, dt, ns, renorm, linear, 0, 256, fb, 0)
+    ctx = ctypes.c_void_p()
+    rc = lib.ttt_create(ctypes.byref(ctx), ctypes.byref(cfg))
+    if expect == "ok":
+        assert rc in (0, -7), (rc, lib.ttt_create_error())
+        if rc == 0:
+            lib.ttt_destroy(ctx)
+        else:
+            assert not ctx.value and lib.ttt_create_error()
+    else:
+        assert rc == expect, (rc, lib.ttt_create_error())
+        assert not ctx.value and len(lib.ttt_create_error()) > 0
