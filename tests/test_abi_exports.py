@@ -118,3 +118,42 @@ def test_supported_shape_set_is_decided_before_the_device_query(lib, shape, expe
     else:
         assert rc == expect, (rc, lib.ttt_create_error())
         assert not ctx.value and len(lib.ttt_create_error()) > 0
+
+
+def test_binding_fails_loudly_when_the_library_is_missing(monkeypatch, tmp_path):
+    """No CPU / PyTorch fallback: without the built library the binding raises at load time."""
+    from paper_2604_08542_b200 import binding
+    monkeypatch.setattr(binding, "_lib", None)
+    monkeypatch.setattr(binding, "_LIB_PATH", str(tmp_path / "libttt_b200.so"))
+    with pytest.raises(ImportError, match="no CPU or PyTorch fallback"):
+        binding.load_library()
+    with pytest.raises(ImportError):
+        binding.TTT(nh=1, hd=64, hidden=128)
+
+
+def test_context_creation_fails_loudly_without_a_b200(lib):
+    """On a box without a CUDA device ttt_create returns TTT_ERR_CUDA and the binding raises; nothing
+    routes the call anywhere else (on a B200 the same call succeeds: covered by the -m gpu tests)."""
+    import torch
+    from paper_2604_08542_b200 import binding
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(binding.TTTError) as e:
+        binding.TTT(nh=16, hd=64, hidden=128, max_tokens=1024)
+    assert e.value.status == -7 and "device" in str(e.value)
+
+
+def test_product_package_does_not_reach_for_the_oracle():
+    """oracle/ is test infrastructure: nothing under paper_2604_08542_b200/ imports, opens or links it,
+    and oracle/ does not import the package (the two share only ttt_inputs.py)."""
+    pkg = os.path.join(ROOT, "paper_2604_08542_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                hit = re.search(r"import\s+oracle|from\s+oracle|oracle[/.]|ttt_oracle|libttt_oracle", src)
+                assert hit is None, (os.path.join(dirpath, f), hit.group(0))   # (comments may name it)
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".h")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_2604_08542_b200" not in src and "libttt_b200" not in src, f
