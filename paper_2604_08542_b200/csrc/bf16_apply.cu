@@ -2,12 +2,12 @@
 //   O = ( SiLU(Q W1) o (Q W3) ) W2        Eq. 4 with Eq. 12, updated weights.
 //
 // Formulation ("tokens on lanes"): a CTA owns one head and a strided set of 128-token tiles.
-//   Q tile  -> shared memory by TMA (4-stage ring) -> TMEM as the A operand (bf16 [128 x hd])
+//   Q tile  -> shared memory by TMA (4-stage ring) -> TMEM as the A operand (fp16 [128 x hd], converted from bf16 in registers)
 //   step n  (64 hidden units):  Aq = Q W1[:, n], Bq = Q W3[:, n]   MMA 128 x 64 x hd, B = weights (K-major)
-//            epilogue  Hq = SiLU(Aq) o Bq -> bf16 -> TMEM over its own fp32 source
+//            epilogue  Hq = SiLU(Aq) o Bq -> fp16 -> TMEM over its own fp32 source
 //            O += Hq W2[n, :]                                      MMA 128 x hd x 64, B = W2 slice (MN-major)
 //   O (fp32, TMEM) -> bf16 -> swizzled shared memory -> TMA store (rows beyond M are clipped).
-// The bf16 weights of the head (3 x H x hd) sit in shared memory for the CTA's lifetime (TMA, 128-B
+// The fp16 weights of the head (3 x H x hd) sit in shared memory for the CTA's lifetime (TMA, 128-B
 // swizzle). Forward accumulators, Q operands and O accumulators are double-buffered in TMEM, so the
 // MMA of step n+1 overlaps the SwiGLU epilogue of step n, and Q loads / O stores overlap both.
 //
@@ -33,7 +33,7 @@ constexpr int QL_WARP0 = 24;    // Q: shared -> TMEM (A operand)
 constexpr int QST = 4;         // Q tile ring stages
 constexpr int TILE_BYTES = TM * 128;   // one [128 x 64] bf16 tile
 // TMEM column plan for hd = 64
-constexpr uint32_t C_Q = 0;      // 2 x 32 cols: Q operand (bf16)
+constexpr uint32_t C_Q = 0;      // 2 x 32 cols: Q operand (fp16)
 constexpr uint32_t C_O = 64;     // 64 cols: O accumulator (fp32), single
 constexpr uint32_t C_F = 128;    // 3 x 128 cols: Aq (64) | Bq (64) forward accumulators (fp32)
 constexpr int NF = 3;            // forward buffers: two in the epilogue (one per warpgroup) + one in the MMAs
@@ -58,7 +58,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
   // tiles of this CTA: blockIdx.x, blockIdx.x + gridDim.x, ...
   const int my_tiles = (tiles_total - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
   const int total_steps = my_tiles * nsl;
-  const uint32_t w_bytes = 3u * H * 128u;                    // bf16 weights of the head
+  const uint32_t w_bytes = 3u * H * 128u;                    // fp16 weights of the head
   uint8_t* q_ring = smem + w_bytes;                          // QST x 16 KB
   uint8_t* o_stage = q_ring + QST * TILE_BYTES;              // 2 x 16 KB
 
@@ -210,7 +210,7 @@ bf16_apply_kernel(const __grid_constant__ CUtensorMap mapW, const __grid_constan
           const uint64_t th = pack2(tanh_approx(x0), tanh_approx(x1));
           ph[c >> 1] = pack_f16x2_from2(fmul2(ffma2(hf, th, hf), bb));  // Hq = SiLU(a) b, SiLU(a) = h + h tanh(h)
         }
-        tmem_st_x8(buf + 8 * part, ph);          // Hq (bf16) over Aq columns this thread has already read
+        tmem_st_x8(buf + 8 * part, ph);          // Hq (fp16) over Aq columns this thread has already read
       }
       tc_wait_st();
       tc_fence_before();

@@ -6,7 +6,7 @@
 //   forward   x^T  = (W1/2)^T K^T,  b^T = W3^T K^T,  g0^T = W2 V^T   [128 x T]  (contract over hd)
 //             g = -eta g0 = dHd (dot-product loss: dL/df = -eta v, Eq. 9)
 //   epilogue  th = tanh(x);  S = x + x th = SiLU(a);  t = (1 + th) + S (1 - th) = 2 SiLU'(a)
-//             dA2 = g b t (= 2 dA);  dB = g S;  Hd' = -eta S b                 (fp32 -> bf16)
+//             dA2 = g b t (= 2 dA);  dB = g S;  Hd' = -eta S b                 (fp32 -> fp16)
 //   gradient  2 G1^T += dA2^T K,  G3^T += dB^T K,  G2 += Hd'^T V     [128 x hd] (contract over tokens)
 // The A operand of every MMA lives in TMEM (weights: loaded once, W1 pre-halved (exact) so the
 // accumulator is the tanh argument; dA2/dB/Hd: written by the epilogue over their own fp32 sources),
@@ -25,7 +25,7 @@
 // 16-token K step each; packed fp32x2 math, tanh.approx sigmoid).
 // Pipeline (TMEM is the scarce resource: weights 96 + gradient accumulators 192 columns leave 224):
 // the x | b forward accumulators are double-buffered, g is single-buffered and released first, as
-// soon as an epilogue group has pulled it into registers; the bf16 gradient operands have their own
+// soon as an epilogue group has pulled it into registers; the fp16 gradient operands have their own
 // (single) columns, so nothing aliases; forward and gradient MMAs are issued by different warps —
 // the MMAs of tiles i+1, i+2 overlap the epilogue math of tile i.
 // Measured budget per 32-token tile and SM (B200 microbenchmarks): tensor pipe 384 clk
@@ -54,11 +54,11 @@ constexpr int TILE_BYTES = T * 128;  // one [T x 64] bf16 tile
 constexpr int STAGE_BYTES = 2 * TILE_BYTES;
 
 // TMEM column plan for hd = 64 (512 columns x 128 lanes x 32 bit)
-constexpr uint32_t C_W1 = 0, C_W3 = 32, C_W2 = 64;        // bf16 weights as A operands, 32 cols each
+constexpr uint32_t C_W1 = 0, C_W3 = 32, C_W2 = 64;        // fp16 weights as A operands, 32 cols each
 constexpr uint32_t C_G1 = 96, C_G3 = 160, C_G2 = 224;     // fp32 gradient accumulators, 64 cols each
 constexpr uint32_t C_XB = 288, XB_STRIDE = 64;            // two forward buffers x | b (fp32, 32 cols each)
 constexpr uint32_t C_GG = 416;                            // forward accumulator g (fp32, 32 cols), single
-constexpr uint32_t C_H = 448;                             // bf16 operands dA2 | dB | Hd, 16 cols each, single
+constexpr uint32_t C_H = 448;                             // fp16 operands dA2 | dB | Hd, 16 cols each, single
 }  // namespace upd
 
 template <bool LOSS>
@@ -122,7 +122,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     fence_mbar_init();
   }
   __syncwarp();
-  // epilogue warps request their share of the bf16 weights now (row j of W1^T, W2, W3^T; 16-byte
+  // epilogue warps request their share of the fp16 weights now (row j of W1^T, W2, W3^T; 16-byte
   // chunks 2 tc, 2 tc + 1), so the L2 latency overlaps the TMEM allocation
   uint4 wpre[3][2];
   if (warp >= 4) {
@@ -307,7 +307,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     const size_t me = (size_t)nh * H * HD;
     const size_t row = ((size_t)h * H + (size_t)slice * HS + j) * HD;
     {
-      // weights -> TMEM as A operands: row j of W1^T / 2, W3^T, W2 (64 bf16 = 32 words each); warp
+      // weights -> TMEM as A operands: row j of W1^T / 2, W3^T, W2 (64 fp16 = 32 words each); warp
       // group tc loads 16-byte chunks 2 tc, 2 tc + 1 of each row (8 words = columns 8 tc .. 8 tc + 7)
       const uint32_t cols[3] = {C_W1, C_W2, C_W3};
       uint4 (&x)[3][2] = wpre;           // requested before the TMEM allocation barrier
@@ -448,7 +448,7 @@ bf16_update_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_consta
     // ---- fused commit (Eq. 8): W <- W - sum_s P[s], summed in split order [+ re-normalisation] ----
     // The `gridDim.x` CTAs that share this (head, slice) meet at a counter in global memory (the
     // launch is cooperative: all CTAs are resident), then each commits its share of the slice's
-    // 3 x 128 rows: fp32 master + bf16 operand copy. Deterministic: fixed summation order.
+    // 3 x 128 rows: fp32 master + fp16 operand copy. Deterministic: fixed summation order.
     const int nsplit = gridDim.x;
     if (tid == 0) {
       __threadfence();
@@ -607,9 +607,9 @@ int bf16_update_tensor_path(const ttt_config* cfg) {
   return narrow_tensor_path(cfg) || bf16_update_wide_supported(cfg) || bf16_large_supported(cfg);
 }
 
-// bf16 token tensors are accepted for every shape the fp32 path takes; shapes outside the tcgen05
-// kernels' set (hd = 64, hidden 128 | 256) run on the fp32 CUDA-core kernels behind a bf16 <-> fp32
-// conversion (same semantics, fp32 arithmetic).
+// Shapes the bf16 <-> fp32 conversion in front of the fp32 CUDA-core kernels can take at all; whether a
+// bf16 shape is ACCEPTED is decided in ttt_create: a tcgen05 kernel exists (bf16_*_tensor_path), or the
+// caller opted in with cfg.cuda_core_fallback (same semantics, fp32 arithmetic).
 int bf16_supported(const ttt_config* cfg, char* why, size_t why_len) {
   if (cfg->linear_fast_weight) { snprintf(why, why_len, "bf16 path: linear test mode is f32-only"); return 0; }
   if (cfg->hd % 8 != 0) { snprintf(why, why_len, "bf16 path: hd must be a multiple of 8 (got %d)", cfg->hd); return 0; }

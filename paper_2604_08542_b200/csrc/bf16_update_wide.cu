@@ -7,7 +7,7 @@
 // 128-hidden slice take 3 x 128 = 384 of the 512 columns, so
 //   * the weights stay in shared memory (A operands of SS-mode MMAs, 96 KB per slice),
 //   * the forward accumulators x | b | g of one 32-token tile are single-buffered (96 columns),
-//   * the bf16 operand Hd' of the W2 gradient re-uses the columns of x; the MMA order
+//   * the fp16 operand Hd' of the W2 gradient re-uses the columns of x; the MMA order
 //     b(i+1) g(i+1) | G2(i) | x(i+1) | commit | G1(i) G3(i) keeps the tensor pipe busy while the epilogue
 //     of tile i+1 loads its accumulators and makes the overwrite of x safe (MMAs of one thread execute
 //     in issue order). Measured: the issuing thread is stalled by pipe back-pressure 80 % of the time,
@@ -35,7 +35,7 @@ constexpr int THREADS = (4 + EPI_WARPS + CVT_WARPS - 2) * 32;
 constexpr int SUB_BYTES = T * 128;          // one [T x 64] bf16 sub-tile (half of hd), 128-B swizzled
 constexpr int TILE_BYTES = 2 * SUB_BYTES;   // K or V tile
 constexpr int STAGE_BYTES = 2 * TILE_BYTES;
-constexpr int WSUB_BYTES = HS * 128;        // one [128 x 64] bf16 weight sub-tile
+constexpr int WSUB_BYTES = HS * 128;        // one [128 x 64] fp16 weight sub-tile
 constexpr int WMAT_BYTES = 2 * WSUB_BYTES;
 constexpr int W_BYTES = 3 * WMAT_BYTES;
 constexpr int SLD = 64 + 4;                 // flush staging row stride (floats)
@@ -45,8 +45,8 @@ constexpr size_t SMEM_BYTES = (size_t)W_BYTES + (size_t)STAGES * STAGE_BYTES + S
 // TMEM column plan (512 columns x 128 lanes x 32 bit)
 constexpr uint32_t C_G1 = 0, C_G3 = 128, C_G2 = 256;   // fp32 gradient accumulators [hidden][hd]
 constexpr uint32_t C_X = 384, C_B = 416, C_G = 448;    // fp32 forward accumulators [hidden][token]
-constexpr uint32_t C_OA = 480, C_OB = 496;             // bf16 operands 2 dA, dB [hidden][token], 16 cols
-constexpr uint32_t C_OH = C_X;                         // bf16 operand Hd' = -eta Hd, over the dead x
+constexpr uint32_t C_OA = 480, C_OB = 496;             // fp16 operands 2 dA, dB [hidden][token], 16 cols
+constexpr uint32_t C_OH = C_X;                         // fp16 operand Hd' = -eta Hd, over the dead x
 }  // namespace updw
 
 // Work distribution: the (head, slice) pairs x 32-token tiles form one list of units, pair-major; CTA c
@@ -479,7 +479,7 @@ int bf16_accumulate_wide(ttt_ctx* ctx, const __nv_bfloat16* K, const __nv_bfloat
   if (rc != TTT_OK) return rc;
   rc = make_token_map(ctx, &mapV, V, M, (int64_t)c.nh * c.hd, ld, updw::T);
   if (rc != TTT_OK) return rc;
-  // bf16 operand copy of the weights as one [3 nh H][hd] matrix, boxes of [128 rows][64]
+  // fp16 operand copy of the weights as one [3 nh H][hd] matrix, boxes of [128 rows][64]
   rc = make_token_map(ctx, &mapW, ctx->Wb, (int64_t)3 * c.nh * c.hidden, c.hd, c.hd, updw::HS);
   if (rc != TTT_OK) return rc;
   if (!(ctx->attr_done & ATTR_UPDW)) {
